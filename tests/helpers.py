@@ -33,7 +33,7 @@ def arm(n=3, gravity=(0, 0, -9.81), damping=0.0, with_contacts=False, slide_last
     caps = []
     for i in range(n):
         quat = np.array([1.0, 0.1 * i, -0.05, 0.07 * i]); quat /= np.linalg.norm(quat)
-        b = mb.body(parent, pos=(0.05, 0.02 * i, 0.3 if i else 0.4), quat=tuple(quat), mass=1.0 + 0.5 * i,
+        b = mb.body(parent, pos=(0.05, 0.02 * i, 0.3 if i else (0.12 if with_contacts else 0.4)), quat=tuple(quat), mass=1.0 + 0.5 * i,
                     ipos=(0.01, 0.02, 0.12), iquat=(math.cos(0.3), 0, math.sin(0.3), 0), inertia_unit=(0.01, 0.02, 0.005))
         jt = W.JNT_SLIDE if (slide_last and i == n - 1) else W.JNT_HINGE
         mb.joint(b, jt, axis=axes[i % 4], pos=(0.0, 0.01, -0.02), damping=damping, armature=0.01 * (i == 1))
