@@ -1,0 +1,165 @@
+/* dmx.h — C-ABI of the B200-native DiffMJX hot path (arxiv 2506.14186).
+ *
+ * Batched adaptive-step rollouts of a MuJoCo-style penalty-contact rigid-body simulator over
+ * independent environments, and the reverse-mode gradient of a terminal loss through the
+ * accepted steps with Contacts From Distance (CFD) applied only in the backward pass.
+ * Every step of the path runs in hand-written CUDA kernels (sm_100a); there is no CPU fallback.
+ *
+ * Conventions
+ *   - "host" / "device" says where a pointer must live.  All device buffers and the CUDA
+ *     stream are owned by the caller; the library owns only the dmx_model.
+ *   - Batched arrays are env-major and row-contiguous.  Element type `real` is double for a
+ *     model created with precision 64 and float for precision 32 (x0, ctrl, params, xT, dLd*,
+ *     tape); h_replay and all statistics are always double / int.
+ *   - State x = [q | v]: q[nq] (free joint: 3 position + unit quaternion
+ *     w,x,y,z; hinge / slide: one scalar), v[nv] (free joint: world linear, body angular).
+ *   - Calls only enqueue work on `cuda_stream`; they do not synchronise.  One call may be in
+ *     flight per dmx_model at a time (the model owns the work-queue counters and scratch).
+ *   - Return value: 0 ok; <0 invalid argument / CUDA error (text via dmx_last_error()).
+ *     Numerical trouble inside one environment never fails a call, it is reported in
+ *     stats.status[e]: 0 ok, 1 step budget exceeded, 2 step-size
+ *     underflow, 3 non-finite, 4 tape full.  A failed environment returns its last accepted
+ *     state and zero gradients.
+ */
+#ifndef DMX_H
+#define DMX_H
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { DMX_JNT_FREE = 0, DMX_JNT_HINGE = 1, DMX_JNT_SLIDE = 2 };
+enum { DMX_GEOM_PLANE = 0, DMX_GEOM_SPHERE = 1, DMX_GEOM_CAPSULE = 2, DMX_GEOM_BOX = 3 };
+enum { DMX_ACT_MOTOR = 0, DMX_ACT_PD = 1 };
+enum { DMX_DOPRI5 = 0, DMX_TSIT5 = 1 };
+
+typedef struct dmx_model dmx_model; /* opaque; owns device copies of the constants */
+
+/* Model description: flattened kinematic tree, geoms, solref/solimp, friction
+ * (BASELINE.json north_star; PAPER.md:41-45 state and dynamics, :51 collision, :58-68 Eq. 3,
+ * impedance and regulariser).  All pointers are HOST pointers, copied at create.
+ * Restrictions: body 0 is the world; body_parent[b] < b; at most one joint per body; free
+ * joints only on children of the world; planes on the world body and first in a pair;
+ * supported pairs: plane-sphere, plane-capsule (two end caps), plane-box (eight corners),
+ * sphere-sphere (north_star subsystem 2). */
+typedef struct {
+  int nbody, njnt, nq, nv, nu, ngeom, npair;
+  const int *body_parent;                                   /* [nbody]                        */
+  const double *body_pos, *body_quat;                       /* [nbody*3], [nbody*4] in parent  */
+  const double *body_mass;                                  /* [nbody]                        */
+  const double *body_ipos, *body_iquat;                     /* inertial frame in the body     */
+  const double *body_inertia_unit;                          /* [nbody*3] principal inertia per unit mass */
+  const int *jnt_type, *jnt_body, *jnt_qadr, *jnt_vadr;     /* [njnt]                         */
+  const double *jnt_axis, *jnt_pos;                         /* [njnt*3] in the body frame      */
+  const double *jnt_damping, *jnt_armature;                 /* [njnt]                         */
+  const int *geom_type, *geom_body;                         /* [ngeom]                        */
+  const double *geom_size, *geom_pos, *geom_quat;           /* [ngeom*3], [ngeom*3], [ngeom*4] */
+  const int *pair_geom1, *pair_geom2, *pair_condim;         /* [npair]; condim 1 or 3 (pyramidal) */
+  const double *pair_friction;                              /* [npair]                        */
+  const double *pair_solref;                                /* [npair*2] (timeconst, dampratio), Eq. 3 */
+  const double *pair_solimp;                                /* [npair*5] (d_o,d_w,w,mid,power) */
+  const double *pair_solimp_cfd;                            /* [npair*5] (d_c,d_0,w_c,m_c,p_c) */
+  const double *pair_cfd_beta;                              /* [npair] softplus sharpness */
+  const int *act_type, *act_jnt;                            /* [nu]                           */
+  const double *act_gear, *act_kp, *act_kd;                 /* [nu]                           */
+  double gravity[3];
+  int newton_iters, ls_iters;                               /* fixed iteration scheme */
+  const double *qpos0;                                      /* [nq] reference pose for the diagonal approximation
+                                                               A^ of J M^-1 J^T   */
+} dmx_model_desc;
+
+/* Adaptive embedded Runge-Kutta options (Tsit5 / Dopri5 and the PID controller
+ * with P=0.2, I=0.4, D=0 at PAPER.md:347). */
+typedef struct {
+  int tableau;          /* DMX_DOPRI5 | DMX_TSIT5 */
+  double rtol, atol;    /* error = sqrt(mean((e_j / (atol + rtol*max(|y_n|,|y_n+1|)_j))^2)), accept iff <= 1 */
+  double h0;            /* initial step proposal */
+  double pcoeff, icoeff, safety, fac_min, fac_max;
+  int max_steps;        /* budget of attempted steps per environment */
+} dmx_solver_opts;
+
+/* Per-environment step statistics; DEVICE pointers, each [nenv]; any may be NULL. */
+typedef struct {
+  int *n_accept, *n_reject, *n_feval, *n_newton_unconverged, *status;
+  double *h_min, *h_max, *t_end;
+} dmx_stats;
+
+/* Builds the device model.  precision: 64 (double) or 32 (float stage arithmetic; time, step
+ * size, error norm, controller and state accumulation stay fp64).  Synchronises the device.
+ * Returns 0 and *out on success. */
+int dmx_model_create(const dmx_model_desc *desc, int precision, dmx_model **out);
+void dmx_model_destroy(dmx_model *m);
+
+/* Sizes derived at create.  np = nbody + 8*npair: parameter vector
+ * p = [body_mass(nbody) | pair_friction(npair) | pair_solref(2*npair) | pair_solimp(5*npair)];
+ * inertia = mass * inertia_unit.  nc = flattened candidate contacts. */
+int dmx_model_np(const dmx_model *m);
+int dmx_model_nc(const dmx_model *m);
+/* Copies the default parameter vector ([np] doubles) to a HOST buffer. */
+int dmx_model_default_params(const dmx_model *m, double *p_host);
+/* Lanes per environment the kernels use for this model (1, 8, 16 or 32). */
+int dmx_model_lanes(const dmx_model *m);
+
+/* Bytes of tape for nenv environments with room for tape_steps accepted steps each
+ * (checkpoint record = (y_n, t_n, h_n): (nq+nv+2) reals). */
+size_t dmx_tape_bytes(const dmx_model *m, int nenv, int tape_steps);
+
+/* Forward rollout (PAPER.md:41 x_{k+1}=step(x_k,a_k,p); Eq. 5 at PAPER.md:422-425): integrates
+ * every environment from t=0 to `horizon` with its own error-controlled step size
+ * (PAPER.md:98, 493).
+ *   x0      device [nenv, nq+nv] real
+ *   ctrl    device [nenv, nknot, nu] real, zero-order hold with knot spacing knot_dt; NULL if nu==0
+ *   params  device [nenv, np] real, or NULL for the model defaults
+ *   h_replay device [nenv, n_replay] double or NULL: if given, exactly these steps are taken
+ *           (a non-positive entry ends the rollout), no error control
+ *   xT      device [nenv, nq+nv] real (out)
+ *   stats   device arrays (out), may be NULL
+ *   tape    device buffer of tape_bytes, or NULL for no tape */
+int dmx_rollout(const dmx_model *m, int nenv, const void *x0, const void *ctrl, int nknot, double knot_dt,
+                const void *params, double horizon, const dmx_solver_opts *opts, const double *h_replay,
+                int n_replay, void *xT, const dmx_stats *stats, void *tape, size_t tape_bytes,
+                void *cuda_stream);
+
+/* Forward rollout with tape, then the reverse sweep through the accepted steps with frozen
+ * step sizes (discretize-then-optimize).  With cfd_on the vector-Jacobian
+ * products are those of the CFD field F~ evaluated on the unmodified trajectory
+ * (straight-through estimator, Eq. 4); xT, stats and tape do not depend on
+ * cfd_on.
+ *   dLdxT     device [nenv, nq+nv] real, ambient gradient of the loss at x_T
+ *   dLdx0     device [nenv, 2*nv] real (out), tangent coordinates (translations world frame,
+ *             rotations body frame)
+ *   dLdctrl   device [nenv, nknot, nu] real (out) or NULL
+ *   dLdparams device [nenv, np] real (out) or NULL (skips the parameter directions)
+ *   tape      device buffer, required */
+int dmx_rollout_grad(const dmx_model *m, int nenv, const void *x0, const void *ctrl, int nknot, double knot_dt,
+                     const void *params, double horizon, const dmx_solver_opts *opts, const double *h_replay,
+                     int n_replay, const void *dLdxT, int cfd_on, void *xT, void *dLdx0, void *dLdctrl,
+                     void *dLdparams, const dmx_stats *stats, void *tape, size_t tape_bytes, void *cuda_stream);
+
+/* Reverse sweep only, over a tape written by dmx_rollout with the same inputs. */
+int dmx_rollout_backward(const dmx_model *m, int nenv, const void *ctrl, int nknot, const void *params,
+                         const dmx_solver_opts *opts, const void *xT, const void *dLdxT, int cfd_on,
+                         void *dLdx0, void *dLdctrl, void *dLdparams, const int *status /* device [nenv] or NULL */,
+                         const void *tape, size_t tape_bytes, void *cuda_stream);
+
+/* Building blocks exposed for parity tests (one lane-group per state, same device code as the
+ * rollouts).  All pointers DEVICE, real typed; n states.
+ *   dmx_vector_field: acc[n,nv] = F(q,v,u,p) or F~ when cfd (Eq. 1, 2, 4); nrow[n] rows in the solve.
+ *   dmx_vjp_field: (qbar,vbar,ubar,pbar) = kappa^T dF/d(q,v,u,p). */
+int dmx_vector_field(const dmx_model *m, int n, const void *x, const void *u, const void *params, int cfd,
+                     void *acc, int *nrow, void *cuda_stream);
+int dmx_vjp_field(const dmx_model *m, int n, const void *x, const void *u, const void *params, const void *kappa,
+                  int cfd, void *qbar, void *vbar, void *ubar, void *pbar, void *cuda_stream);
+
+/* FP64 / FP32 FMA-chain microbenchmark used for the roofline denominator:
+ * runs `iters` dependent-chain FMAs x 8 chains per thread on the whole chip and returns the
+ * measured FLOP/s (2 per FMA) in *flops_per_s.  Synchronises. */
+int dmx_fma_peak(int precision, int iters, double *flops_per_s, double *ms);
+
+const char *dmx_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DMX_H */

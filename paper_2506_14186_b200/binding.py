@@ -1,0 +1,254 @@
+"""Thin Python binding of the C-ABI in include/dmx.h (argument marshalling only).
+
+PyTorch is used for device memory and the CUDA stream; every step of the path runs in the CUDA
+kernels of libdmx.so.  There is no CPU fallback: importing works without a GPU (so that the symbol
+table can be checked), but any call that computes raises if the library or a device is missing.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdmx.so")
+
+SYMBOLS = ["dmx_model_create", "dmx_model_destroy", "dmx_model_np", "dmx_model_nc", "dmx_model_default_params",
+           "dmx_model_lanes", "dmx_tape_bytes", "dmx_rollout", "dmx_rollout_grad", "dmx_rollout_backward",
+           "dmx_vector_field", "dmx_vjp_field", "dmx_fma_peak", "dmx_last_error"]
+
+_pd, _pi = C.POINTER(C.c_double), C.POINTER(C.c_int)
+_INT_FIELDS = ["nbody", "njnt", "nq", "nv", "nu", "ngeom", "npair"]
+_PTR_FIELDS = [
+    ("body_parent", "i"), ("body_pos", "d"), ("body_quat", "d"), ("body_mass", "d"), ("body_ipos", "d"),
+    ("body_iquat", "d"), ("body_inertia_unit", "d"),
+    ("jnt_type", "i"), ("jnt_body", "i"), ("jnt_qadr", "i"), ("jnt_vadr", "i"),
+    ("jnt_axis", "d"), ("jnt_pos", "d"), ("jnt_damping", "d"), ("jnt_armature", "d"),
+    ("geom_type", "i"), ("geom_body", "i"), ("geom_size", "d"), ("geom_pos", "d"), ("geom_quat", "d"),
+    ("pair_geom1", "i"), ("pair_geom2", "i"), ("pair_condim", "i"),
+    ("pair_friction", "d"), ("pair_solref", "d"), ("pair_solimp", "d"), ("pair_solimp_cfd", "d"), ("pair_cfd_beta", "d"),
+    ("act_type", "i"), ("act_jnt", "i"), ("act_gear", "d"), ("act_kp", "d"), ("act_kd", "d"),
+]
+
+
+class ModelDesc(C.Structure):
+    _fields_ = ([(n, C.c_int) for n in _INT_FIELDS] + [(n, _pi if t == "i" else _pd) for n, t in _PTR_FIELDS] +
+                [("gravity", C.c_double * 3), ("newton_iters", C.c_int), ("ls_iters", C.c_int), ("qpos0", _pd)])
+
+
+class SolverOpts(C.Structure):
+    _fields_ = [("tableau", C.c_int), ("rtol", C.c_double), ("atol", C.c_double), ("h0", C.c_double),
+                ("pcoeff", C.c_double), ("icoeff", C.c_double), ("safety", C.c_double), ("fac_min", C.c_double),
+                ("fac_max", C.c_double), ("max_steps", C.c_int)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("n_accept", C.c_void_p), ("n_reject", C.c_void_p), ("n_feval", C.c_void_p),
+                ("n_newton_unconverged", C.c_void_p), ("status", C.c_void_p),
+                ("h_min", C.c_void_p), ("h_max", C.c_void_p), ("t_end", C.c_void_p)]
+
+
+_lib = None
+
+
+def load():
+    """dlopen libdmx.so (built in-tree by build.py); raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("libdmx.so not built: run `python -m paper_2506_14186_b200.build` (no CPU fallback exists)")
+        L = C.CDLL(LIB_PATH)
+        L.dmx_last_error.restype = C.c_char_p
+        L.dmx_tape_bytes.restype = C.c_size_t
+        L.dmx_tape_bytes.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.dmx_model_create.argtypes = [C.POINTER(ModelDesc), C.c_int, C.POINTER(C.c_void_p)]
+        L.dmx_model_destroy.argtypes = [C.c_void_p]
+        for f in ("dmx_model_np", "dmx_model_nc", "dmx_model_lanes"):
+            getattr(L, f).argtypes = [C.c_void_p]
+        L.dmx_model_default_params.argtypes = [C.c_void_p, C.c_void_p]
+        vp, i, d, sz = C.c_void_p, C.c_int, C.c_double, C.c_size_t
+        L.dmx_rollout.argtypes = [vp, i, vp, vp, i, d, vp, d, C.POINTER(SolverOpts), vp, i, vp, C.POINTER(Stats), vp, sz, vp]
+        L.dmx_rollout_grad.argtypes = [vp, i, vp, vp, i, d, vp, d, C.POINTER(SolverOpts), vp, i, vp, i, vp, vp, vp, vp,
+                                       C.POINTER(Stats), vp, sz, vp]
+        L.dmx_rollout_backward.argtypes = [vp, i, vp, i, vp, C.POINTER(SolverOpts), vp, vp, i, vp, vp, vp, vp, vp, sz, vp]
+        L.dmx_vector_field.argtypes = [vp, i, vp, vp, vp, i, vp, vp, vp]
+        L.dmx_vjp_field.argtypes = [vp, i, vp, vp, vp, vp, i, vp, vp, vp, vp, vp]
+        L.dmx_fma_peak.argtypes = [i, i, _pd, _pd]
+        _lib = L
+    return _lib
+
+
+def _err():
+    return load().dmx_last_error().decode()
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("dmx needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _opts(o):
+    return SolverOpts(int(o["tableau"]), o["rtol"], o["atol"], o["h0"], o["pcoeff"], o["icoeff"], o["safety"],
+                      o["fac_min"], o["fac_max"], int(o["max_steps"]))
+
+
+def fma_peak(precision=64, iters=1 << 16):
+    """Measured FMA-chain peak (FLOP/s) of the CUDA cores; roofline denominator."""
+    _torch()
+    f, ms = C.c_double(0), C.c_double(0)
+    if load().dmx_fma_peak(int(precision), int(iters), C.byref(f), C.byref(ms)) != 0:
+        raise RuntimeError("dmx_fma_peak: " + _err())
+    return f.value, ms.value
+
+
+class Model:
+    """dmx_model handle.  `model` is the dict of flat arrays built by workloads.ModelBuilder."""
+
+    def __init__(self, model, precision=64, device="cuda:0"):
+        self.torch = _torch()
+        self.device = self.torch.device(device)
+        self.torch.cuda.set_device(self.device)
+        L = load()
+        d = ModelDesc()
+        keep = []
+        for n in _INT_FIELDS:
+            setattr(d, n, int(model[n]))
+        for n, t in _PTR_FIELDS:
+            a = np.ascontiguousarray(model[n], dtype=np.int32 if t == "i" else np.float64)
+            keep.append(a)
+            setattr(d, n, a.ctypes.data_as(_pi if t == "i" else _pd))
+        for k in range(3):
+            d.gravity[k] = float(model["gravity"][k])
+        d.newton_iters, d.ls_iters = int(model["newton_iters"]), int(model["ls_iters"])
+        q0 = np.ascontiguousarray(model["qpos0"], dtype=np.float64)
+        d.qpos0 = q0.ctypes.data_as(_pd)
+        h = C.c_void_p()
+        if L.dmx_model_create(C.byref(d), int(precision), C.byref(h)) != 0:
+            raise RuntimeError("dmx_model_create: " + _err())
+        self.h = h
+        self.precision = int(precision)
+        self.dtype = self.torch.float64 if precision == 64 else self.torch.float32
+        self.nq, self.nv, self.nu = int(model["nq"]), int(model["nv"]), int(model["nu"])
+        self.np_ = L.dmx_model_np(h)
+        self.nc = L.dmx_model_nc(h)
+        self.lanes = L.dmx_model_lanes(h)
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            load().dmx_model_destroy(self.h)
+            self.h = None
+
+    def default_params(self):
+        p = np.zeros(self.np_)
+        load().dmx_model_default_params(self.h, p.ctypes.data_as(C.c_void_p))
+        return p
+
+    def tape_bytes(self, nenv, tape_steps):
+        return int(load().dmx_tape_bytes(self.h, int(nenv), int(tape_steps)))
+
+    # ---- helpers -------------------------------------------------------------------------------
+    def dev(self, a, dtype=None):
+        """numpy / tensor -> contiguous device tensor of the model's real type (None passes through)."""
+        if a is None:
+            return None
+        t = self.torch.as_tensor(a)
+        return t.to(device=self.device, dtype=dtype or self.dtype).contiguous()
+
+    def alloc_stats(self, nenv):
+        T = self.torch
+        s = dict(n_accept=T.zeros(nenv, dtype=T.int32, device=self.device), n_reject=T.zeros(nenv, dtype=T.int32, device=self.device),
+                 n_feval=T.zeros(nenv, dtype=T.int32, device=self.device),
+                 n_newton_unconverged=T.zeros(nenv, dtype=T.int32, device=self.device),
+                 status=T.zeros(nenv, dtype=T.int32, device=self.device),
+                 h_min=T.zeros(nenv, dtype=T.float64, device=self.device), h_max=T.zeros(nenv, dtype=T.float64, device=self.device),
+                 t_end=T.zeros(nenv, dtype=T.float64, device=self.device))
+        return s
+
+    @staticmethod
+    def _stats_struct(s):
+        if s is None:
+            return None
+        return Stats(*[s[k].data_ptr() for k in ("n_accept", "n_reject", "n_feval", "n_newton_unconverged", "status",
+                                                 "h_min", "h_max", "t_end")])
+
+    def alloc_tape(self, nenv, tape_steps):
+        return self.torch.empty(self.tape_bytes(nenv, tape_steps), dtype=self.torch.uint8, device=self.device)
+
+    def _stream(self, stream):
+        s = stream if stream is not None else self.torch.cuda.current_stream(self.device)
+        return C.c_void_p(s.cuda_stream)
+
+    # ---- the C-ABI calls (device tensors in, device tensors out) ---------------------------------
+    def rollout(self, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay=None, xT=None, stats=None, tape=None, stream=None):
+        nenv = x0.shape[0]
+        xT = self.torch.empty_like(x0) if xT is None else xT
+        st = self._stats_struct(stats)
+        o = _opts(opts)
+        nrep = 0 if h_replay is None else h_replay.shape[1]
+        rc = load().dmx_rollout(self.h, nenv, _ptr(x0), _ptr(ctrl), int(nknot), float(knot_dt), _ptr(params), float(horizon), C.byref(o),
+                                _ptr(h_replay), nrep, _ptr(xT), C.byref(st) if st else None, _ptr(tape),
+                                0 if tape is None else tape.numel(), self._stream(stream))
+        if rc != 0:
+            raise RuntimeError("dmx_rollout: " + _err())
+        return xT
+
+    def rollout_backward(self, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, tape, want_params=True, status=None, stream=None,
+                         out=None):
+        T = self.torch
+        nenv = xT.shape[0]
+        if out is None:
+            out = dict(dLdx0=T.empty((nenv, 2 * self.nv), dtype=self.dtype, device=self.device),
+                       dLdctrl=T.empty((nenv, nknot, self.nu), dtype=self.dtype, device=self.device) if (ctrl is not None and nknot > 0) else None,
+                       dLdparams=T.empty((nenv, self.np_), dtype=self.dtype, device=self.device) if want_params else None)
+        o = _opts(opts)
+        rc = load().dmx_rollout_backward(self.h, nenv, _ptr(ctrl), int(nknot), _ptr(params), C.byref(o), _ptr(xT), _ptr(dLdxT), int(cfd_on),
+                                         _ptr(out["dLdx0"]), _ptr(out["dLdctrl"]), _ptr(out["dLdparams"]), _ptr(status), _ptr(tape),
+                                         tape.numel(), self._stream(stream))
+        if rc != 0:
+            raise RuntimeError("dmx_rollout_backward: " + _err())
+        return out
+
+    def rollout_grad(self, x0, ctrl, nknot, knot_dt, params, horizon, opts, dLdxT, cfd_on, tape, h_replay=None, want_params=True,
+                     stats=None, stream=None, out=None):
+        T = self.torch
+        nenv = x0.shape[0]
+        if out is None:
+            out = dict(xT=T.empty_like(x0), dLdx0=T.empty((nenv, 2 * self.nv), dtype=self.dtype, device=self.device),
+                       dLdctrl=T.empty((nenv, nknot, self.nu), dtype=self.dtype, device=self.device) if (ctrl is not None and nknot > 0) else None,
+                       dLdparams=T.empty((nenv, self.np_), dtype=self.dtype, device=self.device) if want_params else None)
+        st = self._stats_struct(stats)
+        o = _opts(opts)
+        nrep = 0 if h_replay is None else h_replay.shape[1]
+        rc = load().dmx_rollout_grad(self.h, nenv, _ptr(x0), _ptr(ctrl), int(nknot), float(knot_dt), _ptr(params), float(horizon), C.byref(o),
+                                     _ptr(h_replay), nrep, _ptr(dLdxT), int(cfd_on), _ptr(out["xT"]), _ptr(out["dLdx0"]), _ptr(out["dLdctrl"]),
+                                     _ptr(out["dLdparams"]), C.byref(st) if st else None, _ptr(tape), tape.numel(), self._stream(stream))
+        if rc != 0:
+            raise RuntimeError("dmx_rollout_grad: " + _err())
+        return out
+
+    def vector_field(self, x, u=None, params=None, cfd=False, stream=None):
+        T = self.torch
+        n = x.shape[0]
+        acc = T.empty((n, self.nv), dtype=self.dtype, device=self.device)
+        nrow = T.zeros(n, dtype=T.int32, device=self.device)
+        rc = load().dmx_vector_field(self.h, n, _ptr(x), _ptr(u), _ptr(params), int(cfd), _ptr(acc), _ptr(nrow), self._stream(stream))
+        if rc != 0:
+            raise RuntimeError("dmx_vector_field: " + _err())
+        return acc, nrow
+
+    def vjp_field(self, x, u, params, kappa, cfd=False, want_params=True, stream=None):
+        T = self.torch
+        n = x.shape[0]
+        mk = lambda k: T.empty((n, max(k, 1)), dtype=self.dtype, device=self.device)
+        qb, vb, ub = mk(self.nv), mk(self.nv), mk(self.nu)
+        pb = mk(self.np_) if want_params else None
+        rc = load().dmx_vjp_field(self.h, n, _ptr(x), _ptr(u), _ptr(params), _ptr(kappa), int(cfd), _ptr(qb), _ptr(vb), _ptr(ub), _ptr(pb),
+                                  self._stream(stream))
+        if rc != 0:
+            raise RuntimeError("dmx_vjp_field: " + _err())
+        return qb, vb, ub[:, :self.nu], pb

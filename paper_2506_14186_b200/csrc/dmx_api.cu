@@ -1,0 +1,540 @@
+// dmx_api.cu — the C-ABI of include/dmx.h: model flattening and upload, workspace layouts, kernel
+// dispatch.  Host code only prepares constants and launches; every step of the path (S1-S12 of
+// SURVEY.md §8(a)) runs in the kernels of dmx_kernels.cuh.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <cmath>
+#include <string>
+#include <vector>
+#include <stdexcept>
+#include "../../include/dmx.h"
+#include "dmx_kernels.cuh"
+
+using namespace dmx;
+
+static thread_local char g_err[512] = "";
+static int fail(const char* fmt, const char* a = "") { std::snprintf(g_err, sizeof(g_err), fmt, a); return -1; }
+#define CUDA_OK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return fail("CUDA error: %s", cudaGetErrorString(e_)); } while (0)
+
+namespace {
+
+// ---- dispatch table over (real type, lanes) ----------------------------------------------------------
+template <class R> struct Launchers {
+  cudaError_t (*rollout)(const ModelDev<R>&, const RolloutArgs<R>&, LaunchCfg, cudaStream_t);
+  cudaError_t (*backward)(const ModelDev<R>&, const BackwardArgs<R>&, LaunchCfg, cudaStream_t);
+  cudaError_t (*field)(const ModelDev<R>&, const FieldArgs<R>&, LaunchCfg, cudaStream_t);
+  cudaError_t (*invweight)(const ModelDev<R>&, const R*, const R*, R*, const WsLayout&, const RkLayout&, LaunchCfg, cudaStream_t);
+  cudaError_t (*occupancy)(int, size_t, size_t, int*, int*);
+};
+template <class R, int G> Launchers<R> make_launchers() {
+  Launchers<R> l;
+  l.rollout = &launch_rollout<R, G>; l.backward = &launch_backward<R, G>; l.field = &launch_field<R, G>;
+  l.invweight = &launch_invweight<R, G>; l.occupancy = &kernel_occupancy<R, G>;
+  return l;
+}
+template <class R> Launchers<R> launchers_for(int G) {
+  switch (G) {
+    case 1: return make_launchers<R, 1>();
+    case 8: return make_launchers<R, 8>();
+    case 16: return make_launchers<R, 16>();
+    default: return make_launchers<R, 32>();
+  }
+}
+
+// ---- device arena: one allocation holding every constant array ------------------------------------------
+struct Arena {
+  std::vector<unsigned char> host; unsigned char* dev = nullptr;
+  size_t add(const void* p, size_t bytes) {
+    size_t off = (host.size() + 15) & ~size_t(15);
+    host.resize(off + bytes);
+    if (bytes) std::memcpy(host.data() + off, p, bytes);
+    return off;
+  }
+};
+
+struct HostModel {   // flattened description, doubles
+  int nbody, njnt, nq, nv, nu, npair, nc, np, nlevel, ntw, nmp, nrmax, newton_iters, ls_iters;
+  std::vector<int> body_parent, body_jnt, level_ptr, level_body, jnt_type, jnt_qadr, jnt_vadr, jnt_body, dof_jnt, dof_body, dof_rot,
+      tw_ptr, tw_body, tw_dof, tw_idx, sub_ptr, sub_body, mp_i, mp_j, mp_deep, ct_kind, ct_b1, ct_b2, ct_condim, ct_pair, act_type, act_jnt;
+  std::vector<double> body_pos, body_rot, body_ipos, body_irot, body_iunit, jnt_axis, jnt_pos, jnt_damping, jnt_armature, ct_p1, ct_p2,
+      ct_rho1, ct_rho2, ct_n, ct_t1, ct_t2, pair_invweight, pair_solimp_cfd, pair_cfd_beta, act_gear, act_kp, act_kd, p_default, qpos0;
+  std::vector<int> pair_body1, pair_body2;
+  double gravity[3];
+};
+
+void quat_rot(const double* q, double* Rm) {   // rotation matrix (row-major) of a quaternion (w,x,y,z)
+  double w = q[0], x = q[1], y = q[2], z = q[3];
+  Rm[0] = w * w + x * x - y * y - z * z; Rm[1] = 2 * (x * y - w * z); Rm[2] = 2 * (x * z + w * y);
+  Rm[3] = 2 * (x * y + w * z); Rm[4] = w * w - x * x + y * y - z * z; Rm[5] = 2 * (y * z - w * x);
+  Rm[6] = 2 * (x * z - w * y); Rm[7] = 2 * (y * z + w * x); Rm[8] = w * w - x * x - y * y + z * z;
+}
+void mat_vec(const double* Rm, const double* v, double* o) { for (int i = 0; i < 3; ++i) o[i] = Rm[3 * i] * v[0] + Rm[3 * i + 1] * v[1] + Rm[3 * i + 2] * v[2]; }
+
+template <class T> std::vector<T> cpv(const T* p, size_t n) { return p ? std::vector<T>(p, p + n) : std::vector<T>(n, T(0)); }
+
+void flatten(const dmx_model_desc* d, HostModel& h) {
+  h.nbody = d->nbody; h.njnt = d->njnt; h.nq = d->nq; h.nv = d->nv; h.nu = d->nu; h.npair = d->npair;
+  h.newton_iters = d->newton_iters; h.ls_iters = d->ls_iters;
+  for (int k = 0; k < 3; ++k) h.gravity[k] = d->gravity[k];
+  const int nb = h.nbody, nv = h.nv;
+  if (nb < 1 || nv < 1 || h.nq < nv) throw std::runtime_error("empty model");
+  h.np = nb + 8 * h.npair;
+  h.body_parent = cpv(d->body_parent, nb); h.body_pos = cpv(d->body_pos, 3 * nb); h.body_ipos = cpv(d->body_ipos, 3 * nb);
+  h.body_iunit = cpv(d->body_inertia_unit, 3 * nb);
+  h.body_rot.assign(9 * nb, 0.0); h.body_irot.assign(9 * nb, 0.0);
+  for (int b = 0; b < nb; ++b) { quat_rot(d->body_quat + 4 * b, &h.body_rot[9 * b]); quat_rot(d->body_iquat + 4 * b, &h.body_irot[9 * b]); }
+  h.jnt_type = cpv(d->jnt_type, h.njnt); h.jnt_qadr = cpv(d->jnt_qadr, h.njnt); h.jnt_vadr = cpv(d->jnt_vadr, h.njnt); h.jnt_body = cpv(d->jnt_body, h.njnt);
+  h.jnt_axis = cpv(d->jnt_axis, 3 * h.njnt); h.jnt_pos = cpv(d->jnt_pos, 3 * h.njnt); h.jnt_damping = cpv(d->jnt_damping, h.njnt);
+  h.jnt_armature = cpv(d->jnt_armature, h.njnt);
+  h.body_jnt.assign(nb, -1); h.dof_jnt.assign(nv, -1); h.dof_body.assign(nv, -1); h.dof_rot.assign(nv, 0);
+  for (int b = 1; b < nb; ++b) if (h.body_parent[b] < 0 || h.body_parent[b] >= b) throw std::runtime_error("body_parent must precede the child");
+  for (int j = 0; j < h.njnt; ++j) {
+    int b = h.jnt_body[j], t = h.jnt_type[j];
+    if (b <= 0 || b >= nb || h.body_jnt[b] >= 0) throw std::runtime_error("each body carries at most one joint");
+    if (t == JNT_FREE && h.body_parent[b] != 0) throw std::runtime_error("free joints only on children of the world");
+    if (t != JNT_FREE && t != JNT_HINGE && t != JNT_SLIDE) throw std::runtime_error("unknown joint type");
+    h.body_jnt[b] = j;
+    int nd = t == JNT_FREE ? 6 : 1;
+    if (h.jnt_vadr[j] < 0 || h.jnt_vadr[j] + nd > nv) throw std::runtime_error("jnt_vadr out of range");
+    for (int c = 0; c < nd; ++c) {
+      h.dof_jnt[h.jnt_vadr[j] + c] = j; h.dof_body[h.jnt_vadr[j] + c] = b;
+      h.dof_rot[h.jnt_vadr[j] + c] = (t == JNT_HINGE) || (t == JNT_FREE && c >= 3);
+    }
+  }
+  for (int j = 0; j < nv; ++j) if (h.dof_jnt[j] < 0) throw std::runtime_error("dof without a joint");
+  // tree levels
+  std::vector<int> depth(nb, 0); int maxd = 0;
+  for (int b = 1; b < nb; ++b) { depth[b] = depth[h.body_parent[b]] + 1; maxd = std::max(maxd, depth[b]); }
+  h.nlevel = maxd; h.level_ptr.assign(1, 0);
+  for (int l = 1; l <= maxd; ++l) { for (int b = 1; b < nb; ++b) if (depth[b] == l) h.level_body.push_back(b); h.level_ptr.push_back((int)h.level_body.size()); }
+  auto anc = [&](int a, int b) { while (b > 0) { if (b == a) return true; b = h.body_parent[b]; } return false; };
+  // (body, ancestor dof) table and subtree lists
+  h.tw_idx.assign((size_t)nb * nv, -1); h.tw_ptr.assign(nb + 1, 0); h.sub_ptr.assign(nb + 1, 0);
+  for (int b = 0; b < nb; ++b) {
+    h.tw_ptr[b] = (int)h.tw_dof.size();
+    if (b > 0) for (int j = 0; j < nv; ++j) if (anc(h.dof_body[j], b)) { h.tw_idx[(size_t)b * nv + j] = (int)h.tw_dof.size(); h.tw_dof.push_back(j); h.tw_body.push_back(b); }
+    h.sub_ptr[b] = (int)h.sub_body.size();
+    if (b > 0) for (int c = b; c < nb; ++c) if (anc(b, c)) h.sub_body.push_back(c);
+  }
+  h.tw_ptr[nb] = (int)h.tw_dof.size(); h.sub_ptr[nb] = (int)h.sub_body.size(); h.ntw = (int)h.tw_dof.size();
+  for (int i = 0; i < nv; ++i) for (int j = 0; j <= i; ++j) {
+    int bi = h.dof_body[i], bj = h.dof_body[j];
+    h.mp_i.push_back(i); h.mp_j.push_back(j);
+    h.mp_deep.push_back(anc(bj, bi) ? bi : (anc(bi, bj) ? bj : -1));
+  }
+  h.nmp = (int)h.mp_i.size();
+  // candidate contacts: every supported geom pair flattens to sphere-like points
+  h.pair_body1.resize(h.npair); h.pair_body2.resize(h.npair);
+  auto push = [&](int pi, int kind, int b1, int b2, int condim, const double* p1, const double* p2, double r1, double r2, const double* fr) {
+    h.ct_pair.push_back(pi); h.ct_kind.push_back(kind); h.ct_b1.push_back(b1); h.ct_b2.push_back(b2); h.ct_condim.push_back(condim);
+    for (int k = 0; k < 3; ++k) { h.ct_p1.push_back(p1[k]); h.ct_p2.push_back(p2[k]); h.ct_t1.push_back(fr ? fr[3 * k] : 0.0); h.ct_t2.push_back(fr ? fr[3 * k + 1] : 0.0); h.ct_n.push_back(fr ? fr[3 * k + 2] : 0.0); }
+    h.ct_rho1.push_back(r1); h.ct_rho2.push_back(r2);
+  };
+  for (int pi = 0; pi < h.npair; ++pi) {
+    int g1 = d->pair_geom1[pi], g2 = d->pair_geom2[pi];
+    if (g1 < 0 || g2 < 0 || g1 >= d->ngeom || g2 >= d->ngeom) throw std::runtime_error("pair geom out of range");
+    int t1 = d->geom_type[g1], t2 = d->geom_type[g2], b1 = d->geom_body[g1], b2 = d->geom_body[g2], cd = d->pair_condim[pi];
+    if (cd != 1 && cd != 3) throw std::runtime_error("condim must be 1 or 3");
+    h.pair_body1[pi] = b1; h.pair_body2[pi] = b2;
+    double R2[9]; quat_rot(d->geom_quat + 4 * g2, R2);
+    const double* o2 = d->geom_pos + 3 * g2; const double* sz = d->geom_size + 3 * g2;
+    if (t1 == DMX_GEOM_PLANE) {
+      if (b1 != 0) throw std::runtime_error("plane geoms must be attached to the world body");
+      double Rp[9]; quat_rot(d->geom_quat + 4 * g1, Rp);
+      const double* pp = d->geom_pos + 3 * g1;
+      if (t2 == DMX_GEOM_SPHERE) push(pi, CK_POINT_PLANE, b1, b2, cd, pp, o2, 0.0, sz[0], Rp);
+      else if (t2 == DMX_GEOM_CAPSULE) {
+        for (int s = -1; s <= 1; s += 2) { double l[3] = {0, 0, s * sz[1]}, w[3]; mat_vec(R2, l, w); for (int k = 0; k < 3; ++k) w[k] += o2[k]; push(pi, CK_POINT_PLANE, b1, b2, cd, pp, w, 0.0, sz[0], Rp); }
+      } else if (t2 == DMX_GEOM_BOX) {
+        for (int c = 0; c < 8; ++c) {
+          double l[3] = {(c & 1 ? 1 : -1) * sz[0], (c & 2 ? 1 : -1) * sz[1], (c & 4 ? 1 : -1) * sz[2]}, w[3];
+          mat_vec(R2, l, w); for (int k = 0; k < 3; ++k) w[k] += o2[k];
+          push(pi, CK_POINT_PLANE, b1, b2, cd, pp, w, 0.0, 0.0, Rp);
+        }
+      } else throw std::runtime_error("unsupported geom pair");
+    } else if (t1 == DMX_GEOM_SPHERE && t2 == DMX_GEOM_SPHERE) {
+      push(pi, CK_POINT_POINT, b1, b2, cd, d->geom_pos + 3 * g1, o2, d->geom_size[3 * g1], sz[0], nullptr);
+    } else throw std::runtime_error("unsupported geom pair (plane must be geom1)");
+  }
+  h.nc = (int)h.ct_kind.size();
+  h.nrmax = 0; for (int c = 0; c < h.nc; ++c) h.nrmax += h.ct_condim[c] == 3 ? 4 : 1;
+  h.pair_solimp_cfd = cpv(d->pair_solimp_cfd, 5 * h.npair); h.pair_cfd_beta = cpv(d->pair_cfd_beta, h.npair);
+  h.pair_invweight.assign(h.npair, 0.0);
+  h.act_type = cpv(d->act_type, h.nu); h.act_jnt = cpv(d->act_jnt, h.nu); h.act_gear = cpv(d->act_gear, h.nu); h.act_kp = cpv(d->act_kp, h.nu); h.act_kd = cpv(d->act_kd, h.nu);
+  for (int i = 0; i < h.nu; ++i) if (h.act_jnt[i] < 0 || h.act_jnt[i] >= h.njnt || h.jnt_type[h.act_jnt[i]] == JNT_FREE) throw std::runtime_error("actuators act on hinge / slide joints");
+  h.p_default.assign(h.np, 0.0);
+  for (int b = 0; b < nb; ++b) h.p_default[b] = d->body_mass[b];
+  for (int i = 0; i < h.npair; ++i) h.p_default[nb + i] = d->pair_friction[i];
+  for (int i = 0; i < 2 * h.npair; ++i) h.p_default[nb + h.npair + i] = d->pair_solref[i];
+  for (int i = 0; i < 5 * h.npair; ++i) h.p_default[nb + 3 * h.npair + i] = d->pair_solimp[i];
+  h.qpos0 = cpv(d->qpos0, h.nq);
+}
+
+void make_layouts(const HostModel& h, WsLayout& wl, WsLayout& rwl, RkLayout& rl) {
+  const int nb = h.nbody, nv = h.nv, nq = h.nq, nc = std::max(h.nc, 1), nr = std::max(h.nrmax, 1);
+  std::memset(&wl, 0, sizeof(wl)); std::memset(&rwl, 0, sizeof(rwl)); std::memset(&rl, 0, sizeof(rl));
+  int o = 0;
+  auto take = [&](int& f, int n) { f = o; o += n; };
+  take(wl.fp, 3 * nb); take(wl.fR, 9 * nb); take(wl.fw, 3 * nb); take(wl.fal, 3 * nb); take(wl.fvp, 3 * nb); take(wl.fap, 3 * nb);
+  take(wl.com, 3 * nb); take(wl.dax, 3 * nv); take(wl.dan, 3 * nv);
+  rwl = wl; rwl.size = o;                                  // the tangent pass needs the frames only
+  take(wl.Fb, 3 * nb); take(wl.Nb, 3 * nb); take(wl.Iw, 9 * nb); take(wl.Isub, 9 * nb); take(wl.tw, 3 * std::max(h.ntw, 1));
+  take(wl.M, nv * nv); take(wl.Hc, nv * nv); take(wl.tau, nv); take(wl.c, nv); take(wl.a0, nv); take(wl.x, nv); take(wl.g, nv);
+  take(wl.dl, nv); take(wl.Md, nv); take(wl.xa, nv); take(wl.kap, nv);
+  take(wl.cr, nc); take(wl.cn, 3 * nc); take(wl.cpos, 3 * nc); take(wl.ct1, 3 * nc); take(wl.ct2, 3 * nc);
+  take(wl.cD, nc); take(wl.cpost, nc); take(wl.cbd, nc); take(wl.cmu, nc);
+  take(wl.J, nr * nv); take(wl.aref, nr); take(wl.D, nr); take(wl.s, nr); take(wl.pr, nr);
+  wl.size = o;
+  rl.Yqr = o; rl.Vr = o + nq; rl.rsize = nq + nv;
+  o = 0;
+  take(wl.i_incl, nc); take(wl.i_rowstart, nc); take(wl.i_rowcand, nr); take(wl.i_active, nr);
+  wl.isize = o;
+  o = 0;
+  take(rl.q, nq); take(rl.v, nv); take(rl.Yq, nq); take(rl.V, nv); take(rl.Dl, nv); take(rl.K, 7 * nv); take(rl.A, 7 * nv); take(rl.err, 2 * nv);
+  rl.size_fwd = o;
+  take(rl.sYq, 6 * nq); take(rl.sV, 6 * nv); take(rl.sDl, 6 * nv); take(rl.Kb, 6 * nv); take(rl.Ab, 6 * nv);
+  take(rl.qb, nv); take(rl.vb, nv); take(rl.dbar, nv); take(rl.Vb, nv); take(rl.lam, 2 * nv); take(rl.delta, nv);
+  take(rl.qbar, nv); take(rl.vbar, nv); take(rl.ubar, std::max(h.nu, 1)); take(rl.pbar, h.np); take(rl.gp, h.np);
+  rl.size_bwd = o;
+}
+
+template <class R> size_t add_real(Arena& a, const std::vector<double>& v) {
+  std::vector<R> t(v.size()); for (size_t i = 0; i < v.size(); ++i) t[i] = (R)v[i];
+  return a.add(t.data(), t.size() * sizeof(R));
+}
+inline size_t add_int(Arena& a, const std::vector<int>& v) { return a.add(v.data(), v.size() * sizeof(int)); }
+
+// lay the constants out in an arena; pointers are patched once the device address is known
+template <class R> void build_dev(const HostModel& h, Arena& ar, ModelDev<R>& m, bool patch) {
+  static thread_local std::vector<size_t> offs;
+  if (!patch) {
+    offs.clear();
+    const std::vector<int>* iv[] = {&h.body_parent, &h.body_jnt, &h.level_ptr, &h.level_body, &h.jnt_type, &h.jnt_qadr, &h.jnt_vadr, &h.jnt_body,
+                                    &h.dof_jnt, &h.dof_body, &h.dof_rot, &h.tw_ptr, &h.tw_body, &h.tw_dof, &h.tw_idx, &h.sub_ptr, &h.sub_body,
+                                    &h.mp_i, &h.mp_j, &h.mp_deep, &h.ct_kind, &h.ct_b1, &h.ct_b2, &h.ct_condim, &h.ct_pair, &h.act_type, &h.act_jnt};
+    for (auto v : iv) offs.push_back(add_int(ar, *v));
+    const std::vector<double>* rv[] = {&h.body_pos, &h.body_rot, &h.body_ipos, &h.body_irot, &h.body_iunit, &h.jnt_axis, &h.jnt_pos, &h.jnt_damping,
+                                       &h.jnt_armature, &h.ct_p1, &h.ct_p2, &h.ct_rho1, &h.ct_rho2, &h.ct_n, &h.ct_t1, &h.ct_t2, &h.pair_invweight,
+                                       &h.pair_solimp_cfd, &h.pair_cfd_beta, &h.act_gear, &h.act_kp, &h.act_kd, &h.p_default};
+    for (auto v : rv) offs.push_back(add_real<R>(ar, *v));
+    return;
+  }
+  m.nbody = h.nbody; m.njnt = h.njnt; m.nq = h.nq; m.nv = h.nv; m.nu = h.nu; m.npair = h.npair; m.nc = h.nc; m.np = h.np;
+  m.nlevel = h.nlevel; m.ntw = h.ntw; m.nmp = h.nmp; m.nrmax = h.nrmax; m.newton_iters = h.newton_iters; m.ls_iters = h.ls_iters;
+  m.p_fric = h.nbody; m.p_solref = h.nbody + h.npair; m.p_solimp = h.nbody + 3 * h.npair;
+  for (int k = 0; k < 3; ++k) m.gravity[k] = (R)h.gravity[k];
+  size_t k = 0;
+  auto ip = [&]() { return reinterpret_cast<const int*>(ar.dev + offs[k++]); };
+  auto rp = [&]() { return reinterpret_cast<const R*>(ar.dev + offs[k++]); };
+  m.body_parent = ip(); m.body_jnt = ip(); m.level_ptr = ip(); m.level_body = ip(); m.jnt_type = ip(); m.jnt_qadr = ip(); m.jnt_vadr = ip(); m.jnt_body = ip();
+  m.dof_jnt = ip(); m.dof_body = ip(); m.dof_rot = ip(); m.tw_ptr = ip(); m.tw_body = ip(); m.tw_dof = ip(); m.tw_idx = ip(); m.sub_ptr = ip(); m.sub_body = ip();
+  m.mp_i = ip(); m.mp_j = ip(); m.mp_deep = ip(); m.ct_kind = ip(); m.ct_b1 = ip(); m.ct_b2 = ip(); m.ct_condim = ip(); m.ct_pair = ip(); m.act_type = ip(); m.act_jnt = ip();
+  m.body_pos = rp(); m.body_rot = rp(); m.body_ipos = rp(); m.body_irot = rp(); m.body_iunit = rp(); m.jnt_axis = rp(); m.jnt_pos = rp(); m.jnt_damping = rp();
+  m.jnt_armature = rp(); m.ct_p1 = rp(); m.ct_p2 = rp(); m.ct_rho1 = rp(); m.ct_rho2 = rp(); m.ct_n = rp(); m.ct_t1 = rp(); m.ct_t2 = rp(); m.pair_invweight = rp();
+  m.pair_solimp_cfd = rp(); m.pair_cfd_beta = rp(); m.act_gear = rp(); m.act_kp = rp(); m.act_kd = rp(); m.p_default = rp();
+}
+
+}  // namespace
+
+// ---- the model object -------------------------------------------------------------------------------------
+struct dmx_model {
+  int precision, G, block, sm_count;
+  HostModel h;
+  Arena arena;
+  ModelDev<double> md; ModelDev<float> mf;
+  WsLayout wl, rwl; RkLayout rl;
+  size_t smem_fwd, smem_bwd; int occ_fwd, occ_bwd;
+  int* queue = nullptr;            // [4] work-queue counters
+  void* zero_u = nullptr;          // zeros: controls when ctrl == NULL, velocities at create
+  void* scratch = nullptr; size_t scratch_bytes = 0;   // tangent workspaces of the VJP lanes
+};
+
+namespace {
+
+size_t rsize(const dmx_model* m) { return m->precision == 64 ? sizeof(double) : sizeof(float); }
+
+size_t group_bytes(const dmx_model* m, bool bwd) {
+  return (size_t)(bwd ? m->rl.size_bwd : m->rl.size_fwd) * sizeof(double) + (size_t)(m->wl.size + m->rl.rsize) * rsize(m) +
+         (size_t)m->wl.isize * sizeof(int);
+}
+int groups_per_block(const dmx_model* m) { return m->G == 1 ? m->block : m->block / m->G; }
+
+int ensure_scratch(dmx_model* m, int grid) {
+  size_t dual = 2 * rsize(m);
+  size_t need = (size_t)grid * (m->block / 32) * 32 * (size_t)m->rwl.size * dual;
+  if (need <= m->scratch_bytes) return 0;
+  if (m->scratch) cudaFree(m->scratch);
+  m->scratch = nullptr; m->scratch_bytes = 0;
+  CUDA_OK(cudaMalloc(&m->scratch, need));
+  m->scratch_bytes = need;
+  return 0;
+}
+
+template <class R> const ModelDev<R>& dev_of(const dmx_model* m);
+template <> const ModelDev<double>& dev_of<double>(const dmx_model* m) { return m->md; }
+template <> const ModelDev<float>& dev_of<float>(const dmx_model* m) { return m->mf; }
+
+SolverOpts opts_of(const dmx_solver_opts* o) {
+  SolverOpts s; s.tableau = o->tableau; s.rtol = o->rtol; s.atol = o->atol; s.h0 = o->h0; s.pcoeff = o->pcoeff; s.icoeff = o->icoeff;
+  s.safety = o->safety; s.fac_min = o->fac_min; s.fac_max = o->fac_max; s.max_steps = o->max_steps;
+  return s;
+}
+size_t tape_header_bytes(int nenv) { return (((size_t)nenv * 2 * sizeof(int)) + 255) & ~size_t(255); }
+
+template <class R>
+int create_typed(dmx_model* m) {
+  HostModel& h = m->h;
+  ModelDev<R> dev;
+  build_dev<R>(h, m->arena, dev, false);
+  CUDA_OK(cudaMalloc(&m->arena.dev, m->arena.host.size()));
+  CUDA_OK(cudaMemcpy(m->arena.dev, m->arena.host.data(), m->arena.host.size(), cudaMemcpyHostToDevice));
+  build_dev<R>(h, m->arena, dev, true);
+  Launchers<R> L = launchers_for<R>(m->G);
+  // A^: body inverse weights at qpos0 on the device (same kinematics / mass-matrix / Cholesky code as the rollouts)
+  std::vector<R> q0(h.nq); for (int i = 0; i < h.nq; ++i) q0[i] = (R)h.qpos0[i];
+  R *dq0 = nullptr, *dw = nullptr;
+  CUDA_OK(cudaMalloc(&dq0, sizeof(R) * h.nq)); CUDA_OK(cudaMalloc(&dw, sizeof(R) * h.nbody));
+  CUDA_OK(cudaMemcpy(dq0, q0.data(), sizeof(R) * h.nq, cudaMemcpyHostToDevice));
+  LaunchCfg c; c.block = 32; c.grid = 1; c.smem = (m->G == 1 ? 32 : 32 / m->G) * group_bytes(m, true);
+  CUDA_OK(L.invweight(dev, dq0, (const R*)m->zero_u, dw, m->wl, m->rl, c, 0));
+  CUDA_OK(cudaDeviceSynchronize());
+  std::vector<R> bw(h.nbody);
+  CUDA_OK(cudaMemcpy(bw.data(), dw, sizeof(R) * h.nbody, cudaMemcpyDeviceToHost));
+  cudaFree(dq0); cudaFree(dw);
+  for (int b = 1; b < h.nbody; ++b) if (!std::isfinite((double)bw[b])) return fail("mass matrix at qpos0 is not positive definite");
+  std::vector<R> pw(h.npair);
+  for (int i = 0; i < h.npair; ++i) { h.pair_invweight[i] = (double)bw[h.pair_body1[i]] + (double)bw[h.pair_body2[i]]; pw[i] = (R)h.pair_invweight[i]; }
+  if (h.npair) CUDA_OK(cudaMemcpy(const_cast<R*>(dev.pair_invweight), pw.data(), sizeof(R) * h.npair, cudaMemcpyHostToDevice));
+  if (sizeof(R) == 8) std::memcpy(&m->md, &dev, sizeof(dev)); else std::memcpy(&m->mf, &dev, sizeof(dev));
+  CUDA_OK(L.occupancy(m->block, m->smem_fwd, m->smem_bwd, &m->occ_fwd, &m->occ_bwd));
+  if (m->occ_fwd < 1 || m->occ_bwd < 1) return fail("kernel does not fit on an SM (shared memory / registers)");
+  return 0;
+}
+
+int pick_lanes(const HostModel& h) {
+  const char* e = std::getenv("DMX_LANES");
+  if (e) { int g = std::atoi(e); if (g == 1 || g == 8 || g == 16 || g == 32) return g; }
+  if (h.nv <= 2) return 1;
+  if (h.nv <= 8 && h.nc <= 4) return 8;
+  if (h.nv <= 8) return 16;
+  return 32;
+}
+
+template <class R>
+int rollout_typed(const dmx_model* m, int nenv, const void* x0, const void* ctrl, int nknot, double knot_dt, const void* params, double horizon,
+                  const dmx_solver_opts* opts, const double* h_replay, int n_replay, void* xT, const dmx_stats* st, void* tape, size_t tape_bytes,
+                  cudaStream_t s) {
+  RolloutArgs<R> a; std::memset(&a, 0, sizeof(a));
+  const int rec = m->h.nq + m->h.nv + 2;
+  a.nenv = nenv; a.nknot = nknot; a.n_replay = h_replay ? n_replay : 0; a.want_tape = tape != nullptr;
+  if (tape) {
+    size_t hdr = tape_header_bytes(nenv);
+    if (tape_bytes < hdr + (size_t)nenv * rec * sizeof(R)) return fail("tape too small");
+    a.tape_cap = (int)std::min<size_t>((tape_bytes - hdr) / ((size_t)nenv * rec * sizeof(R)), (size_t)1 << 30);
+    a.tape_hdr = (int*)tape; a.tape = (R*)((unsigned char*)tape + hdr);
+  }
+  a.x0 = (const R*)x0; a.ctrl = (const R*)ctrl; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u; a.h_replay = h_replay;
+  a.knot_dt = knot_dt; a.horizon = horizon; a.so = opts_of(opts); a.xT = (R*)xT;
+  if (st) { a.n_accept = st->n_accept; a.n_reject = st->n_reject; a.n_feval = st->n_feval; a.n_unconv = st->n_newton_unconverged; a.status = st->status;
+            a.h_min = st->h_min; a.h_max = st->h_max; a.t_end = st->t_end; }
+  a.queue = m->queue; a.wl = m->wl; a.rl = m->rl;
+  CUDA_OK(cudaMemsetAsync(m->queue, 0, sizeof(int), s));
+  LaunchCfg c; c.block = m->block; c.smem = m->smem_fwd;
+  int gpb = groups_per_block(m);
+  c.grid = std::max(1, std::min(m->occ_fwd * m->sm_count, (nenv + gpb - 1) / gpb));
+  CUDA_OK(launchers_for<R>(m->G).rollout(dev_of<R>(m), a, c, s));
+  return 0;
+}
+
+template <class R>
+int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const void* params, const dmx_solver_opts* opts, const void* xT,
+                   const void* dLdxT, int cfd_on, void* dLdx0, void* dLdctrl, void* dLdparams, const int* status, const void* tape,
+                   size_t tape_bytes, cudaStream_t s) {
+  BackwardArgs<R> a; std::memset(&a, 0, sizeof(a));
+  const int rec = m->h.nq + m->h.nv + 2;
+  size_t hdr = tape_header_bytes(nenv);
+  if (!tape || tape_bytes < hdr + (size_t)nenv * rec * sizeof(R)) return fail("tape missing or too small");
+  a.nenv = nenv; a.nknot = nknot; a.want_p = dLdparams != nullptr; a.cfd = cfd_on;
+  a.tape_cap = (int)std::min<size_t>((tape_bytes - hdr) / ((size_t)nenv * rec * sizeof(R)), (size_t)1 << 30);
+  a.tape_hdr = (const int*)tape; a.tape = (const R*)((const unsigned char*)tape + hdr);
+  a.ctrl = (const R*)ctrl; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u; a.xT = (const R*)xT; a.dLdxT = (const R*)dLdxT;
+  a.status = status; a.so = opts_of(opts); a.dLdx0 = (R*)dLdx0; a.dLdctrl = (R*)dLdctrl; a.dLdparams = (R*)dLdparams;
+  a.queue = m->queue + 1; a.wl = m->wl; a.rwl = m->rwl; a.rl = m->rl; a.res_size = m->rwl.size;
+  LaunchCfg c; c.block = m->block; c.smem = m->smem_bwd;
+  int gpb = groups_per_block(m);
+  c.grid = std::max(1, std::min(m->occ_bwd * m->sm_count, (nenv + gpb - 1) / gpb));
+  if (ensure_scratch(m, c.grid)) return -1;
+  a.scratch = (Dual<R>*)m->scratch;
+  CUDA_OK(cudaMemsetAsync(m->queue + 1, 0, sizeof(int), s));
+  if (dLdctrl && nknot > 0 && m->h.nu > 0) CUDA_OK(cudaMemsetAsync(dLdctrl, 0, (size_t)nenv * nknot * m->h.nu * sizeof(R), s));
+  CUDA_OK(launchers_for<R>(m->G).backward(dev_of<R>(m), a, c, s));
+  return 0;
+}
+
+template <class R>
+int field_typed(dmx_model* m, int n, const void* x, const void* u, const void* params, const void* kappa, int cfd, void* acc, int* nrow,
+                void* qbar, void* vbar, void* ubar, void* pbar, cudaStream_t s) {
+  FieldArgs<R> a; std::memset(&a, 0, sizeof(a));
+  a.n = n; a.cfd = cfd; a.want_p = pbar != nullptr; a.x = (const R*)x; a.u = (const R*)u; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u;
+  a.kappa = (const R*)kappa; a.acc = (R*)acc; a.nrow = nrow; a.qbar = (R*)qbar; a.vbar = (R*)vbar; a.ubar = (R*)ubar; a.pbar = (R*)pbar;
+  a.wl = m->wl; a.rwl = m->rwl; a.rl = m->rl; a.res_size = m->rwl.size;
+  LaunchCfg c; c.block = m->block; c.smem = m->smem_bwd;
+  int gpb = groups_per_block(m);
+  c.grid = std::max(1, std::min(m->occ_bwd * m->sm_count, (n + gpb - 1) / gpb));
+  if (kappa) { if (ensure_scratch(m, c.grid)) return -1; a.scratch = (Dual<R>*)m->scratch; }
+  CUDA_OK(launchers_for<R>(m->G).field(dev_of<R>(m), a, c, s));
+  return 0;
+}
+
+// FMA-chain microbenchmark: 8 independent chains per thread
+template <class T> __global__ void fma_chain_kernel(T* out, int iters, T a, T b) {
+  T x0 = T(threadIdx.x), x1 = x0 + T(1), x2 = x0 + T(2), x3 = x0 + T(3), x4 = x0 + T(4), x5 = x0 + T(5), x6 = x0 + T(6), x7 = x0 + T(7);
+  for (int i = 0; i < iters; ++i) {
+    x0 = x0 * a + b; x1 = x1 * a + b; x2 = x2 * a + b; x3 = x3 * a + b; x4 = x4 * a + b; x5 = x5 * a + b; x6 = x6 * a + b; x7 = x7 * a + b;
+  }
+  out[blockIdx.x * blockDim.x + threadIdx.x] = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+}
+template <class T> int fma_peak_typed(int iters, double* flops, double* ms_out) {
+  int dev = 0, sms = 0; CUDA_OK(cudaGetDevice(&dev)); CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  int block = 256, grid = sms * 8;
+  T* out = nullptr; CUDA_OK(cudaMalloc(&out, sizeof(T) * block * grid));
+  cudaEvent_t e0, e1; CUDA_OK(cudaEventCreate(&e0)); CUDA_OK(cudaEventCreate(&e1));
+  fma_chain_kernel<T><<<grid, block>>>(out, iters / 4, T(0.999), T(0.001));
+  float best = 1e30f;
+  for (int r = 0; r < 3; ++r) {
+    CUDA_OK(cudaEventRecord(e0));
+    fma_chain_kernel<T><<<grid, block>>>(out, iters, T(0.999), T(0.001));
+    CUDA_OK(cudaEventRecord(e1)); CUDA_OK(cudaEventSynchronize(e1));
+    float ms; CUDA_OK(cudaEventElapsedTime(&ms, e0, e1)); best = std::min(best, ms);
+  }
+  CUDA_OK(cudaGetLastError());
+  cudaFree(out); cudaEventDestroy(e0); cudaEventDestroy(e1);
+  *flops = 2.0 * 8.0 * (double)iters * block * grid / (best * 1e-3); *ms_out = best;
+  return 0;
+}
+
+}  // namespace
+
+// ---- C-ABI ------------------------------------------------------------------------------------------------
+extern "C" {
+
+const char* dmx_last_error(void) { return g_err; }
+
+int dmx_model_create(const dmx_model_desc* desc, int precision, dmx_model** out) {
+  if (!desc || !out) return fail("null argument");
+  if (precision != 64 && precision != 32) return fail("precision must be 64 or 32");
+  dmx_model* m = new dmx_model();
+  try { flatten(desc, m->h); } catch (std::exception& e) { fail("model: %s", e.what()); delete m; return -1; }
+  m->precision = precision;
+  m->G = pick_lanes(m->h);
+  make_layouts(m->h, m->wl, m->rwl, m->rl);
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+    fail("no CUDA device: the dmx library has no CPU fallback"); delete m; return -1;
+  }
+  int max_smem = 0; cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  m->block = m->G == 1 ? 32 : 128;
+  for (;;) {
+    m->smem_fwd = groups_per_block(m) * group_bytes(m, false); m->smem_bwd = groups_per_block(m) * group_bytes(m, true);
+    if ((int)m->smem_bwd <= max_smem || m->block == 32) break;
+    m->block /= 2;
+  }
+  if ((int)m->smem_bwd > max_smem) {
+    if (m->G < 32) { fail("model too large for shared memory at this lane count; set DMX_LANES=32"); delete m; return -1; }
+    fail("model too large for the per-environment shared-memory workspace"); delete m; return -1;
+  }
+  size_t zbytes = sizeof(double) * (size_t)std::max(std::max(m->h.nu, m->h.nv), 1);
+  if (cudaMalloc(&m->zero_u, zbytes) != cudaSuccess || cudaMemset(m->zero_u, 0, zbytes) != cudaSuccess ||
+      cudaMalloc(&m->queue, 4 * sizeof(int)) != cudaSuccess) { fail("cudaMalloc failed"); dmx_model_destroy(m); return -1; }
+  int rc = precision == 64 ? create_typed<double>(m) : create_typed<float>(m);
+  if (rc) { dmx_model_destroy(m); return -1; }
+  *out = m;
+  return 0;
+}
+
+void dmx_model_destroy(dmx_model* m) {
+  if (!m) return;
+  if (m->arena.dev) cudaFree(m->arena.dev);
+  if (m->queue) cudaFree(m->queue);
+  if (m->zero_u) cudaFree(m->zero_u);
+  if (m->scratch) cudaFree(m->scratch);
+  delete m;
+}
+
+int dmx_model_np(const dmx_model* m) { return m ? m->h.np : -1; }
+int dmx_model_nc(const dmx_model* m) { return m ? m->h.nc : -1; }
+int dmx_model_lanes(const dmx_model* m) { return m ? m->G : -1; }
+int dmx_model_default_params(const dmx_model* m, double* p_host) {
+  if (!m || !p_host) return fail("null argument");
+  for (int i = 0; i < m->h.np; ++i) p_host[i] = m->h.p_default[i];
+  return 0;
+}
+
+size_t dmx_tape_bytes(const dmx_model* m, int nenv, int tape_steps) {
+  if (!m || nenv <= 0 || tape_steps <= 0) return 0;
+  return tape_header_bytes(nenv) + (size_t)nenv * (size_t)tape_steps * (size_t)(m->h.nq + m->h.nv + 2) * rsize(m);
+}
+
+static int check_common(const dmx_model* m, int nenv, const void* x0, const dmx_solver_opts* o, double horizon) {
+  if (!m) return fail("null model");
+  if (nenv <= 0) return fail("nenv must be positive");
+  if (!x0 || !o) return fail("null argument");
+  if (o->tableau != DMX_DOPRI5 && o->tableau != DMX_TSIT5) return fail("unknown tableau");
+  if (!(o->rtol >= 0) || !(o->atol >= 0) || !(o->rtol + o->atol > 0) || !(o->h0 > 0) || !(horizon >= 0)) return fail("bad tolerances / h0 / horizon");
+  return 0;
+}
+
+int dmx_rollout(const dmx_model* m, int nenv, const void* x0, const void* ctrl, int nknot, double knot_dt, const void* params, double horizon,
+                const dmx_solver_opts* opts, const double* h_replay, int n_replay, void* xT, const dmx_stats* stats, void* tape, size_t tape_bytes,
+                void* cuda_stream) {
+  if (check_common(m, nenv, x0, opts, horizon)) return -1;
+  if (!xT) return fail("null xT");
+  if (ctrl && m->h.nu > 0 && (nknot <= 0 || !(knot_dt > 0))) return fail("ctrl given but nknot / knot_dt invalid");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  return m->precision == 64 ? rollout_typed<double>(m, nenv, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay, n_replay, xT, stats, tape, tape_bytes, s)
+                            : rollout_typed<float>(m, nenv, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay, n_replay, xT, stats, tape, tape_bytes, s);
+}
+
+int dmx_rollout_backward(const dmx_model* m, int nenv, const void* ctrl, int nknot, const void* params, const dmx_solver_opts* opts, const void* xT,
+                         const void* dLdxT, int cfd_on, void* dLdx0, void* dLdctrl, void* dLdparams, const int* status, const void* tape,
+                         size_t tape_bytes, void* cuda_stream) {
+  if (!m || nenv <= 0 || !opts || !xT || !dLdxT || !dLdx0) return fail("null argument");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  dmx_model* mm = const_cast<dmx_model*>(m);   // scratch is grown lazily
+  return m->precision == 64 ? backward_typed<double>(mm, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, status, tape, tape_bytes, s)
+                            : backward_typed<float>(mm, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, status, tape, tape_bytes, s);
+}
+
+int dmx_rollout_grad(const dmx_model* m, int nenv, const void* x0, const void* ctrl, int nknot, double knot_dt, const void* params, double horizon,
+                     const dmx_solver_opts* opts, const double* h_replay, int n_replay, const void* dLdxT, int cfd_on, void* xT, void* dLdx0,
+                     void* dLdctrl, void* dLdparams, const dmx_stats* stats, void* tape, size_t tape_bytes, void* cuda_stream) {
+  if (!tape) return fail("dmx_rollout_grad needs a tape");
+  int rc = dmx_rollout(m, nenv, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay, n_replay, xT, stats, tape, tape_bytes, cuda_stream);
+  if (rc) return rc;
+  return dmx_rollout_backward(m, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, nullptr, tape, tape_bytes, cuda_stream);
+}
+
+int dmx_vector_field(const dmx_model* m, int n, const void* x, const void* u, const void* params, int cfd, void* acc, int* nrow, void* cuda_stream) {
+  if (!m || n <= 0 || !x || !acc) return fail("null argument");
+  dmx_model* mm = const_cast<dmx_model*>(m);
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  return m->precision == 64 ? field_typed<double>(mm, n, x, u, params, nullptr, cfd, acc, nrow, nullptr, nullptr, nullptr, nullptr, s)
+                            : field_typed<float>(mm, n, x, u, params, nullptr, cfd, acc, nrow, nullptr, nullptr, nullptr, nullptr, s);
+}
+
+int dmx_vjp_field(const dmx_model* m, int n, const void* x, const void* u, const void* params, const void* kappa, int cfd, void* qbar, void* vbar,
+                  void* ubar, void* pbar, void* cuda_stream) {
+  if (!m || n <= 0 || !x || !kappa || !qbar || !vbar || (!ubar && m->h.nu > 0)) return fail("null argument");
+  dmx_model* mm = const_cast<dmx_model*>(m);
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  return m->precision == 64 ? field_typed<double>(mm, n, x, u, params, kappa, cfd, nullptr, nullptr, qbar, vbar, ubar, pbar, s)
+                            : field_typed<float>(mm, n, x, u, params, kappa, cfd, nullptr, nullptr, qbar, vbar, ubar, pbar, s);
+}
+
+int dmx_fma_peak(int precision, int iters, double* flops_per_s, double* ms) {
+  if (!flops_per_s || !ms || iters <= 0) return fail("bad argument");
+  return precision == 64 ? fma_peak_typed<double>(iters, flops_per_s, ms) : fma_peak_typed<float>(iters, flops_per_s, ms);
+}
+
+}  // extern "C"

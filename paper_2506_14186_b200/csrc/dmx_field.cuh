@@ -1,0 +1,626 @@
+// dmx_field.cuh — the vector field F_theta(t,x) of PAPER.md Eq. (1)/(5) and its CFD variant F~
+// as lane-group device code:
+//   S1 forward kinematics, S2 mass matrix + Cholesky, S3 bias / applied forces, S4 narrow phase,
+//   S5 constraint rows (Eq. 3, impedance, regulariser), S6 fixed-iteration Newton contact solve
+//   (Eq. 2), and S11/S12 the vector-Jacobian product by implicit differentiation of the
+//   stationarity condition at the final active set (PAPER.md:543 suggests implicit
+//   differentiation).
+#pragma once
+#include "dmx_model.cuh"
+
+namespace dmx {
+
+// ---- inputs of one evaluation -----------------------------------------------------------------
+template <class R> struct InPlain {
+  typedef R S;
+  Arr<R> qa, va, aa; const R* ua; const R* pa;
+  DMX_DI R q(int i) const { return qa[i]; }
+  DMX_DI R v(int i) const { return va[i]; }
+  DMX_DI R a(int i) const { return aa[i]; }
+  DMX_DI R u(int i) const { return ua[i]; }
+  DMX_DI R p(int i) const { return pa[i]; }
+};
+// the same inputs carrying one tangent direction (kind 0: configuration, 1: velocity, 2: control,
+// 3: parameter); the acceleration argument (x*) is held fixed
+template <class R> struct InDual {
+  typedef Dual<R> S;
+  Arr<R> qa, va, aa; const R* ua; const R* pa;
+  int kind, idx; R dq0, dq1, dq2, dq3;
+  DMX_DI S q(int i) const {
+    R t = R(0);
+    if (kind == 0) { int k = i - idx; t = k == 0 ? dq0 : (k == 1 ? dq1 : (k == 2 ? dq2 : (k == 3 ? dq3 : R(0)))); }
+    return S(qa[i], t);
+  }
+  DMX_DI S v(int i) const { return S(va[i], (kind == 1 && i == idx) ? R(1) : R(0)); }
+  DMX_DI S a(int i) const { return S(aa[i], R(0)); }
+  DMX_DI S u(int i) const { return S(ua[i], (kind == 2 && i == idx) ? R(1) : R(0)); }
+  DMX_DI S p(int i) const { return S(pa[i], (kind == 3 && i == idx) ? R(1) : R(0)); }
+};
+
+template <class S> struct FrameT { V3<S> p; M3<S> R; V3<S> w, al, vp, ap; };
+
+template <class S> DMX_DI V3<S> point_vel(const FrameT<S>& f, const V3<S>& x) { return f.vp + cross(f.w, x - f.p); }
+template <class S> DMX_DI V3<S> point_acc(const FrameT<S>& f, const V3<S>& x) {
+  V3<S> d = x - f.p;
+  return f.ap + cross(f.al, d) + cross(f.w, cross(f.w, d));
+}
+
+// ---- S1: forward kinematics with first and second time derivatives ---------------
+// One body: frame from the parent's frame and the body's joint.  ACC: joint accelerations in.a
+// enter (inverse dynamics at a given acceleration); otherwise they are zero (bias force).
+template <class S, class R, class IN, bool ACC>
+DMX_DI void body_kin(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, int b) {
+  int par = m.body_parent[b];
+  FrameT<S> P;
+  P.p = ld3(ws.fp, par); P.R = ld9(ws.fR, par); P.w = ld3(ws.fw, par); P.al = ld3(ws.fal, par);
+  P.vp = ld3(ws.fvp, par); P.ap = ld3(ws.fap, par);
+  FrameT<S> f;
+  f.p = P.p + P.R * c3<S>(m.body_pos, b);
+  f.R = P.R * c9<S>(m.body_rot, b);
+  f.w = P.w; f.al = P.al;
+  f.vp = point_vel(P, f.p); f.ap = point_acc(P, f.p);
+  int j = m.body_jnt[b];
+  if (j >= 0) {
+    int qa = m.jnt_qadr[j], va = m.jnt_vadr[j], jt = m.jnt_type[j];
+    if (jt == JNT_HINGE) {
+      V3<S> ax = f.R * c3<S>(m.jnt_axis, j);
+      V3<S> o = f.p + f.R * c3<S>(m.jnt_pos, j);
+      V3<S> vo = point_vel(f, o), ao = point_acc(f, o);
+      M3<S> Rot = axis_angle(ax, in.q(qa));
+      S vj = in.v(va);
+      FrameT<S> g;
+      g.R = Rot * f.R;
+      g.p = o + Rot * (f.p - o);
+      g.w = f.w + ax * vj;
+      g.al = f.al + cross(f.w, ax) * vj;
+      if (ACC) g.al = g.al + ax * in.a(va);
+      V3<S> d = g.p - o;
+      g.vp = vo + cross(g.w, d);
+      g.ap = ao + cross(g.al, d) + cross(g.w, cross(g.w, d));
+      f = g;
+      st3(ws.dax, va, ax); st3(ws.dan, va, o);
+    } else if (jt == JNT_SLIDE) {
+      V3<S> ax = f.R * c3<S>(m.jnt_axis, j);
+      V3<S> s = ax * in.q(qa);
+      S vj = in.v(va);
+      V3<S> np = f.p + s;
+      V3<S> nvp = f.vp + cross(f.w, s) + ax * vj;
+      V3<S> nap = f.ap + cross(f.al, s) + cross(f.w, cross(f.w, s)) + cross(f.w, ax) * (S(2.0) * vj);
+      if (ACC) nap = nap + ax * in.a(va);
+      f.p = np; f.vp = nvp; f.ap = nap;
+      st3(ws.dax, va, ax); st3(ws.dan, va, np);
+    } else {  // free joint: world linear velocity, body angular velocity
+      f.p = mk3<S>(in.q(qa), in.q(qa + 1), in.q(qa + 2));
+      f.R = quat_to_mat<S>(in.q(qa + 3), in.q(qa + 4), in.q(qa + 5), in.q(qa + 6));
+      f.vp = mk3<S>(in.v(va), in.v(va + 1), in.v(va + 2));
+      f.w = f.R * mk3<S>(in.v(va + 3), in.v(va + 4), in.v(va + 5));
+      S z(0.0);
+      if (ACC) {
+        f.ap = mk3<S>(in.a(va), in.a(va + 1), in.a(va + 2));
+        f.al = f.R * mk3<S>(in.a(va + 3), in.a(va + 4), in.a(va + 5));
+      } else { f.ap = mk3<S>(z, z, z); f.al = f.ap; }
+      S one(1.0);
+      st3(ws.dax, va, mk3<S>(one, z, z)); st3(ws.dax, va + 1, mk3<S>(z, one, z)); st3(ws.dax, va + 2, mk3<S>(z, z, one));
+#pragma unroll
+      for (int c = 0; c < 3; ++c) { st3(ws.dan, va + c, f.p); st3(ws.dax, va + 3 + c, colv(f.R, c)); st3(ws.dan, va + 3 + c, f.p); }
+    }
+  }
+  st3(ws.fp, b, f.p); st9(ws.fR, b, f.R); st3(ws.fw, b, f.w); st3(ws.fal, b, f.al); st3(ws.fvp, b, f.vp); st3(ws.fap, b, f.ap);
+  st3(ws.com, b, f.p + f.R * c3<S>(m.body_ipos, b));
+}
+
+// Bodies of one tree level are independent: one lane per body, levels in order.
+template <class S, class R, int G, class IN, bool ACC>
+DMX_D void kinematics(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, const Grp<G>& gr) {
+  if (gr.lane == 0) {
+    S z(0.0), o(1.0);
+    V3<S> z3 = mk3<S>(z, z, z);
+    st3(ws.fp, 0, z3); st3(ws.fw, 0, z3); st3(ws.fal, 0, z3); st3(ws.fvp, 0, z3); st3(ws.fap, 0, z3); st3(ws.com, 0, z3);
+    M3<S> I; for (int k = 0; k < 9; ++k) I.m[k] = (k % 4 == 0) ? o : z;
+    st9(ws.fR, 0, I);
+  }
+  gr.sync();
+  for (int lv = 0; lv < m.nlevel; ++lv) {
+    for (int i = m.level_ptr[lv] + gr.lane; i < m.level_ptr[lv + 1]; i += G) body_kin<S, R, IN, ACC>(m, in, ws, m.level_body[i]);
+    gr.sync();
+  }
+}
+
+// linear velocity of the world point x fixed to a body per unit rate of dof j (j on the body's
+// path to the world)
+template <class S> DMX_DI V3<S> twist_lin(const Ws<S>& ws, int j, int rot, const V3<S>& x) {
+  V3<S> ax = ld3(ws.dax, j);
+  if (!rot) return ax;
+  return cross(ax, x - ld3(ws.dan, j));
+}
+
+// Newton-Euler wrench of body b about its centre of mass and its world inertia
+template <class S, class R, class IN>
+DMX_DI void body_wrench(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, int b, V3<S>& Fb, V3<S>& Nb, M3<S>& Iw) {
+  FrameT<S> f;
+  f.p = ld3(ws.fp, b); f.R = ld9(ws.fR, b); f.w = ld3(ws.fw, b); f.al = ld3(ws.fal, b); f.ap = ld3(ws.fap, b);
+  S mass = in.p(b);
+  V3<S> ac = point_acc(f, ld3(ws.com, b));
+  Fb = (ac - mk3<S>(S(m.gravity[0]), S(m.gravity[1]), S(m.gravity[2]))) * mass;
+  M3<S> Ri = f.R * c9<S>(m.body_irot, b);
+  M3<S> Dg;
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) Dg.m[3 * i + j] = Ri.m[3 * i + j] * (mass * S(m.body_iunit[3 * b + j]));
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) Iw.m[3 * i + j] = Dg.m[3 * i] * Ri.m[3 * j] + Dg.m[3 * i + 1] * Ri.m[3 * j + 1] + Dg.m[3 * i + 2] * Ri.m[3 * j + 2];
+  Nb = Iw * f.al + cross(f.w, Iw * f.w);
+}
+
+// ---- S2/S3: M(q), c(q,v), tau(x,u) ---------------------------------------------
+// M = sum_b m Jc^T Jc + Jw^T I Jw + diag(armature): the linear part is summed over the subtree
+// below the deeper dof from a (body, ancestor-dof) twist table; the angular part uses the summed
+// world inertias of that subtree.  c_j = sum_b lin_jb . F_b + ang_j . N_b (virtual work).
+template <class S, class R, int G, class IN>
+DMX_D void dynamics(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, const Grp<G>& gr) {
+  const int nv = m.nv, nb = m.nbody;
+  for (int b = 1 + gr.lane; b < nb; b += G) {
+    V3<S> Fb, Nb; M3<S> Iw;
+    body_wrench<S, R, IN>(m, in, ws, b, Fb, Nb, Iw);
+    st3(ws.Fb, b, Fb); st3(ws.Nb, b, Nb); st9(ws.Iw, b, Iw);
+  }
+  for (int e = gr.lane; e < m.ntw; e += G) {
+    int j = m.tw_dof[e];
+    st3(ws.tw, e, twist_lin(ws, j, m.dof_rot[j], ld3(ws.com, m.tw_body[e])));
+  }
+  gr.sync();
+  for (int i = gr.lane; i < 9 * (nb - 1); i += G) {
+    int b = 1 + i / 9, k = i % 9;
+    S acc(0.0);
+    for (int t = m.sub_ptr[b]; t < m.sub_ptr[b + 1]; ++t) acc = acc + ws.Iw[9 * m.sub_body[t] + k];
+    ws.Isub[9 * b + k] = acc;
+  }
+  gr.sync();
+  for (int e = gr.lane; e < m.nmp; e += G) {
+    int i = m.mp_i[e], j = m.mp_j[e], deep = m.mp_deep[e];
+    S acc(0.0);
+    if (deep >= 0) {
+      for (int t = m.sub_ptr[deep]; t < m.sub_ptr[deep + 1]; ++t) {
+        int b = m.sub_body[t];
+        acc = acc + in.p(b) * dot(ld3(ws.tw, m.tw_idx[b * nv + i]), ld3(ws.tw, m.tw_idx[b * nv + j]));
+      }
+      if (m.dof_rot[i] && m.dof_rot[j]) acc = acc + dot(ld3(ws.dax, i), ld9(ws.Isub, deep) * ld3(ws.dax, j));
+      if (i == j) acc = acc + S(m.jnt_armature[m.dof_jnt[i]]);
+    }
+    ws.M[i * nv + j] = acc; ws.M[j * nv + i] = acc;
+  }
+  for (int j = gr.lane; j < nv; j += G) {
+    int bj = m.dof_body[j], rot = m.dof_rot[j];
+    V3<S> ax = ld3(ws.dax, j);
+    S acc(0.0);
+    for (int t = m.sub_ptr[bj]; t < m.sub_ptr[bj + 1]; ++t) {
+      int b = m.sub_body[t];
+      acc = acc + dot(ld3(ws.tw, m.tw_idx[b * nv + j]), ld3(ws.Fb, b));
+      if (rot) acc = acc + dot(ax, ld3(ws.Nb, b));
+    }
+    ws.c[j] = acc;
+    S tau = -(S(m.jnt_damping[m.dof_jnt[j]]) * in.v(j));
+    for (int i = 0; i < m.nu; ++i) {
+      int jn = m.act_jnt[i];
+      if (m.jnt_vadr[jn] != j) continue;
+      if (m.act_type[i] == ACT_MOTOR) tau = tau + S(m.act_gear[i]) * in.u(i);
+      else tau = tau + S(m.act_kp[i]) * (in.u(i) - in.q(m.jnt_qadr[jn])) - S(m.act_kd[i]) * in.v(j);
+    }
+    ws.tau[j] = tau;
+  }
+  gr.sync();
+}
+
+// ---- dense Cholesky on the lower triangle, one column at a time, lanes over rows ---------------
+template <class S, int G> DMX_D bool cholesky(const Arr<S>& A, int n, const Grp<G>& gr) {
+  for (int j = 0; j < n; ++j) {
+    for (int i = j + gr.lane; i < n; i += G) {
+      S t = A[i * n + j];
+      for (int k = 0; k < j; ++k) t = t - A[i * n + k] * A[j * n + k];
+      A[i * n + j] = t;
+    }
+    gr.sync();
+    S s = A[j * n + j];
+    if (!(val(s) > 0)) return false;       // uniform over the group
+    S l = m_sqrt(s);
+    gr.sync();
+    for (int i = j + gr.lane; i < n; i += G) A[i * n + j] = (i == j) ? l : A[i * n + j] / l;
+    gr.sync();
+  }
+  return true;
+}
+// b <- (L L^T)^-1 b; column-oriented substitutions
+template <class S, int G> DMX_D void chol_solve(const Arr<S>& L, int n, const Arr<S>& b, const Grp<G>& gr) {
+  for (int i = 0; i < n; ++i) {
+    S bi = b[i] / L[i * n + i];
+    for (int k = i + 1 + gr.lane; k < n; k += G) b[k] = b[k] - L[k * n + i] * bi;
+    gr.sync();
+  }
+  for (int i = gr.lane; i < n; i += G) b[i] = b[i] / L[i * n + i];
+  gr.sync();
+  for (int i = n - 1; i >= 0; --i) {
+    S bi = b[i] / L[i * n + i];
+    for (int k = gr.lane; k < i; k += G) b[k] = b[k] - L[i * n + k] * bi;
+    gr.sync();
+  }
+  for (int i = gr.lane; i < n; i += G) b[i] = b[i] / L[i * n + i];
+  gr.sync();
+}
+
+// ---- S5: impedance d(r) from solimp (spline: SURVEY G5) and the CFD continuation --
+template <class S> DMX_DI S imp_spline(const S& x, const S& mid, const S& power) {
+  if (val(x) <= 0) return S(0.0) * x;
+  if (val(x) >= 1) return S(1.0) + S(0.0) * x;
+  S one(1.0);
+  if (val(x) <= val(mid)) return m_pow(x, power) / m_pow(mid, power - one);
+  return one - m_pow(one - x, power) / m_pow(one - mid, power - one);
+}
+template <class S> DMX_DI S clamp_imp(S d) {
+  if (val(d) < 0) d = S(0.0);
+  if (val(d) > 1.0 - 1e-4) d = S(1.0 - 1e-4);
+  return d;
+}
+template <class S> DMX_DI S impedance(const S& r, const S& d_o, const S& d_w, const S& w, const S& mid, const S& power) {
+  S ar = val(r) < 0 ? -r : r;
+  S x = ar / w;
+  if (val(x) > 1) x = S(1.0);
+  return clamp_imp(d_o + imp_spline(x, mid, power) * (d_w - d_o));
+}
+template <class S, class R> DMX_DI S impedance_cfd(const S& r, const R* sc) {   // (d_c, d_0, w_c, m_c, p_c)
+  S x = r / S(sc[2]);
+  return clamp_imp(S(sc[1]) + imp_spline(x, S(sc[3]), S(sc[4])) * S(sc[0] - sc[1]));
+}
+template <class S, class R> DMX_DI S softplus(const S& z, R beta) {
+  S bz = z * S(beta), one(1.0);
+  if (val(bz) > 0) return z + m_log(one + m_exp(-bz)) / S(beta);
+  return m_log(one + m_exp(bz)) / S(beta);
+}
+
+// ---- S4: narrow phase of one flattened candidate ----------
+template <class S> struct GeoT { S r; V3<S> n, pos, t1, t2; };
+template <class S, class R> DMX_DI GeoT<S> collide(const ModelDev<R>& m, const Ws<S>& ws, int c) {
+  GeoT<S> g;
+  int b2 = m.ct_b2[c];
+  V3<S> c2 = ld3(ws.fp, b2) + ld9(ws.fR, b2) * c3<S>(m.ct_p2, c);
+  S rho2(m.ct_rho2[c]);
+  if (m.ct_kind[c] == CK_POINT_PLANE) {
+    g.n = c3<S>(m.ct_n, c); g.t1 = c3<S>(m.ct_t1, c); g.t2 = c3<S>(m.ct_t2, c);
+    g.r = dot(g.n, c2 - c3<S>(m.ct_p1, c)) - rho2;
+    g.pos = c2 - g.n * (rho2 + S(0.5) * g.r);
+  } else {
+    int b1 = m.ct_b1[c];
+    V3<S> c1 = ld3(ws.fp, b1) + ld9(ws.fR, b1) * c3<S>(m.ct_p1, c);
+    V3<S> dl = c2 - c1;
+    S dist = m_sqrt(dot(dl, dl)), rho1(m.ct_rho1[c]);
+    g.n = dl * (S(1.0) / dist);
+    g.r = dist - rho1 - rho2;
+    g.pos = c1 + g.n * (rho1 + S(0.5) * g.r);
+    typename RealOf<S>::type ax = fabs(val(g.n.x)), ay = fabs(val(g.n.y)), az = fabs(val(g.n.z));
+    int e = 0; if (ay < ax) { e = 1; ax = ay; } if (az < ax) e = 2;
+    S z(0.0), o(1.0);
+    V3<S> ev = mk3<S>(e == 0 ? o : z, e == 1 ? o : z, e == 2 ? o : z);
+    V3<S> t = ev - g.n * dot(ev, g.n);
+    g.t1 = t * (S(1.0) / m_sqrt(dot(t, t)));
+    g.t2 = cross(g.n, g.t1);
+  }
+  return g;
+}
+
+// per-candidate scalars of Eq. 3 and the regulariser: D = d / (A^ (1-d)), position term of a_ref,
+// damping coefficient b.  cfd: impedance continued for r>0 and softplus.
+template <class S, class R, class IN>
+DMX_DI void candidate_terms(const ModelDev<R>& m, const IN& in, int c, const S& r, bool cfd, S& Dw, S& post, S& bdamp, S& mu) {
+  int pr = m.ct_pair[c];
+  int o = m.p_solimp + 5 * pr;
+  S d_o = in.p(o), d_w = in.p(o + 1), wid = in.p(o + 2), mid = in.p(o + 3), pw = in.p(o + 4);
+  S tc = in.p(m.p_solref + 2 * pr), phi = in.p(m.p_solref + 2 * pr + 1);
+  mu = in.p(m.p_fric + pr);
+  S kden = d_w * d_w * tc * tc * phi * phi;
+  S d;
+  if (cfd) {
+    d = val(r) > 0 ? impedance_cfd<S, R>(r, m.pair_solimp_cfd + 5 * pr) : impedance(r, d_o, d_w, wid, mid, pw);
+    post = (d / kden) * softplus<S, R>(-r, m.pair_cfd_beta[pr]);
+  } else {
+    d = impedance(r, d_o, d_w, wid, mid, pw);
+    post = -((d / kden) * r);
+  }
+  bdamp = S(2.0) / (d_w * tc);
+  S Ahat(m.pair_invweight[pr]);
+  if (m.ct_condim[c] == 3) Ahat = Ahat * (S(1.0) + mu * mu);
+  Dw = d / (Ahat * (S(1.0) - d));
+}
+
+// relative velocity of the contact point per unit rate of dof j, body2 minus body1
+template <class S, class R>
+DMX_DI V3<S> rel_twist(const ModelDev<R>& m, const Ws<S>& ws, int j, int b1, int b2, const V3<S>& pos) {
+  S z(0.0);
+  V3<S> d = mk3<S>(z, z, z);
+  int rot = m.dof_rot[j];
+  if (m.tw_idx[b2 * m.nv + j] >= 0) d = twist_lin(ws, j, rot, pos);
+  if (m.tw_idx[b1 * m.nv + j] >= 0) d = d - twist_lin(ws, j, rot, pos);
+  return d;
+}
+
+// ---- S4+S5: rows of every candidate with r<0 (cfd: r<w_c), compacted in candidate order ----------
+template <class S, class R, int G, class IN>
+DMX_D int build_rows(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, bool cfd, const Grp<G>& gr) {
+  const int nv = m.nv, nc = m.nc;
+  for (int c = gr.lane; c < nc; c += G) {
+    GeoT<S> g = collide<S, R>(m, ws, c);
+    ws.cr[c] = g.r; st3(ws.cn, c, g.n); st3(ws.cpos, c, g.pos); st3(ws.ct1, c, g.t1); st3(ws.ct2, c, g.t2);
+    bool inc = (val(g.r) < 0) || (cfd && val(g.r) < m.pair_solimp_cfd[5 * m.ct_pair[c] + 2]);
+    ws.incl[c] = inc ? (m.ct_condim[c] == 3 ? 4 : 1) : 0;
+    if (inc) {
+      S Dw, post, bd, mu;
+      candidate_terms<S, R, IN>(m, in, c, g.r, cfd, Dw, post, bd, mu);
+      ws.cD[c] = Dw; ws.cpost[c] = post; ws.cbd[c] = bd; ws.cmu[c] = mu;
+    }
+  }
+  gr.sync();
+  int nr = 0;
+  for (int c = 0; c < nc; ++c) {
+    int n = ws.incl[c];
+    if (gr.lane == 0) { ws.rowstart[c] = nr; for (int e = 0; e < n; ++e) ws.rowcand[nr + e] = 4 * c + e; }
+    nr += n;
+  }
+  gr.sync();
+  if (nr == 0) return 0;
+  // Jacobian entries: one (candidate, dof) item yields that candidate's 1 or 4 row entries
+  for (int it = gr.lane; it < nc * nv; it += G) {
+    int c = it / nv, j = it - c * nv;
+    int n = ws.incl[c];
+    if (n == 0) continue;
+    int r0 = ws.rowstart[c];
+    V3<S> d = rel_twist<S, R>(m, ws, j, m.ct_b1[c], m.ct_b2[c], ld3(ws.cpos, c));
+    S nd = dot(ld3(ws.cn, c), d);
+    if (n == 1) ws.J[r0 * nv + j] = nd;
+    else {
+      S mu = ws.cmu[c];
+      S t1d = mu * dot(ld3(ws.ct1, c), d), t2d = mu * dot(ld3(ws.ct2, c), d);
+      ws.J[r0 * nv + j] = nd + t1d; ws.J[(r0 + 1) * nv + j] = nd - t1d;
+      ws.J[(r0 + 2) * nv + j] = nd + t2d; ws.J[(r0 + 3) * nv + j] = nd - t2d;
+    }
+  }
+  gr.sync();
+  for (int i = gr.lane; i < nr; i += G) {
+    int c = ws.rowcand[i] >> 2;
+    S Jv(0.0);
+    for (int j = 0; j < nv; ++j) Jv = Jv + ws.J[i * nv + j] * in.v(j);
+    ws.aref[i] = ws.cpost[c] - ws.cbd[c] * Jv;
+    ws.D[i] = ws.cD[c];
+  }
+  gr.sync();
+  return nr;
+}
+
+// ---- S6: Newton with a fixed iteration budget on the reduced primal problem of Eq. 2 -------------
+//   Phi(x) = 1/2 (x-a0)^T M (x-a0) + 1/2 sum_i D_i min(0, J_i x - aref_i)^2
+// (iterations / ls_iterations PAPER.md:515, 539).
+// Returns true when the last step was a full step inside an unchanged active set.
+template <class S, int G>
+DMX_D bool newton(int nv, int nr, int n_it, int n_ls, const Ws<S>& ws, const Grp<G>& gr) {
+  for (int j = gr.lane; j < nv; j += G) ws.x[j] = ws.a0[j];
+  gr.sync();
+  if (nr == 0) return true;
+  bool conv = false;
+  for (int it = 0; it < n_it; ++it) {
+    for (int i = gr.lane; i < nr; i += G) {
+      S t(0.0);
+      for (int j = 0; j < nv; ++j) t = t + ws.J[i * nv + j] * ws.x[j];
+      ws.s[i] = t - ws.aref[i];
+    }
+    for (int j = gr.lane; j < nv; j += G) ws.xa[j] = ws.x[j] - ws.a0[j];
+    gr.sync();
+    for (int a = gr.lane; a < nv; a += G) {
+      S t(0.0);
+      for (int b = 0; b < nv; ++b) t = t + ws.M[a * nv + b] * ws.xa[b];
+      for (int i = 0; i < nr; ++i) if (val(ws.s[i]) < 0) t = t + ws.J[i * nv + a] * ws.D[i] * ws.s[i];
+      ws.g[a] = t; ws.dl[a] = -t;
+    }
+    for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
+      int a = 0; while ((a + 1) * (a + 2) / 2 <= e) ++a;
+      int b = e - a * (a + 1) / 2;
+      S t = ws.M[a * nv + b];
+      for (int i = 0; i < nr; ++i) if (val(ws.s[i]) < 0) t = t + ws.D[i] * ws.J[i * nv + a] * ws.J[i * nv + b];
+      ws.Hc[a * nv + b] = t;
+    }
+    gr.sync();
+    if (!cholesky<S, G>(ws.Hc, nv, gr)) break;
+    chol_solve<S, G>(ws.Hc, nv, ws.dl, gr);
+    bool same = true;
+    for (int i = gr.lane; i < nr; i += G) {
+      S t(0.0);
+      for (int j = 0; j < nv; ++j) t = t + ws.J[i * nv + j] * ws.dl[j];
+      ws.pr[i] = t;
+      if ((val(ws.s[i]) < 0) != (val(ws.s[i] + t) < 0)) same = false;
+    }
+    same = gr.all(same);
+    gr.sync();
+    S alpha(1.0);
+    if (!same) {
+      // D1: phi'(a) = dl^T M (x + a dl - a0) + sum_i D_i p_i min(0, s_i + a p_i); every lane runs the
+      // scalar line search redundantly in row order (same summation order as a serial code)
+      for (int a = gr.lane; a < nv; a += G) {
+        S t(0.0);
+        for (int b = 0; b < nv; ++b) t = t + ws.M[a * nv + b] * ws.dl[b];
+        ws.Md[a] = t;
+      }
+      gr.sync();
+      S dMd(0.0), dMxa(0.0);
+      for (int a = 0; a < nv; ++a) { dMd = dMd + ws.dl[a] * ws.Md[a]; dMxa = dMxa + ws.Md[a] * ws.xa[a]; }
+      S lo(0.0), hi(0.0), a(0.0), d2, d1a; bool hi_inf = true, frozen = false;
+      {
+        d1a = dMxa; d2 = dMd;
+        for (int i = 0; i < nr; ++i) { S si = ws.s[i]; if (val(si) < 0) { d1a = d1a + ws.D[i] * ws.pr[i] * si; d2 = d2 + ws.D[i] * ws.pr[i] * ws.pr[i]; } }
+      }
+      for (int ls = 0; ls < n_ls && !frozen; ++ls) {
+        S an = (ls == 0) ? S(1.0) : a - d1a / d2;
+        bool inside = (val(an) > val(lo)) && (hi_inf || val(an) < val(hi));
+        if (!inside) an = hi_inf ? S(2.0) * (val(a) > 1 ? a : S(1.0)) : S(0.5) * (lo + hi);
+        a = an;
+        d1a = dMxa + a * dMd; d2 = dMd;
+        for (int i = 0; i < nr; ++i) {
+          S si = ws.s[i] + a * ws.pr[i];
+          if (val(si) < 0) { d1a = d1a + ws.D[i] * ws.pr[i] * si; d2 = d2 + ws.D[i] * ws.pr[i] * ws.pr[i]; }
+        }
+        if (val(d1a) < 0) lo = a; else if (val(d1a) > 0) { hi = a; hi_inf = false; } else frozen = true;
+      }
+      alpha = a;
+    }
+    for (int j = gr.lane; j < nv; j += G) ws.x[j] = ws.x[j] + alpha * ws.dl[j];
+    gr.sync();
+    if (same) { conv = true; break; }
+  }
+  return conv;
+}
+
+// ---- F (cfd=false) or F~ (cfd=true) at one state: result in ws.x, rows and M left in ws ----------
+// returns nr >= 0, or -1 when M is not positive definite / the result is not finite
+template <class S, class R, int G, class IN>
+DMX_D int vector_field(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, bool cfd, bool& conv, const Grp<G>& gr) {
+  const int nv = m.nv;
+  kinematics<S, R, G, IN, false>(m, in, ws, gr);
+  dynamics<S, R, G, IN>(m, in, ws, gr);
+  for (int e = gr.lane; e < nv * nv; e += G) ws.Hc[e] = ws.M[e];
+  for (int j = gr.lane; j < nv; j += G) ws.a0[j] = ws.tau[j] - ws.c[j];
+  gr.sync();
+  conv = true;
+  if (!cholesky<S, G>(ws.Hc, nv, gr)) return -1;
+  chol_solve<S, G>(ws.Hc, nv, ws.a0, gr);
+  int nr = build_rows<S, R, G, IN>(m, in, ws, cfd, gr);
+  conv = newton<S, G>(nv, nr, m.newton_iters, m.ls_iters, ws, gr);
+  bool fin = true;
+  for (int j = gr.lane; j < nv; j += G) if (!isfinite(val(ws.x[j]))) fin = false;
+  if (!gr.all(fin)) return -1;
+  return nr;
+}
+
+// ---- S11/S12, cooperative part: final active set A, H = M + J_A^T D_A J_A, w = H^-1 kappa ---------
+// ws.kap holds kappa on entry and w on exit.  Returns false if H is not positive definite.
+template <class S, int G>
+DMX_D bool vjp_prepare(int nv, int nr, const Ws<S>& ws, const Grp<G>& gr) {
+  for (int i = gr.lane; i < nr; i += G) {
+    S t(0.0);
+    for (int j = 0; j < nv; ++j) t = t + ws.J[i * nv + j] * ws.x[j];
+    t = t - ws.aref[i];
+    ws.s[i] = t;
+    ws.active[i] = val(t) < 0 ? 1 : 0;
+  }
+  gr.sync();
+  for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
+    int a = 0; while ((a + 1) * (a + 2) / 2 <= e) ++a;
+    int b = e - a * (a + 1) / 2;
+    S t = ws.M[a * nv + b];
+    for (int i = 0; i < nr; ++i) if (ws.active[i]) t = t + ws.D[i] * ws.J[i * nv + a] * ws.J[i * nv + b];
+    ws.Hc[a * nv + b] = t;
+  }
+  gr.sync();
+  if (!cholesky<S, G>(ws.Hc, nv, gr)) return false;
+  chol_solve<S, G>(ws.Hc, nv, ws.kap, gr);
+  return true;
+}
+
+// ---- S11/S12, tangent part: one lane, one direction ----------------------------------------------
+// Directional derivative of  w^T g(z; x*)  with
+//   g = ID(q,v,x*) - tau(q,v,u) + sum_{i in A} J_i^T D_i (J_i x* - aref_i)      (stationarity of Eq. 2)
+// along the direction carried by `in`; x*, A, w and the row inclusion decisions are those of the
+// cooperative pass.  Uses the virtual-work identity  w^T ID = sum_b vel_w(com_b).F_b + omega_w(b).N_b
+// and, for the rows,  J_i y = dir_i . relvel_y(pos_i)  with y in {x*, v, w}.
+// dws: this lane's tangent workspace (frames only).
+template <class R, class IN>
+DMX_D R residual_tangent(const ModelDev<R>& m, const IN& in, const Ws<Dual<R> >& dws, const Arr<R>& w,
+                         const Arr<int>& incl, const Arr<int>& rowstart, const Arr<int>& active, bool cfd) {
+  typedef Dual<R> S;
+  const int nv = m.nv;
+  Grp<1> g1; g1.lane = 0; g1.mask = 0;
+  kinematics<S, R, 1, IN, true>(m, in, dws, g1);
+  S acc(R(0));
+  for (int b = 1; b < m.nbody; ++b) {
+    V3<S> Fb, Nb; M3<S> Iw;
+    body_wrench<S, R, IN>(m, in, dws, b, Fb, Nb, Iw);
+    V3<S> comb = ld3(dws.com, b);
+    S z(R(0));
+    V3<S> vw = mk3<S>(z, z, z), ow = vw;
+    for (int e = m.tw_ptr[b]; e < m.tw_ptr[b + 1]; ++e) {
+      int j = m.tw_dof[e], rot = m.dof_rot[j];
+      S wj(w[j]);
+      vw = vw + twist_lin(dws, j, rot, comb) * wj;
+      if (rot) ow = ow + ld3(dws.dax, j) * wj;
+    }
+    acc = acc + dot(vw, Fb) + dot(ow, Nb);
+  }
+  for (int j = 0; j < nv; ++j) {
+    S tau = -(S(m.jnt_damping[m.dof_jnt[j]]) * in.v(j));
+    for (int i = 0; i < m.nu; ++i) {
+      int jn = m.act_jnt[i];
+      if (m.jnt_vadr[jn] != j) continue;
+      if (m.act_type[i] == ACT_MOTOR) tau = tau + S(m.act_gear[i]) * in.u(i);
+      else tau = tau + S(m.act_kp[i]) * (in.u(i) - in.q(m.jnt_qadr[jn])) - S(m.act_kd[i]) * in.v(j);
+    }
+    acc = acc + S(w[j]) * (S(m.jnt_armature[m.dof_jnt[j]]) * in.a(j) - tau);
+  }
+  for (int c = 0; c < m.nc; ++c) {
+    int n = incl[c];
+    if (n == 0) continue;
+    int r0 = rowstart[c];
+    bool any = false;
+    for (int e = 0; e < n; ++e) any = any || active[r0 + e];
+    if (!any) continue;
+    GeoT<S> g = collide<S, R>(m, dws, c);
+    S Dw, post, bd, mu;
+    candidate_terms<S, R, IN>(m, in, c, g.r, cfd, Dw, post, bd, mu);
+    S z(R(0));
+    S nX = z, t1X = z, t2X = z, nV = z, t1V = z, t2V = z, nW = z, t1W = z, t2W = z;
+    int b1 = m.ct_b1[c], b2 = m.ct_b2[c];
+    for (int j = 0; j < nv; ++j) {
+      if (m.tw_idx[b2 * nv + j] < 0 && m.tw_idx[b1 * nv + j] < 0) continue;
+      V3<S> d = rel_twist<S, R>(m, dws, j, b1, b2, g.pos);
+      S nd = dot(g.n, d);
+      S xj = in.a(j), vj = in.v(j), wj(w[j]);
+      nX = nX + nd * xj; nV = nV + nd * vj; nW = nW + nd * wj;
+      if (n == 4) {
+        S t1d = dot(g.t1, d), t2d = dot(g.t2, d);
+        t1X = t1X + t1d * xj; t1V = t1V + t1d * vj; t1W = t1W + t1d * wj;
+        t2X = t2X + t2d * xj; t2V = t2V + t2d * vj; t2W = t2W + t2d * wj;
+      }
+    }
+    for (int e = 0; e < n; ++e) {
+      if (!active[r0 + e]) continue;
+      S JX = nX, JV = nV, JW = nW;
+      if (n == 4) {
+        S sg = (e & 1) ? -mu : mu;
+        if (e < 2) { JX = JX + sg * t1X; JV = JV + sg * t1V; JW = JW + sg * t1W; }
+        else { JX = JX + sg * t2X; JV = JV + sg * t2V; JW = JW + sg * t2W; }
+      }
+      S s = JX - (post - bd * JV);
+      acc = acc + JW * (Dw * s);
+    }
+  }
+  return acc.d;
+}
+
+// tangent of q (+) eps e_d at eps = 0: fills the seed of an InDual
+template <class R>
+DMX_DI void seed_direction(const ModelDev<R>& m, InDual<R>& in, int d) {
+  const int nv = m.nv;
+  in.dq0 = R(1); in.dq1 = in.dq2 = in.dq3 = R(0);
+  if (d < nv) {
+    in.kind = 0;
+    int j = m.dof_jnt[d], c = d - m.jnt_vadr[j], qa = m.jnt_qadr[j];
+    if (m.jnt_type[j] != JNT_FREE || c < 3) { in.idx = qa + c; return; }
+    in.idx = qa + 3;
+    R w0 = in.qa[qa + 3], w1 = in.qa[qa + 4], w2 = in.qa[qa + 5], w3 = in.qa[qa + 6];
+    R e0 = c == 3 ? R(0.5) : R(0), e1 = c == 4 ? R(0.5) : R(0), e2 = c == 5 ? R(0.5) : R(0);
+    in.dq0 = -w1 * e0 - w2 * e1 - w3 * e2;
+    in.dq1 = w0 * e0 + w2 * e2 - w3 * e1;
+    in.dq2 = w0 * e1 - w1 * e2 + w3 * e0;
+    in.dq3 = w0 * e2 + w1 * e1 - w2 * e0;
+  } else if (d < 2 * nv) { in.kind = 1; in.idx = d - nv; }
+  else if (d < 2 * nv + m.nu) { in.kind = 2; in.idx = d - 2 * nv; }
+  else { in.kind = 3; in.idx = d - 2 * nv - m.nu; }
+}
+
+}  // namespace dmx

@@ -1,0 +1,51 @@
+// dmx_inst.cuh — launcher definitions; each inst_*.cu instantiates them for one (real type, lanes)
+// pair so that the translation units compile in parallel.
+#pragma once
+#include "dmx_kernels.cuh"
+
+namespace dmx {
+
+template <class R, int G> cudaError_t launch_rollout(const ModelDev<R>& m, const RolloutArgs<R>& a, LaunchCfg c, cudaStream_t s) {
+  cudaError_t e = cudaFuncSetAttribute(rollout_kernel<R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+  if (e != cudaSuccess) return e;
+  rollout_kernel<R, G><<<c.grid, c.block, c.smem, s>>>(m, a);
+  return cudaGetLastError();
+}
+template <class R, int G> cudaError_t launch_backward(const ModelDev<R>& m, const BackwardArgs<R>& a, LaunchCfg c, cudaStream_t s) {
+  cudaError_t e = cudaFuncSetAttribute(backward_kernel<R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+  if (e != cudaSuccess) return e;
+  backward_kernel<R, G><<<c.grid, c.block, c.smem, s>>>(m, a);
+  return cudaGetLastError();
+}
+template <class R, int G> cudaError_t launch_field(const ModelDev<R>& m, const FieldArgs<R>& a, LaunchCfg c, cudaStream_t s) {
+  cudaError_t e = cudaFuncSetAttribute(field_kernel<R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+  if (e != cudaSuccess) return e;
+  field_kernel<R, G><<<c.grid, c.block, c.smem, s>>>(m, a);
+  return cudaGetLastError();
+}
+template <class R, int G> cudaError_t launch_invweight(const ModelDev<R>& m, const R* qpos0, const R* zero_v, R* body_w, const WsLayout& wl,
+                                                       const RkLayout& rl, LaunchCfg c, cudaStream_t s) {
+  cudaError_t e = cudaFuncSetAttribute(invweight_kernel<R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+  if (e != cudaSuccess) return e;
+  invweight_kernel<R, G><<<1, c.block, c.smem, s>>>(m, qpos0, zero_v, body_w, wl, rl);
+  return cudaGetLastError();
+}
+template <class R, int G> cudaError_t kernel_occupancy(int block, size_t smem_fwd, size_t smem_bwd, int* occ_fwd, int* occ_bwd) {
+  cudaError_t e = cudaFuncSetAttribute(rollout_kernel<R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fwd);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(backward_kernel<R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bwd);
+  if (e != cudaSuccess) return e;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_fwd, rollout_kernel<R, G>, block, smem_fwd);
+  if (e != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_bwd, backward_kernel<R, G>, block, smem_bwd);
+}
+
+}  // namespace dmx
+
+#define DMX_INSTANTIATE(R, G)                                                                                                  \
+  template cudaError_t dmx::launch_rollout<R, G>(const dmx::ModelDev<R>&, const dmx::RolloutArgs<R>&, dmx::LaunchCfg, cudaStream_t);   \
+  template cudaError_t dmx::launch_backward<R, G>(const dmx::ModelDev<R>&, const dmx::BackwardArgs<R>&, dmx::LaunchCfg, cudaStream_t); \
+  template cudaError_t dmx::launch_field<R, G>(const dmx::ModelDev<R>&, const dmx::FieldArgs<R>&, dmx::LaunchCfg, cudaStream_t);       \
+  template cudaError_t dmx::launch_invweight<R, G>(const dmx::ModelDev<R>&, const R*, const R*, R*, const dmx::WsLayout&,             \
+                                                   const dmx::RkLayout&, dmx::LaunchCfg, cudaStream_t);                             \
+  template cudaError_t dmx::kernel_occupancy<R, G>(int, size_t, size_t, int*, int*);

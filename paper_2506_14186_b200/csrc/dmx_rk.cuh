@@ -1,0 +1,313 @@
+// dmx_rk.cuh — embedded Runge-Kutta pair on the configuration manifold, PI step-size control and
+// the discrete adjoint through the accepted steps (PAPER.md:88 adaptive integration; :429 exact
+// quaternion integration; :347 Tsit5/Dopri5 and the PID controller; :431, 456
+// discretize-then-optimize).  Time, step size, the stage combinations, the error norm and the
+// controller are always fp64; the vector field runs in the model's real type R.
+#pragma once
+#include "dmx_field.cuh"
+
+namespace dmx {
+
+// ---- Butcher tableaus: index 0 Dopri5 (Dormand & Prince 1980), 1 Tsit5 (Tsitouras 2011)
+static __device__ const double TAB_A[2][7][7] = {
+    {{0},
+     {1.0 / 5},
+     {3.0 / 40, 9.0 / 40},
+     {44.0 / 45, -56.0 / 15, 32.0 / 9},
+     {19372.0 / 6561, -25360.0 / 2187, 64448.0 / 6561, -212.0 / 729},
+     {9017.0 / 3168, -355.0 / 33, 46732.0 / 5247, 49.0 / 176, -5103.0 / 18656},
+     {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84}},
+    {{0},
+     {0.161},
+     {-0.008480655492356989, 0.335480655492357},
+     {2.8971530571054935, -6.359448489975075, 4.3622954328695815},
+     {5.325864828439257, -11.748883564062828, 7.4955393428898365, -0.09249506636175525},
+     {5.86145544294642, -12.92096931784711, 8.159367898576159, -0.071584973281401, -0.028269050394068383},
+     {0.09646076681806523, 0.01, 0.4798896504144996, 1.379008574103742, -3.290069515436081, 2.324710524099774}}};
+// e = b - bhat; b is row 6 of a (FSAL)
+static __device__ const double TAB_E[2][7] = {
+    {35.0 / 384 - 5179.0 / 57600, 0.0, 500.0 / 1113 - 7571.0 / 16695, 125.0 / 192 - 393.0 / 640,
+     -2187.0 / 6784 - (-92097.0 / 339200), 11.0 / 84 - 187.0 / 2100, 0.0 - 1.0 / 40},
+    {-0.00178001105222577714, -0.0008164344596567469, 0.007880878010261995, -0.1447110071732629,
+     0.5823571654525552, -0.45808210592918697, 0.015151515151515152}};
+
+struct SolverOpts { int tableau; double rtol, atol, h0, pcoeff, icoeff, safety, fac_min, fac_max; int max_steps; };
+
+// ---- the retraction q (+) delta, the chart rate and their pullbacks (reading G10) ------
+DMX_DI void rotvec_to_quat(const double* d, double* e) {
+  double th2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2], th = sqrt(th2);
+  double s, c; sincos(0.5 * th, &s, &c);
+  double k = th < 1e-4 ? 0.5 - th2 / 48.0 : s / th;
+  e[0] = c; e[1] = k * d[0]; e[2] = k * d[1]; e[3] = k * d[2];
+}
+DMX_DI void cross3(const double* a, const double* b, double* r) {
+  r[0] = a[1] * b[2] - a[2] * b[1]; r[1] = a[2] * b[0] - a[0] * b[2]; r[2] = a[0] * b[1] - a[1] * b[0];
+}
+// joint jn of: qout = q (+) delta and K = chart_rate(delta, V)
+template <class R>
+DMX_DI void retract_joint(const ModelDev<R>& m, int jn, const Arr<double>& q, const Arr<double>& delta, const Arr<double>& V,
+                          const Arr<double>& qout, const Arr<double>& K) {
+  int qa = m.jnt_qadr[jn], va = m.jnt_vadr[jn];
+  if (m.jnt_type[jn] != JNT_FREE) { qout[qa] = q[qa] + delta[va]; K[va] = V[va]; return; }
+  double d[3], w[3], e[4], a[4], r[4];
+  for (int c = 0; c < 3; ++c) { qout[qa + c] = q[qa + c] + delta[va + c]; K[va + c] = V[va + c]; d[c] = delta[va + 3 + c]; w[c] = V[va + 3 + c]; }
+  for (int c = 0; c < 4; ++c) a[c] = q[qa + 3 + c];
+  rotvec_to_quat(d, e);
+  r[0] = a[0] * e[0] - a[1] * e[1] - a[2] * e[2] - a[3] * e[3];
+  r[1] = a[0] * e[1] + a[1] * e[0] + a[2] * e[3] - a[3] * e[2];
+  r[2] = a[0] * e[2] - a[1] * e[3] + a[2] * e[0] + a[3] * e[1];
+  r[3] = a[0] * e[3] + a[1] * e[2] - a[2] * e[1] + a[3] * e[0];
+  double n = sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2] + r[3] * r[3]);
+  for (int c = 0; c < 4; ++c) qout[qa + 3 + c] = r[c] / n;
+  // Theta' = dexp^-1_Theta(w) truncated after the B_2 term: w + 1/2 Theta x w + 1/12 Theta x (Theta x w)
+  double t1[3], t2[3]; cross3(d, w, t1); cross3(d, t1, t2);
+  for (int c = 0; c < 3; ++c) K[va + 3 + c] = w[c] + 0.5 * t1[c] + t2[c] / 12.0;
+}
+DMX_DI void rot_AB(const double* d, double& A, double& B, double& C) {
+  double th2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2], th = sqrt(th2);
+  double s, c; sincos(th, &s, &c);
+  bool sm = th < 1e-4;
+  A = sm ? 1.0 - th2 / 6.0 : s / th;
+  B = sm ? 0.5 - th2 / 24.0 : (1.0 - c) / th2;
+  C = sm ? 1.0 / 6.0 - th2 / 120.0 : (th - s) / (th2 * th);
+}
+// joint jn of: base += T^T Qbar (T = blockdiag(I, R(exp delta)^T)), dbar += Jr(delta)^T Qbar
+template <class R>
+DMX_DI void retract_pullback_joint(const ModelDev<R>& m, int jn, const Arr<double>& delta, const Arr<double>& Qbar,
+                                   const Arr<double>& base, const Arr<double>& dbar) {
+  int va = m.jnt_vadr[jn];
+  if (m.jnt_type[jn] != JNT_FREE) { base[va] += Qbar[va]; dbar[va] += Qbar[va]; return; }
+  double d[3], qb[3];
+  for (int c = 0; c < 3; ++c) { base[va + c] += Qbar[va + c]; dbar[va + c] += Qbar[va + c]; d[c] = delta[va + 3 + c]; qb[c] = Qbar[va + 3 + c]; }
+  double A, B, C; rot_AB(d, A, B, C);
+  // R qb = qb + A d x qb + B d x (d x qb);  Jr^T qb = qb + B d x qb + C d x (d x qb)   (K^T = -K)
+  double k1[3], k2[3]; cross3(d, qb, k1); cross3(d, k1, k2);
+  for (int c = 0; c < 3; ++c) { base[va + 3 + c] += qb[c] + A * k1[c] + B * k2[c]; dbar[va + 3 + c] += qb[c] + B * k1[c] + C * k2[c]; }
+}
+// joint jn of: Vbar += (dK/dV)^T Kbar, dbar += (dK/dTheta)^T Kbar
+template <class R>
+DMX_DI void chart_pullback_joint(const ModelDev<R>& m, int jn, const Arr<double>& delta, const Arr<double>& V, const Arr<double>& Kbar,
+                                 const Arr<double>& Vbar, const Arr<double>& dbar) {
+  int va = m.jnt_vadr[jn];
+  if (m.jnt_type[jn] != JNT_FREE) { Vbar[va] += Kbar[va]; return; }
+  double th[3], w[3], kb[3];
+  for (int c = 0; c < 3; ++c) { Vbar[va + c] += Kbar[va + c]; th[c] = delta[va + 3 + c]; w[c] = V[va + 3 + c]; kb[c] = Kbar[va + 3 + c]; }
+  double t1[3], t2[3], tw[3], a[3], b[3], c3v[3];
+  cross3(th, kb, t1); cross3(th, t1, t2);
+  for (int c = 0; c < 3; ++c) Vbar[va + 3 + c] += kb[c] - 0.5 * t1[c] + t2[c] / 12.0;
+  cross3(w, kb, a); cross3(th, w, tw); cross3(tw, kb, b); cross3(w, t1, c3v);
+  for (int c = 0; c < 3; ++c) dbar[va + 3 + c] += 0.5 * a[c] + b[c] / 12.0 - c3v[c] / 12.0;
+}
+
+// ---- per-environment fp64 integrator state in the group's workspace ---------------------------------
+struct RkLayout {
+  int q, v, Yq, V, Dl, K, A, err;            // forward (Yq, V, Dl: one stage; K, A: 7 stages)
+  int sYq, sV, sDl;                          // backward: 6 stages each
+  int Kb, Ab, qb, vb, dbar, Vb, lam, delta, qbar, vbar, ubar, pbar, gp;
+  int size_fwd, size_bwd;
+  int Yqr, Vr, rsize;                        // stage inputs in the real type R
+};
+struct Rk {
+  Arr<double> q, v, Yq, V, Dl, K, A, err, sYq, sV, sDl, Kb, Ab, qb, vb, dbar, Vb, lam, delta, qbar, vbar, ubar, pbar, gp;
+  DMX_DI void bind(const RkLayout& L, double* base, int st) {
+    Arr<double> b(base, st);
+    q = b.at(L.q); v = b.at(L.v); Yq = b.at(L.Yq); V = b.at(L.V); Dl = b.at(L.Dl); K = b.at(L.K); A = b.at(L.A); err = b.at(L.err);
+    sYq = b.at(L.sYq); sV = b.at(L.sV); sDl = b.at(L.sDl); Kb = b.at(L.Kb); Ab = b.at(L.Ab); qb = b.at(L.qb); vb = b.at(L.vb);
+    dbar = b.at(L.dbar); Vb = b.at(L.Vb); lam = b.at(L.lam); delta = b.at(L.delta); qbar = b.at(L.qbar); vbar = b.at(L.vbar);
+    ubar = b.at(L.ubar); pbar = b.at(L.pbar); gp = b.at(L.gp);
+  }
+};
+
+// ---- S7: one attempted step: stages 1..7 (stage 1 reused when have_k1), proposal, error vector -----
+// KEEP: also store every stage's (Yq, V, Dl) for the reverse sweep.
+template <class R, int G, bool KEEP>
+DMX_D void rk_attempt(const ModelDev<R>& m, int tab, const Rk& rk, const Arr<R>& Yqr, const Arr<R>& Vr, const R* u, const R* p,
+                      double h, bool have_k1, const Ws<R>& ws, bool& ok, int& unconverged, const Grp<G>& gr) {
+  const int nv = m.nv, nq = m.nq;
+  ok = true; unconverged = 0;
+  const int ns = KEEP ? 6 : 7;     // the reverse sweep needs stages 1..6 only
+  for (int i = 0; i < ns; ++i) {
+    for (int j = gr.lane; j < nv; j += G) {
+      double sq = 0, sv = 0;
+      for (int l = 0; l < i; ++l) { sq += TAB_A[tab][i][l] * rk.K[l * nv + j]; sv += TAB_A[tab][i][l] * rk.A[l * nv + j]; }
+      rk.Dl[j] = h * sq; rk.V[j] = rk.v[j] + h * sv;
+    }
+    gr.sync();
+    for (int jn = gr.lane; jn < m.njnt; jn += G) retract_joint<R>(m, jn, rk.q, rk.Dl, rk.V, rk.Yq, rk.K.at(i * nv));
+    gr.sync();
+    for (int j = gr.lane; j < nq; j += G) { Yqr[j] = (R)rk.Yq[j]; if (KEEP && i < 6) rk.sYq[i * nq + j] = rk.Yq[j]; }
+    for (int j = gr.lane; j < nv; j += G) {
+      Vr[j] = (R)rk.V[j];
+      if (KEEP && i < 6) { rk.sV[i * nv + j] = rk.V[j]; rk.sDl[i * nv + j] = rk.Dl[j]; }
+    }
+    gr.sync();
+    if (i == 0 && have_k1) continue;
+    InPlain<R> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
+    bool conv;
+    int nr = vector_field<R, R, G, InPlain<R> >(m, in, ws, false, conv, gr);
+    if (nr < 0) { ok = false; for (int j = gr.lane; j < nv; j += G) rk.A[i * nv + j] = nan(""); }
+    else { for (int j = gr.lane; j < nv; j += G) rk.A[i * nv + j] = (double)ws.x[j]; if (nr > 0 && !conv) unconverged++; }
+    gr.sync();
+  }
+  if (!KEEP) {
+    // row 6 of a is b: stage 7 is the proposal y_{n+1} = (Yq, V) and k7 = (V, A[6]) (FSAL)
+    for (int j = gr.lane; j < nv; j += G) {
+      double eq = 0, ev = 0;
+      for (int i = 0; i < 7; ++i) { eq += TAB_E[tab][i] * rk.K[i * nv + j]; ev += TAB_E[tab][i] * rk.A[i * nv + j]; }
+      rk.err[j] = h * eq; rk.err[nv + j] = h * ev;
+    }
+    gr.sync();
+  }
+}
+
+// ---- S8: scaled RMS error in index order with plain adds; every lane computes it -------
+template <class R>
+DMX_D double error_norm(const ModelDev<R>& m, const Rk& rk, double rtol, double atol, bool& finite) {
+  const int nv = m.nv;
+  double acc = 0.0;
+  for (int d = 0; d < nv; ++d) {
+    int j = m.dof_jnt[d], c = d - m.jnt_vadr[j];
+    double mag = 1.0;
+    if (m.jnt_type[j] != JNT_FREE || c < 3) { int qi = m.jnt_qadr[j] + c; mag = fmax(fabs(rk.q[qi]), fabs(rk.Yq[qi])); }
+    double e = rk.err[d];
+    if (!isfinite(e)) finite = false;
+    double r = __ddiv_rn(e, __dadd_rn(atol, __dmul_rn(rtol, mag)));
+    acc = __dadd_rn(acc, __dmul_rn(r, r));
+  }
+  for (int d = 0; d < nv; ++d) {
+    double e = rk.err[nv + d];
+    if (!isfinite(e)) finite = false;
+    double r = __ddiv_rn(e, __dadd_rn(atol, __dmul_rn(rtol, fmax(fabs(rk.v[d]), fabs(rk.V[d])))));
+    acc = __dadd_rn(acc, __dmul_rn(r, r));
+  }
+  return sqrt(acc / (2 * nv));
+}
+
+// ---- kernel arguments ------------------------------------------------------------------------------
+template <class R> struct RolloutArgs {
+  int nenv, nknot, n_replay, tape_cap, want_tape;
+  const R *x0, *ctrl, *params, *zero_u;
+  const double* h_replay;
+  double knot_dt, horizon;
+  SolverOpts so;
+  R* xT;
+  int *n_accept, *n_reject, *n_feval, *n_unconv, *status;
+  double *h_min, *h_max, *t_end;
+  int* tape_hdr;          // [nenv*2]: accepted steps on tape, final knot
+  R* tape;                // [nenv][tape_cap][nq+nv+2]
+  int* queue;
+  WsLayout wl; RkLayout rl;
+};
+
+// workspace bases of this thread's lane group inside the CTA's dynamic shared memory:
+// [doubles | reals | ints], each region holding all groups of the CTA
+template <class R, int G>
+DMX_DI void bind_shared(unsigned char* smem, int nd, int nr_, int ni, Rk& rk, Ws<R>& ws, Arr<R>& Yqr, Arr<R>& Vr,
+                        const RkLayout& rl, const WsLayout& wl) {
+  const int ngr = blockDim.x / G;
+  double* dreg = reinterpret_cast<double*>(smem);
+  R* rreg = reinterpret_cast<R*>(smem + (size_t)ngr * nd * sizeof(double));
+  int* ireg = reinterpret_cast<int*>(smem + (size_t)ngr * nd * sizeof(double) + (size_t)ngr * nr_ * sizeof(R));
+  int st; size_t gi;
+  if (G == 1) { st = 32; int w = threadIdx.x >> 5, l = threadIdx.x & 31; dreg += (size_t)w * 32 * nd + l; rreg += (size_t)w * 32 * nr_ + l; ireg += (size_t)w * 32 * ni + l; }
+  else { st = 1; gi = threadIdx.x / G; dreg += gi * nd; rreg += gi * nr_; ireg += gi * ni; }
+  rk.bind(rl, dreg, st);
+  ws.bind(wl, rreg, st, ireg, st);
+  Arr<R> rb(rreg, st);
+  Yqr = rb.at(rl.Yqr); Vr = rb.at(rl.Vr);
+}
+
+// ---- forward rollout: persistent lane groups pulling environments from a global queue --------------
+template <class R, int G>
+__global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ ModelDev<R> m, const __grid_constant__ RolloutArgs<R> a) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const Grp<G> gr = make_group<G>();
+  Rk rk; Ws<R> ws; Arr<R> Yqr, Vr;
+  bind_shared<R, G>(smem, a.rl.size_fwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, a.rl, a.wl);
+  const int nq = m.nq, nv = m.nv, nu = m.nu, nx = nq + nv, tab = a.so.tableau, rec = nx + 2;
+  const bool has_ctrl = a.ctrl != nullptr && a.nknot > 0 && nu > 0;
+  const int nknot = has_ctrl ? a.nknot : 0;
+  for (;;) {
+    int e = 0;
+    if (gr.lane == 0) e = atomicAdd(a.queue, 1);
+    e = gr.bcast_int(e);
+    if (e >= a.nenv) break;
+    const R* x0 = a.x0 + (size_t)e * nx;
+    const R* p = a.params ? a.params + (size_t)e * m.np : m.p_default;
+    for (int j = gr.lane; j < nq; j += G) rk.q[j] = (double)x0[j];
+    for (int j = gr.lane; j < nv; j += G) rk.v[j] = (double)x0[nq + j];
+    gr.sync();
+    double t = 0.0, hprop = a.so.h0, Eprev = 1.0, hmin = INFINITY, hmax = 0.0;
+    int knot = 0, attempts = 0, ir = 0, status = 0, n_acc = 0, n_rej = 0, n_feval = 0, n_unc = 0;
+    bool have_k1 = false, last_nonfinite = false;
+    const double* hr = a.h_replay ? a.h_replay + (size_t)e * a.n_replay : nullptr;
+    R* tape = a.want_tape ? a.tape + (size_t)e * a.tape_cap * rec : nullptr;
+    while (t < a.horizon) {
+      double tb = has_ctrl ? fmin((knot + 1) * a.knot_dt, a.horizon) : a.horizon;
+      if (knot + 1 >= nknot) tb = a.horizon;
+      const R* u = has_ctrl ? a.ctrl + ((size_t)e * nknot + knot) * nu : a.zero_u;
+      double rem = tb - t, h; bool hits;
+      if (hr) {
+        if (ir >= a.n_replay || !(hr[ir] > 0.0)) break;
+        h = hr[ir++]; hits = (h == rem);
+      } else {
+        if (attempts >= a.so.max_steps) { status = 1; break; }
+        if (hprop * (1.0 + 1e-7) >= rem) { h = rem; hits = true; } else { h = hprop; hits = false; }
+        if (!hits && h < 1e-14 * fmax(1.0, fabs(t))) { status = last_nonfinite ? 3 : 2; break; }
+      }
+      if (tape && n_acc >= a.tape_cap) { status = 4; break; }
+      attempts++;
+      bool ok; int unc;
+      rk_attempt<R, G, false>(m, tab, rk, Yqr, Vr, u, p, h, have_k1, ws, ok, unc, gr);
+      n_feval += have_k1 ? 6 : 7; n_unc += unc;
+      have_k1 = true;
+      bool finite = ok;
+      double E = error_norm<R>(m, rk, a.so.rtol, a.so.atol, finite);
+      bool accept = true;
+      last_nonfinite = !finite;
+      if (!hr) {
+        if (!finite) { E = INFINITY; accept = false; } else accept = E <= 1.0;
+        double Ec = fmax(E, 1e-30);
+        double fac = finite ? a.so.safety * exp(-(a.so.pcoeff + a.so.icoeff) / 5.0 * log(Ec)) * exp(a.so.pcoeff / 5.0 * log(Eprev)) : a.so.fac_min;
+        fac = fmin(a.so.fac_max, fmax(a.so.fac_min, fac));
+        if (!accept || !hits) hprop = h * fac;
+        if (accept) Eprev = Ec;
+      } else if (!finite) { status = 3; break; }
+      if (!accept) { n_rej++; continue; }
+      bool knot_up = hits && tb < a.horizon;
+      if (tape) {   // S9: checkpoint record (y_n, t_n, +-h_n); a negative h marks a step that ends a control interval
+        R* r = tape + (size_t)n_acc * rec;
+        for (int j = gr.lane; j < nq; j += G) r[j] = (R)rk.q[j];
+        for (int j = gr.lane; j < nv; j += G) r[nq + j] = (R)rk.v[j];
+        if (gr.lane == 0) { r[nx] = (R)t; r[nx + 1] = (R)(knot_up ? -h : h); }
+      }
+      gr.sync();
+      for (int j = gr.lane; j < nq; j += G) rk.q[j] = rk.Yq[j];
+      for (int j = gr.lane; j < nv; j += G) rk.v[j] = rk.V[j];
+      n_acc++; hmin = fmin(hmin, h); hmax = fmax(hmax, h);
+      if (hits) {
+        t = tb;
+        if (knot_up) { knot++; have_k1 = false; }
+      } else t += h;
+      if (have_k1) for (int j = gr.lane; j < nv; j += G) rk.A[j] = rk.A[6 * nv + j];
+      gr.sync();
+    }
+    R* xT = a.xT + (size_t)e * nx;
+    for (int j = gr.lane; j < nq; j += G) xT[j] = (R)rk.q[j];
+    for (int j = gr.lane; j < nv; j += G) xT[nq + j] = (R)rk.v[j];
+    if (gr.lane == 0) {
+      if (a.n_accept) a.n_accept[e] = n_acc;
+      if (a.n_reject) a.n_reject[e] = n_rej;
+      if (a.n_feval) a.n_feval[e] = n_feval;
+      if (a.n_unconv) a.n_unconv[e] = n_unc;
+      if (a.status) a.status[e] = status;
+      if (a.h_min) a.h_min[e] = hmin;
+      if (a.h_max) a.h_max[e] = hmax;
+      if (a.t_end) a.t_end[e] = t;
+      if (a.want_tape) { a.tape_hdr[2 * e] = n_acc; a.tape_hdr[2 * e + 1] = (status == 0) ? knot : -1 - knot; }
+    }
+    gr.sync();
+  }
+}
+
+}  // namespace dmx
