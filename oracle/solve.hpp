@@ -82,6 +82,7 @@ inline SolveResult contact_solve(int nv, int nr, const std::vector<double>& M, c
       bool frozen = false;
       for (int ls = 0; ls < n_ls && !frozen; ++ls) {
         double an = (ls == 0) ? 1.0 : a - d1a / d2;          // first iterate is exactly alpha = 1
+        if (ls > 0 && an == a) break;                        // D1 (amended): no representable progress -> root reached
         if (!(an > lo && an < hi)) an = std::isfinite(hi) ? 0.5 * (lo + hi) : 2.0 * std::fmax(a, 1.0);
         a = an; d1a = d1(a, d2);
         if (d1a < 0.0) lo = a; else if (d1a > 0.0) hi = a; else frozen = true;

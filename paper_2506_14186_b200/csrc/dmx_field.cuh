@@ -458,6 +458,7 @@ DMX_D bool newton(int nv, int nr, int n_it, int n_ls, const Ws<S>& ws, const Grp
       }
       for (int ls = 0; ls < n_ls && !frozen; ++ls) {
         S an = (ls == 0) ? S(1.0) : a - d1a / d2;
+        if (ls > 0 && val(an) == val(a)) break;      // no representable progress: the root of phi' is reached
         bool inside = (val(an) > val(lo)) && (hi_inf || val(an) < val(hi));
         if (!inside) an = hi_inf ? S(2.0) * (val(a) > 1 ? a : S(1.0)) : S(0.5) * (lo + hi);
         a = an;

@@ -20,6 +20,7 @@ DOPRI5, TSIT5 = 0, 1
 SOLIMP_DEFAULT = (0.0, 0.95, 0.001, 0.5, 2.0)
 SOLIMP_CFD_ON = (0.1, 0.95, 0.001, 0.5, 2.0)
 SOLIMP_CFD = (0.0, 0.1, 1.0, 1.0, 4.0)             # PAPER.md:537 (d_c, d_0, w_c, m_c, p_c)
+SOLIMP_CFD_SMOOTH = (0.01, 0.0, 1.0, 1.0, 4.0)     # PAPER.md:515 ("d_c=0.01, d_0=0 with w_c=1 m"), pairs with d_o=0
 
 
 class SplitMix64:
@@ -94,7 +95,10 @@ class ModelBuilder:
     def pair(self, g1, g2, condim=3, friction=1.0, solref=(0.002, 1.0), solimp=SOLIMP_DEFAULT,
              solimp_cfd=SOLIMP_CFD, cfd_beta=None):
         if cfd_beta is None:
-            cfd_beta = 10.0 / solimp_cfd[2]          # reading G17
+            # reading G17: the softplus turns on over the contact's own length scale, the solimp
+            # width.  A sharpness tied to w_c instead (10/w_c) offsets a_ref by ln2/beta = 7 cm at w_c = 1 m,
+            # which times the impedance slope makes the backward pass of F~ unstable at the forward step sizes.
+            cfd_beta = 1.0 / solimp[2]
         self.pairs.append(dict(g1=g1, g2=g2, condim=condim, friction=friction, solref=solref, solimp=solimp,
                                solimp_cfd=solimp_cfd, cfd_beta=cfd_beta))
         return len(self.pairs) - 1
@@ -258,7 +262,9 @@ def arm_target(nenv=16384, horizon=2.0, seed=250614186 + 4):
     sp = mb.body(0, pos=(0.45, 0, 0.04), mass=0.2, inertia_unit=sphere_inertia(0.04))
     mb.joint(sp, JNT_FREE)
     gs = mb.geom(sp, GEOM_SPHERE, size=(0.04,))
-    kw = dict(condim=3, friction=0.8, solimp=SOLIMP_CFD_ON)
+    # d_o = 0 keeps the contact force continuous at r=0 (with d_o>0 the resting arm chatters
+    # across the force jump and exhausts the step budget); CFD continuation d_0=0 -> d_c=0.01
+    kw = dict(condim=3, friction=0.8, solimp=SOLIMP_DEFAULT, solimp_cfd=SOLIMP_CFD_SMOOTH)
     for i in range(2, 7):
         mb.pair(gp, caps[i], **kw)
     mb.pair(gtip, gs, **kw)
