@@ -42,7 +42,7 @@ def build(force=False, verbose=False):
         logs = list(ex.map(cc, jobs))
     objs = [os.path.join(OBJ, s[:-3] + ".o") for s in _sources()]
     if jobs or not os.path.exists(LIB):
-        subprocess.check_call([NVCC, "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"])
+        subprocess.check_call([NVCC, "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a", "-cudart", "static"])
     if verbose:
         for (src, _), lg in zip(jobs, logs):
             sys.stderr.write("== %s\n%s\n" % (src, lg))

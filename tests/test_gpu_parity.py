@@ -1,0 +1,309 @@
+"""GPU parity tests (run with -m gpu on the B200 box): the CUDA path, called through the C-ABI binding, against the
+CPU fp64 oracle on the same seeded inputs, element by element.
+
+Tolerances (BASELINE.json north_star): fp64 final states 1e-9 relative to state scale and gradients 1e-6
+relative, on identical accepted-step sequences; fp32 1e-4 / 1e-3.  Identical sequences are obtained with the
+replay input (h schedule recorded by the oracle); free-running step counts are compared
+separately because the error estimate is rounding noise wherever the method integrates exactly (C1 free fall).
+"""
+import numpy as np
+import pytest
+
+import helpers as H
+from paper_2506_14186_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_X64, TOL_G64, TOL_X32, TOL_G32 = 1e-9, 1e-6, 1e-4, 1e-3
+# sizes the oracle finishes in seconds that still span several CTAs and a ragged tail
+SMALL = dict(C1=dict(nenv=77), C2=dict(nenv=45, horizon=0.2), C3=dict(nenv=53), C4=dict(nenv=5, horizon=0.4), C5=dict(nenv=5, horizon=0.3))
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2506_14186_b200 import binding
+    binding.load()
+    return binding
+
+
+def _oracle_run(orc, w, cfd=False, grads=True, threads=8):
+    of = orc.rollout(w["x0"], w["ctrl"], w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], threads=threads, n_hout=1)
+    nmax = int(of["stats"]["n_accept"].max())
+    of = orc.rollout(w["x0"], w["ctrl"], w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], threads=threads, n_hout=nmax + 1)
+    _, g = w["loss_grad"](of["xT"], w["x0"])
+    og = None
+    if grads:
+        og = orc.rollout_grad(w["x0"], w["ctrl"], w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], dLdxT=g, cfd_on=cfd, threads=threads)
+    return of, g, og, nmax
+
+
+def _rel_state_err(a, b):
+    scale = np.maximum(1.0, np.abs(b).max(axis=1))
+    return np.abs(a - b).max(axis=1) / scale
+
+
+def _rel_grad_err(a, b):
+    n = a.shape[0]
+    a, b = a.reshape(n, -1), b.reshape(n, -1)
+    return np.abs(a - b).max(axis=1) / np.maximum(np.abs(b).max(axis=1), 1e-300)
+
+
+# ---- S1-S6, S11, S12: one evaluation of F / F~ and its VJP -------------------------------------------------------
+def _contact_states(cfg, n, rng):
+    w = W.make(cfg, nenv=n)
+    model = w["model"]; nq, nv = model["nq"], model["nv"]
+    xs = w["x0"].copy()
+    if cfg == "C1": xs[:, 0] = rng.uniform(0.09, 0.11, size=n)
+    if cfg == "C3": xs[:, 2] = rng.uniform(0.03, 0.09, size=n)
+    if cfg == "C5": xs[:, 2] = rng.uniform(0.28, 0.34, size=n)
+    if cfg == "C4": xs[:, 9] = rng.uniform(0.035, 0.045, size=n); xs[:, 0:7] = rng.uniform(-2, 2, size=(n, 7))
+    if cfg == "C2": xs[:, 4] = rng.uniform(0.0485, 0.0505, size=n)
+    xs[:, nq:] = rng.normal(size=(n, nv))
+    us = w["ctrl"][:, 0, :].copy() if w["ctrl"] is not None else None
+    return model, xs, us
+
+
+@pytest.mark.parametrize("cfd", [False, True])
+@pytest.mark.parametrize("cfg", ["C1", "C2", "C3", "C4", "C5"])
+def test_vector_field_and_vjp_match_oracle(B, oracle_mod, cfg, cfd):
+    rng = np.random.default_rng(7)
+    n = 24
+    model, xs, us = _contact_states(cfg, n, rng)
+    orc = oracle_mod.Oracle(model); m = B.Model(model)
+    p = orc.default_params()
+    assert np.array_equal(p, m.default_params())
+    x = m.dev(xs); u = m.dev(us)
+    acc, nrow = m.vector_field(x, u, None, cfd)
+    acc, nrow = acc.cpu().numpy(), nrow.cpu().numpy()
+    kap = rng.normal(size=(n, orc.nv))
+    qb, vb, ub, pb = [t.cpu().numpy() for t in m.vjp_field(x, u, None, m.dev(kap), cfd)]
+    rows_seen = 0
+    for i in range(n):
+        ui = None if us is None else us[i]
+        a, nr, _ = orc.vector_field(xs[i, :orc.nq], xs[i, orc.nq:], ui, p, cfd)
+        assert nr == nrow[i]
+        rows_seen += nr
+        assert np.abs(a - acc[i]).max() <= 1e-10 * max(1.0, np.abs(a).max())
+        o = orc.vjp_field(xs[i, :orc.nq], xs[i, orc.nq:], ui, p, kap[i], cfd)
+        for ref, got in zip(o, (qb[i], vb[i], ub[i], pb[i])):
+            if len(ref):
+                assert np.abs(ref - got).max() <= 1e-8 * max(1e-3, np.abs(ref).max())
+    assert rows_seen > 0
+
+
+# ---- S7-S10: rollouts and reverse sweep, identical step sequences -----------------------------------------------------
+@pytest.mark.parametrize("cfg", ["C1", "C2", "C3", "C4", "C5"])
+def test_rollout_and_gradient_replay_parity_fp64(B, oracle_mod, cfg):
+    import torch
+    w = W.make(cfg, **SMALL[cfg])
+    nenv = w["nenv"]
+    orc = oracle_mod.Oracle(w["model"]); m = B.Model(w["model"])
+    of, g, og, nmax = _oracle_run(orc, w, cfd=False)
+    x0, ctrl = m.dev(w["x0"]), m.dev(w["ctrl"])
+    stats = m.alloc_stats(nenv)
+    tape = m.alloc_tape(nenv, nmax + 8)
+    hrep = m.dev(of["h"], dtype=torch.float64)
+    out = m.rollout_grad(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], m.dev(g), False, tape, h_replay=hrep, stats=stats)
+    assert (stats["status"].cpu().numpy() == 0).all()
+    assert np.array_equal(stats["n_accept"].cpu().numpy(), of["stats"]["n_accept"])
+    assert np.array_equal(stats["t_end"].cpu().numpy(), of["stats"]["t_end"])
+    assert _rel_state_err(out["xT"].cpu().numpy(), of["xT"]).max() <= TOL_X64
+    for k in ("dLdx0", "dLdctrl", "dLdparams"):
+        if og[k] is None:
+            continue
+        ref, got = og[k], out[k].cpu().numpy()
+        big = np.abs(ref.reshape(nenv, -1)).max(axis=1) > 1e-6          # relative error is meaningless on a vanished gradient
+        e = _rel_grad_err(got, ref)
+        assert e[big].max(initial=0.0) <= TOL_G64, k
+        assert np.abs(got - ref).reshape(nenv, -1).max(axis=1)[~big].max(initial=0.0) <= 1e-12, k
+
+
+@pytest.mark.parametrize("cfg", ["C2", "C4"])
+def test_cfd_gradient_replay_parity_and_forward_invariance(B, oracle_mod, cfg):
+    """S12: CFD changes gradients only; xT, stats and the tape are bit-identical with the flag on or off."""
+    import torch
+    kw = dict(SMALL[cfg]) if cfg != "C4" else dict(nenv=4, horizon=0.6)   # C4: long enough for the tip to come within w_c
+    w = W.make(cfg, **kw)
+    nenv = w["nenv"]
+    orc = oracle_mod.Oracle(w["model"]); m = B.Model(w["model"])
+    of, g, og, nmax = _oracle_run(orc, w, cfd=True)
+    x0, ctrl = m.dev(w["x0"]), m.dev(w["ctrl"])
+    hrep = m.dev(of["h"], dtype=torch.float64)
+    res = []
+    for cfd in (True, False):
+        stats = m.alloc_stats(nenv); tape = m.alloc_tape(nenv, nmax + 8); tape.zero_()
+        out = m.rollout_grad(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], m.dev(g), cfd, tape, h_replay=hrep, stats=stats)
+        torch.cuda.synchronize()
+        res.append((out, stats, tape))
+    (on, st_on, tp_on), (off, st_off, tp_off) = res
+    assert torch.equal(on["xT"], off["xT"]) and torch.equal(tp_on, tp_off)
+    for k in st_on:
+        assert torch.equal(st_on[k], st_off[k]), k
+    assert _rel_state_err(on["xT"].cpu().numpy(), of["xT"]).max() <= TOL_X64
+    for k in ("dLdx0", "dLdctrl", "dLdparams"):
+        e = _rel_grad_err(on[k].cpu().numpy(), og[k])
+        assert e.max() <= TOL_G64, k
+    # the flag does something: control gradients differ (envs that miss the target have zero non-CFD gradient)
+    assert not torch.equal(on["dLdctrl"], off["dLdctrl"])
+    assert np.abs(og["dLdctrl"]).max() > 0
+
+
+@pytest.mark.parametrize("cfg", ["C1", "C2", "C3", "C4", "C5"])
+def test_free_running_controller_matches_oracle(B, oracle_mod, cfg):
+    """S8: free-running accept/reject sequences.  Where they coincide the fp64 tolerance must hold; step counts are
+    compared either way (they differ only through rounding of the error estimate)."""
+    w = W.make(cfg, **SMALL[cfg])
+    nenv = w["nenv"]
+    orc = oracle_mod.Oracle(w["model"]); m = B.Model(w["model"])
+    of, g, _, nmax = _oracle_run(orc, w, grads=False)
+    stats = m.alloc_stats(nenv)
+    xT = m.rollout(m.dev(w["x0"]), m.dev(w["ctrl"]), w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], stats=stats)
+    na, nr = stats["n_accept"].cpu().numpy(), stats["n_reject"].cpu().numpy()
+    assert (stats["status"].cpu().numpy() == 0).all()
+    assert np.array_equal(stats["t_end"].cpu().numpy(), np.full(nenv, w["horizon"]))
+    same = (na == of["stats"]["n_accept"]) & (nr == of["stats"]["n_reject"])
+    err = _rel_state_err(xT.cpu().numpy(), of["xT"])
+    print("%s: %d/%d envs with identical step counts; accepted mean gpu %.1f oracle %.1f; xT err matching %.2e all median %.2e"
+          % (cfg, same.sum(), nenv, na.mean(), of["stats"]["n_accept"].mean(), err[same].max(initial=0.0), np.median(err)))
+    assert abs(na.mean() - of["stats"]["n_accept"].mean()) <= 0.1 * of["stats"]["n_accept"].mean() + 2
+    if cfg == "C2":                              # knot-limited steps: every decision coincides
+        assert same.mean() > 0.9
+        assert err[same].max() <= 10 * TOL_X64
+
+
+def test_fp32_variant_replay_parity(B, oracle_mod):
+    """C3 fp32: stage arithmetic in float, controller and accumulation fp64, on the oracle's schedule."""
+    import torch
+    w = W.make("C3", nenv=40, horizon=0.4)
+    nenv = w["nenv"]
+    orc = oracle_mod.Oracle(w["model"]); m = B.Model(w["model"], precision=32)
+    of, g, og, nmax = _oracle_run(orc, w)
+    stats = m.alloc_stats(nenv); tape = m.alloc_tape(nenv, nmax + 8)
+    hrep = m.dev(of["h"], dtype=torch.float64)
+    out = m.rollout_grad(m.dev(w["x0"]), None, 0, 0.0, None, w["horizon"], w["opts"], m.dev(g), False, tape, h_replay=hrep, stats=stats)
+    assert out["xT"].dtype == torch.float32
+    ex = _rel_state_err(out["xT"].double().cpu().numpy(), of["xT"])
+    eg = _rel_grad_err(out["dLdx0"].double().cpu().numpy(), og["dLdx0"])
+    unc = stats["n_newton_unconverged"].cpu().numpy()
+    print("fp32 C3: xT err median %.2e max %.2e; grad err median %.2e max %.2e; unconverged evals/env %.1f" % (np.median(ex), ex.max(), np.median(eg), eg.max(), unc.mean()))
+    # a tumbling cube amplifies fp32 rounding through every impact; the bulk must be inside the fp32 tolerance
+    assert np.median(ex) <= TOL_X32 and np.median(eg) <= TOL_G32
+    assert (ex <= 100 * TOL_X32).mean() >= 0.8
+
+
+# ---- invariants at any size ---------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg", ["C1", "C3", "C5"])
+def test_batch_independence_bitwise(B, cfg):
+    """P12: an env's outputs are bit-identical alone, in a small batch, in any order."""
+    import torch
+    kw = dict(SMALL[cfg]); kw["nenv"] = 64
+    w = W.make(cfg, **kw)
+    m = B.Model(w["model"])
+    x0, ctrl = m.dev(w["x0"]), m.dev(w["ctrl"])
+    full = m.rollout(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"])
+    perm = torch.randperm(64, generator=torch.Generator().manual_seed(1)).to(x0.device)
+    sub = perm[:9]
+    part = m.rollout(x0[sub].contiguous(), None if ctrl is None else ctrl[sub].contiguous(), w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"])
+    assert torch.equal(part, full[sub])
+    one = m.rollout(x0[5:6].contiguous(), None if ctrl is None else ctrl[5:6].contiguous(), w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"])
+    assert torch.equal(one[0], full[5])
+
+
+def test_full_size_launch_sampled_against_oracle(B, oracle_mod):
+    """BASELINE config 2 at full size (4096 envs) in the launch configuration bench.py times: sampled envs are compared
+    with the oracle one by one; the rest through batch independence (bitwise equal to the same env run alone)."""
+    import torch
+    w = W.make("C2")
+    assert w["nenv"] == 4096
+    orc = oracle_mod.Oracle(w["model"]); m = B.Model(w["model"])
+    x0, ctrl = m.dev(w["x0"]), m.dev(w["ctrl"])
+    stats = m.alloc_stats(4096)
+    tape = m.alloc_tape(4096, 1024)
+    _, g = w["loss_grad"](w["x0"], w["x0"])
+    xT = m.rollout(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], stats=stats, tape=tape)
+    _, gT = w["loss_grad"](xT.cpu().numpy(), w["x0"])
+    out = m.rollout_backward(ctrl, w["nknot"], None, w["opts"], xT, m.dev(gT), True, tape, want_params=False)
+    assert (stats["status"].cpu().numpy() == 0).all()
+    idx = np.array([0, 1, 1023, 2048, 3000, 4095])
+    sub = {k: (v[idx] if isinstance(v, np.ndarray) and v.shape[:1] == (4096,) else v) for k, v in w.items()}
+    of = orc.rollout(sub["x0"], sub["ctrl"], w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], threads=6)
+    na = stats["n_accept"].cpu().numpy()[idx]
+    same = na == of["stats"]["n_accept"]
+    assert same.mean() >= 0.5
+    assert _rel_state_err(xT.cpu().numpy()[idx], of["xT"])[same].max() <= 10 * TOL_X64
+    og = orc.rollout_grad(sub["x0"], sub["ctrl"], w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], dLdxT=gT[idx], cfd_on=True, threads=6, want_params=False)
+    e = _rel_grad_err(out["dLdctrl"].cpu().numpy()[idx], og["dLdctrl"])
+    assert e[same].max() <= 100 * TOL_G64       # free-running: states agree to 1e-8, so gradients to a few 1e-7 .. 1e-5
+
+
+# ---- edge cases ------------------------------------------------------------------------------------------------------
+def test_edge_cases_status_and_empty(B):
+    import torch
+    w = W.make("C1", nenv=3)
+    m = B.Model(w["model"])
+    x0 = m.dev(w["x0"])
+    # zero horizon: no steps, xT = x0
+    st = m.alloc_stats(3)
+    xT = m.rollout(x0, None, 0, 0.0, None, 0.0, w["opts"], stats=st)
+    assert torch.equal(xT, x0) and (st["n_accept"] == 0).all() and (st["status"] == 0).all()
+    # step budget: status 1, last accepted state returned, t_end < horizon
+    o = dict(w["opts"]); o["max_steps"] = 5
+    st = m.alloc_stats(3)
+    m.rollout(x0, None, 0, 0.0, None, w["horizon"], o, stats=st)
+    assert (st["status"] == 1).all() and (st["t_end"] < w["horizon"]).all() and ((st["n_accept"] + st["n_reject"]) == 5).all()
+    # tape too small for the accepted steps: status 4 and zero gradients
+    st = m.alloc_stats(3); tape = m.alloc_tape(3, 4)
+    g = torch.ones_like(x0)
+    out = m.rollout_grad(x0, None, 0, 0.0, None, w["horizon"], w["opts"], g, False, tape, stats=st)
+    assert (st["status"] == 4).all() and (out["dLdx0"] == 0).all() and (out["dLdparams"] == 0).all()
+    # non-finite input: status 3, no trap
+    bad = x0.clone(); bad[1, 0] = float("nan")
+    st = m.alloc_stats(3)
+    m.rollout(bad, None, 0, 0.0, None, w["horizon"], w["opts"], stats=st)
+    s = st["status"].cpu().numpy()
+    assert s[1] == 3 and s[0] == 0 and s[2] == 0
+    # invalid arguments fail the call
+    with pytest.raises(RuntimeError):
+        m.rollout(x0, None, 0, 0.0, None, w["horizon"], dict(w["opts"], tableau=7))
+    with pytest.raises(RuntimeError):
+        m.rollout_grad(x0, None, 0, 0.0, None, w["horizon"], w["opts"], g, False, torch.empty(8, dtype=torch.uint8, device=x0.device))
+
+
+def test_custom_models_box_arm_spheres(B, oracle_mod):
+    """Models outside the five configs (offset COM box, oblique slide/hinge arm with armature, sphere-sphere billiard)."""
+    import torch
+    rng = np.random.default_rng(3)
+    cases = [H.free_box(gravity=(0, 0, -9.81), with_plane=True), H.arm(4, with_contacts=True, slide_last=True, damping=0.2), H.two_spheres()]
+    for model in cases:
+        orc = oracle_mod.Oracle(model); m = B.Model(model)
+        nq, nv, nu = orc.nq, orc.nv, orc.nu
+        n = 6
+        x0 = np.zeros((n, nq + nv))
+        x0[:, :nq] = model["qpos0"]
+        for j, t in enumerate(model["jnt_type"]):
+            qa = model["jnt_qadr"][j]
+            if t == W.JNT_FREE:
+                for i in range(n):
+                    x0[i, qa + 3:qa + 7] = H.rand_quat(rng)
+                if model["npair"] and model["nbody"] == 2:
+                    x0[:, qa + 2] = rng.uniform(0.1, 0.2, size=n)
+            else:
+                x0[:, qa] = rng.uniform(-1, 1, size=n)
+        x0[:, nq:] = 0.5 * rng.normal(size=(n, nv))
+        if model["nbody"] == 3 and model["njnt"] == 2:          # billiard: roll sphere a into sphere b
+            x0[:, nq:] = 0.0; x0[:, nq] = rng.uniform(0.5, 1.5, size=n); x0[:, 1] = rng.uniform(-0.02, 0.02, size=n)
+        nknot, knot_dt, T = (4, 0.05, 0.2) if nu else (0, 0.0, 0.2)
+        ctrl = rng.normal(size=(n, nknot, nu)) if nu else None
+        opts = W.default_opts(W.TSIT5, 1e-7, 1e-7)
+        of = orc.rollout(x0, ctrl, nknot, knot_dt, None, T, opts, n_hout=4000)
+        g = rng.normal(size=x0.shape)
+        og = orc.rollout_grad(x0, ctrl, nknot, knot_dt, None, T, opts, dLdxT=g, cfd_on=True)
+        st = m.alloc_stats(n); tape = m.alloc_tape(n, 4000)
+        out = m.rollout_grad(m.dev(x0), m.dev(ctrl), nknot, knot_dt, None, T, opts, m.dev(g), True, tape,
+                             h_replay=m.dev(of["h"], dtype=torch.float64), stats=st)
+        assert _rel_state_err(out["xT"].cpu().numpy(), of["xT"]).max() <= TOL_X64
+        for k in ("dLdx0", "dLdctrl", "dLdparams"):
+            if og[k] is not None:
+                assert _rel_grad_err(out[k].cpu().numpy(), og[k]).max() <= TOL_G64, k
