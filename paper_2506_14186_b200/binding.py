@@ -10,7 +10,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libdmx.so")
+LIB_PATH = os.environ.get("DMX_LIB", os.path.join(_HERE, "libdmx.so"))
 
 SYMBOLS = ["dmx_model_create", "dmx_model_destroy", "dmx_model_np", "dmx_model_nc", "dmx_model_default_params",
            "dmx_model_lanes", "dmx_tape_bytes", "dmx_rollout", "dmx_rollout_grad", "dmx_rollout_backward",

@@ -10,7 +10,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libdmx.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
-         "-diag-suppress", "128"]
+         "-diag-suppress", "128"] + os.environ.get("DMX_NVCC_FLAGS", "").split()
 
 
 def _sources():

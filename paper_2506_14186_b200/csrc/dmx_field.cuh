@@ -11,9 +11,9 @@
 namespace dmx {
 
 // ---- inputs of one evaluation -----------------------------------------------------------------
-template <class R> struct InPlain {
+template <class R, int ST> struct InPlain {
   typedef R S;
-  Arr<R> qa, va, aa; const R* ua; const R* pa;
+  Arr<R, ST> qa, va, aa; const R* ua; const R* pa;
   DMX_DI R q(int i) const { return qa[i]; }
   DMX_DI R v(int i) const { return va[i]; }
   DMX_DI R a(int i) const { return aa[i]; }
@@ -22,9 +22,9 @@ template <class R> struct InPlain {
 };
 // the same inputs carrying one tangent direction (kind 0: configuration, 1: velocity, 2: control,
 // 3: parameter); the acceleration argument (x*) is held fixed
-template <class R> struct InDual {
+template <class R, int ST> struct InDual {
   typedef Dual<R> S;
-  Arr<R> qa, va, aa; const R* ua; const R* pa;
+  Arr<R, ST> qa, va, aa; const R* ua; const R* pa;
   int kind, idx; R dq0, dq1, dq2, dq3;
   DMX_DI S q(int i) const {
     R t = R(0);
@@ -48,12 +48,13 @@ template <class S> DMX_DI V3<S> point_acc(const FrameT<S>& f, const V3<S>& x) {
 // ---- S1: forward kinematics with first and second time derivatives ---------------
 // One body: frame from the parent's frame and the body's joint.  ACC: joint accelerations in.a
 // enter (inverse dynamics at a given acceleration); otherwise they are zero (bias force).
-template <class S, class R, class IN, bool ACC>
-DMX_DI void body_kin(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, int b) {
+template <class WS, class R, class IN, bool ACC>
+DMX_DI void body_kin(const ModelDev<R>& m, const IN& in, const WS& ws, int b) {
+  typedef typename WS::S S;
   int par = m.body_parent[b];
   FrameT<S> P;
-  P.p = ld3(ws.fp, par); P.R = ld9(ws.fR, par); P.w = ld3(ws.fw, par); P.al = ld3(ws.fal, par);
-  P.vp = ld3(ws.fvp, par); P.ap = ld3(ws.fap, par);
+  P.p = ld3(ws.fp(), par); P.R = ld9(ws.fR(), par); P.w = ld3(ws.fw(), par); P.al = ld3(ws.fal(), par);
+  P.vp = ld3(ws.fvp(), par); P.ap = ld3(ws.fap(), par);
   FrameT<S> f;
   f.p = P.p + P.R * c3<S>(m.body_pos, b);
   f.R = P.R * c9<S>(m.body_rot, b);
@@ -78,7 +79,7 @@ DMX_DI void body_kin(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, int b)
       g.vp = vo + cross(g.w, d);
       g.ap = ao + cross(g.al, d) + cross(g.w, cross(g.w, d));
       f = g;
-      st3(ws.dax, va, ax); st3(ws.dan, va, o);
+      st3(ws.dax(), va, ax); st3(ws.dan(), va, o);
     } else if (jt == JNT_SLIDE) {
       V3<S> ax = f.R * c3<S>(m.jnt_axis, j);
       V3<S> s = ax * in.q(qa);
@@ -88,7 +89,7 @@ DMX_DI void body_kin(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, int b)
       V3<S> nap = f.ap + cross(f.al, s) + cross(f.w, cross(f.w, s)) + cross(f.w, ax) * (S(2.0) * vj);
       if (ACC) nap = nap + ax * in.a(va);
       f.p = np; f.vp = nvp; f.ap = nap;
-      st3(ws.dax, va, ax); st3(ws.dan, va, np);
+      st3(ws.dax(), va, ax); st3(ws.dan(), va, np);
     } else {  // free joint: world linear velocity, body angular velocity
       f.p = mk3<S>(in.q(qa), in.q(qa + 1), in.q(qa + 2));
       f.R = quat_to_mat<S>(in.q(qa + 3), in.q(qa + 4), in.q(qa + 5), in.q(qa + 6));
@@ -100,47 +101,50 @@ DMX_DI void body_kin(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, int b)
         f.al = f.R * mk3<S>(in.a(va + 3), in.a(va + 4), in.a(va + 5));
       } else { f.ap = mk3<S>(z, z, z); f.al = f.ap; }
       S one(1.0);
-      st3(ws.dax, va, mk3<S>(one, z, z)); st3(ws.dax, va + 1, mk3<S>(z, one, z)); st3(ws.dax, va + 2, mk3<S>(z, z, one));
+      st3(ws.dax(), va, mk3<S>(one, z, z)); st3(ws.dax(), va + 1, mk3<S>(z, one, z)); st3(ws.dax(), va + 2, mk3<S>(z, z, one));
 #pragma unroll
-      for (int c = 0; c < 3; ++c) { st3(ws.dan, va + c, f.p); st3(ws.dax, va + 3 + c, colv(f.R, c)); st3(ws.dan, va + 3 + c, f.p); }
+      for (int c = 0; c < 3; ++c) { st3(ws.dan(), va + c, f.p); st3(ws.dax(), va + 3 + c, colv(f.R, c)); st3(ws.dan(), va + 3 + c, f.p); }
     }
   }
-  st3(ws.fp, b, f.p); st9(ws.fR, b, f.R); st3(ws.fw, b, f.w); st3(ws.fal, b, f.al); st3(ws.fvp, b, f.vp); st3(ws.fap, b, f.ap);
-  st3(ws.com, b, f.p + f.R * c3<S>(m.body_ipos, b));
+  st3(ws.fp(), b, f.p); st9(ws.fR(), b, f.R); st3(ws.fw(), b, f.w); st3(ws.fal(), b, f.al); st3(ws.fvp(), b, f.vp); st3(ws.fap(), b, f.ap);
+  st3(ws.com(), b, f.p + f.R * c3<S>(m.body_ipos, b));
 }
 
 // Bodies of one tree level are independent: one lane per body, levels in order.
-template <class S, class R, int G, class IN, bool ACC>
-DMX_D void kinematics(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, const Grp<G>& gr) {
+template <class WS, class R, int G, class IN, bool ACC>
+DMX_DN void kinematics(const ModelDev<R>& m, const IN& in, const WS& ws, const Grp<G>& gr) {
+  typedef typename WS::S S;
   if (gr.lane == 0) {
     S z(0.0), o(1.0);
     V3<S> z3 = mk3<S>(z, z, z);
-    st3(ws.fp, 0, z3); st3(ws.fw, 0, z3); st3(ws.fal, 0, z3); st3(ws.fvp, 0, z3); st3(ws.fap, 0, z3); st3(ws.com, 0, z3);
+    st3(ws.fp(), 0, z3); st3(ws.fw(), 0, z3); st3(ws.fal(), 0, z3); st3(ws.fvp(), 0, z3); st3(ws.fap(), 0, z3); st3(ws.com(), 0, z3);
     M3<S> I; for (int k = 0; k < 9; ++k) I.m[k] = (k % 4 == 0) ? o : z;
-    st9(ws.fR, 0, I);
+    st9(ws.fR(), 0, I);
   }
   gr.sync();
   for (int lv = 0; lv < m.nlevel; ++lv) {
-    for (int i = m.level_ptr[lv] + gr.lane; i < m.level_ptr[lv + 1]; i += G) body_kin<S, R, IN, ACC>(m, in, ws, m.level_body[i]);
+    for (int i = m.level_ptr[lv] + gr.lane; i < m.level_ptr[lv + 1]; i += G) body_kin<WS, R, IN, ACC>(m, in, ws, m.level_body[i]);
     gr.sync();
   }
 }
 
 // linear velocity of the world point x fixed to a body per unit rate of dof j (j on the body's
 // path to the world)
-template <class S> DMX_DI V3<S> twist_lin(const Ws<S>& ws, int j, int rot, const V3<S>& x) {
-  V3<S> ax = ld3(ws.dax, j);
+template <class WS> DMX_DI V3<typename WS::S> twist_lin(const WS& ws, int j, int rot, const V3<typename WS::S>& x) {
+  typedef typename WS::S S;
+  V3<S> ax = ld3(ws.dax(), j);
   if (!rot) return ax;
-  return cross(ax, x - ld3(ws.dan, j));
+  return cross(ax, x - ld3(ws.dan(), j));
 }
 
 // Newton-Euler wrench of body b about its centre of mass and its world inertia
-template <class S, class R, class IN>
-DMX_DI void body_wrench(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, int b, V3<S>& Fb, V3<S>& Nb, M3<S>& Iw) {
+template <class WS, class R, class IN>
+DMX_DI void body_wrench(const ModelDev<R>& m, const IN& in, const WS& ws, int b, V3<typename WS::S>& Fb, V3<typename WS::S>& Nb, M3<typename WS::S>& Iw) {
+  typedef typename WS::S S;
   FrameT<S> f;
-  f.p = ld3(ws.fp, b); f.R = ld9(ws.fR, b); f.w = ld3(ws.fw, b); f.al = ld3(ws.fal, b); f.ap = ld3(ws.fap, b);
+  f.p = ld3(ws.fp(), b); f.R = ld9(ws.fR(), b); f.w = ld3(ws.fw(), b); f.al = ld3(ws.fal(), b); f.ap = ld3(ws.fap(), b);
   S mass = in.p(b);
-  V3<S> ac = point_acc(f, ld3(ws.com, b));
+  V3<S> ac = point_acc(f, ld3(ws.com(), b));
   Fb = (ac - mk3<S>(S(m.gravity[0]), S(m.gravity[1]), S(m.gravity[2]))) * mass;
   M3<S> Ri = f.R * c9<S>(m.body_irot, b);
   M3<S> Dg;
@@ -159,24 +163,25 @@ DMX_DI void body_wrench(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, int
 // M = sum_b m Jc^T Jc + Jw^T I Jw + diag(armature): the linear part is summed over the subtree
 // below the deeper dof from a (body, ancestor-dof) twist table; the angular part uses the summed
 // world inertias of that subtree.  c_j = sum_b lin_jb . F_b + ang_j . N_b (virtual work).
-template <class S, class R, int G, class IN>
-DMX_D void dynamics(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, const Grp<G>& gr) {
+template <class WS, class R, int G, class IN>
+DMX_DN void dynamics(const ModelDev<R>& m, const IN& in, const WS& ws, const Grp<G>& gr) {
+  typedef typename WS::S S;
   const int nv = m.nv, nb = m.nbody;
   for (int b = 1 + gr.lane; b < nb; b += G) {
     V3<S> Fb, Nb; M3<S> Iw;
-    body_wrench<S, R, IN>(m, in, ws, b, Fb, Nb, Iw);
-    st3(ws.Fb, b, Fb); st3(ws.Nb, b, Nb); st9(ws.Iw, b, Iw);
+    body_wrench<WS, R, IN>(m, in, ws, b, Fb, Nb, Iw);
+    st3(ws.Fb(), b, Fb); st3(ws.Nb(), b, Nb); st9(ws.Iw(), b, Iw);
   }
   for (int e = gr.lane; e < m.ntw; e += G) {
     int j = m.tw_dof[e];
-    st3(ws.tw, e, twist_lin(ws, j, m.dof_rot[j], ld3(ws.com, m.tw_body[e])));
+    st3(ws.tw(), e, twist_lin(ws, j, m.dof_rot[j], ld3(ws.com(), m.tw_body[e])));
   }
   gr.sync();
   for (int i = gr.lane; i < 9 * (nb - 1); i += G) {
     int b = 1 + i / 9, k = i % 9;
     S acc(0.0);
-    for (int t = m.sub_ptr[b]; t < m.sub_ptr[b + 1]; ++t) acc = acc + ws.Iw[9 * m.sub_body[t] + k];
-    ws.Isub[9 * b + k] = acc;
+    for (int t = m.sub_ptr[b]; t < m.sub_ptr[b + 1]; ++t) acc = acc + ws.Iw()[9 * m.sub_body[t] + k];
+    ws.Isub()[9 * b + k] = acc;
   }
   gr.sync();
   for (int e = gr.lane; e < m.nmp; e += G) {
@@ -185,23 +190,23 @@ DMX_D void dynamics(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, const G
     if (deep >= 0) {
       for (int t = m.sub_ptr[deep]; t < m.sub_ptr[deep + 1]; ++t) {
         int b = m.sub_body[t];
-        acc = acc + in.p(b) * dot(ld3(ws.tw, m.tw_idx[b * nv + i]), ld3(ws.tw, m.tw_idx[b * nv + j]));
+        acc = acc + in.p(b) * dot(ld3(ws.tw(), m.tw_idx[b * nv + i]), ld3(ws.tw(), m.tw_idx[b * nv + j]));
       }
-      if (m.dof_rot[i] && m.dof_rot[j]) acc = acc + dot(ld3(ws.dax, i), ld9(ws.Isub, deep) * ld3(ws.dax, j));
+      if (m.dof_rot[i] && m.dof_rot[j]) acc = acc + dot(ld3(ws.dax(), i), ld9(ws.Isub(), deep) * ld3(ws.dax(), j));
       if (i == j) acc = acc + S(m.jnt_armature[m.dof_jnt[i]]);
     }
-    ws.M[i * nv + j] = acc; ws.M[j * nv + i] = acc;
+    ws.M()[i * nv + j] = acc; ws.M()[j * nv + i] = acc;
   }
   for (int j = gr.lane; j < nv; j += G) {
     int bj = m.dof_body[j], rot = m.dof_rot[j];
-    V3<S> ax = ld3(ws.dax, j);
+    V3<S> ax = ld3(ws.dax(), j);
     S acc(0.0);
     for (int t = m.sub_ptr[bj]; t < m.sub_ptr[bj + 1]; ++t) {
       int b = m.sub_body[t];
-      acc = acc + dot(ld3(ws.tw, m.tw_idx[b * nv + j]), ld3(ws.Fb, b));
-      if (rot) acc = acc + dot(ax, ld3(ws.Nb, b));
+      acc = acc + dot(ld3(ws.tw(), m.tw_idx[b * nv + j]), ld3(ws.Fb(), b));
+      if (rot) acc = acc + dot(ax, ld3(ws.Nb(), b));
     }
-    ws.c[j] = acc;
+    ws.c()[j] = acc;
     S tau = -(S(m.jnt_damping[m.dof_jnt[j]]) * in.v(j));
     for (int i = 0; i < m.nu; ++i) {
       int jn = m.act_jnt[i];
@@ -209,13 +214,21 @@ DMX_D void dynamics(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, const G
       if (m.act_type[i] == ACT_MOTOR) tau = tau + S(m.act_gear[i]) * in.u(i);
       else tau = tau + S(m.act_kp[i]) * (in.u(i) - in.q(m.jnt_qadr[jn])) - S(m.act_kd[i]) * in.v(j);
     }
-    ws.tau[j] = tau;
+    ws.tau()[j] = tau;
   }
   gr.sync();
 }
 
+// (a, b), b <= a, of the e-th entry of a row-major lower triangle
+DMX_DI void tri_index(int e, int& a, int& b) {
+  a = (int)((sqrtf(8.0f * (float)e + 1.0f) - 1.0f) * 0.5f);
+  if ((a + 1) * (a + 2) / 2 <= e) ++a;
+  if (a * (a + 1) / 2 > e) --a;
+  b = e - a * (a + 1) / 2;
+}
+
 // ---- dense Cholesky on the lower triangle, one column at a time, lanes over rows ---------------
-template <class S, int G> DMX_D bool cholesky(const Arr<S>& A, int n, const Grp<G>& gr) {
+template <class S, int ST, int G> DMX_DN bool cholesky(const Arr<S, ST>& A, int n, const Grp<G>& gr) {
   for (int j = 0; j < n; ++j) {
     for (int i = j + gr.lane; i < n; i += G) {
       S t = A[i * n + j];
@@ -233,7 +246,7 @@ template <class S, int G> DMX_D bool cholesky(const Arr<S>& A, int n, const Grp<
   return true;
 }
 // b <- (L L^T)^-1 b; column-oriented substitutions
-template <class S, int G> DMX_D void chol_solve(const Arr<S>& L, int n, const Arr<S>& b, const Grp<G>& gr) {
+template <class S, int ST, int G> DMX_DN void chol_solve(const Arr<S, ST>& L, int n, const Arr<S, ST>& b, const Grp<G>& gr) {
   for (int i = 0; i < n; ++i) {
     S bi = b[i] / L[i * n + i];
     for (int k = i + 1 + gr.lane; k < n; k += G) b[k] = b[k] - L[k * n + i] * bi;
@@ -281,10 +294,11 @@ template <class S, class R> DMX_DI S softplus(const S& z, R beta) {
 
 // ---- S4: narrow phase of one flattened candidate ----------
 template <class S> struct GeoT { S r; V3<S> n, pos, t1, t2; };
-template <class S, class R> DMX_DI GeoT<S> collide(const ModelDev<R>& m, const Ws<S>& ws, int c) {
+template <class WS, class R> DMX_DI GeoT<typename WS::S> collide(const ModelDev<R>& m, const WS& ws, int c) {
+  typedef typename WS::S S;
   GeoT<S> g;
   int b2 = m.ct_b2[c];
-  V3<S> c2 = ld3(ws.fp, b2) + ld9(ws.fR, b2) * c3<S>(m.ct_p2, c);
+  V3<S> c2 = ld3(ws.fp(), b2) + ld9(ws.fR(), b2) * c3<S>(m.ct_p2, c);
   S rho2(m.ct_rho2[c]);
   if (m.ct_kind[c] == CK_POINT_PLANE) {
     g.n = c3<S>(m.ct_n, c); g.t1 = c3<S>(m.ct_t1, c); g.t2 = c3<S>(m.ct_t2, c);
@@ -292,7 +306,7 @@ template <class S, class R> DMX_DI GeoT<S> collide(const ModelDev<R>& m, const W
     g.pos = c2 - g.n * (rho2 + S(0.5) * g.r);
   } else {
     int b1 = m.ct_b1[c];
-    V3<S> c1 = ld3(ws.fp, b1) + ld9(ws.fR, b1) * c3<S>(m.ct_p1, c);
+    V3<S> c1 = ld3(ws.fp(), b1) + ld9(ws.fR(), b1) * c3<S>(m.ct_p1, c);
     V3<S> dl = c2 - c1;
     S dist = m_sqrt(dot(dl, dl)), rho1(m.ct_rho1[c]);
     g.n = dl * (S(1.0) / dist);
@@ -334,8 +348,9 @@ DMX_DI void candidate_terms(const ModelDev<R>& m, const IN& in, int c, const S& 
 }
 
 // relative velocity of the contact point per unit rate of dof j, body2 minus body1
-template <class S, class R>
-DMX_DI V3<S> rel_twist(const ModelDev<R>& m, const Ws<S>& ws, int j, int b1, int b2, const V3<S>& pos) {
+template <class WS, class R>
+DMX_DI V3<typename WS::S> rel_twist(const ModelDev<R>& m, const WS& ws, int j, int b1, int b2, const V3<typename WS::S>& pos) {
+  typedef typename WS::S S;
   S z(0.0);
   V3<S> d = mk3<S>(z, z, z);
   int rot = m.dof_rot[j];
@@ -345,25 +360,26 @@ DMX_DI V3<S> rel_twist(const ModelDev<R>& m, const Ws<S>& ws, int j, int b1, int
 }
 
 // ---- S4+S5: rows of every candidate with r<0 (cfd: r<w_c), compacted in candidate order ----------
-template <class S, class R, int G, class IN>
-DMX_D int build_rows(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, bool cfd, const Grp<G>& gr) {
+template <class WS, class R, int G, class IN>
+DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, const Grp<G>& gr) {
+  typedef typename WS::S S;
   const int nv = m.nv, nc = m.nc;
   for (int c = gr.lane; c < nc; c += G) {
-    GeoT<S> g = collide<S, R>(m, ws, c);
-    ws.cr[c] = g.r; st3(ws.cn, c, g.n); st3(ws.cpos, c, g.pos); st3(ws.ct1, c, g.t1); st3(ws.ct2, c, g.t2);
+    GeoT<S> g = collide<WS, R>(m, ws, c);
+    ws.cr()[c] = g.r; st3(ws.cn(), c, g.n); st3(ws.cpos(), c, g.pos); st3(ws.ct1(), c, g.t1); st3(ws.ct2(), c, g.t2);
     bool inc = (val(g.r) < 0) || (cfd && val(g.r) < m.pair_solimp_cfd[5 * m.ct_pair[c] + 2]);
-    ws.incl[c] = inc ? (m.ct_condim[c] == 3 ? 4 : 1) : 0;
+    ws.incl()[c] = inc ? (m.ct_condim[c] == 3 ? 4 : 1) : 0;
     if (inc) {
       S Dw, post, bd, mu;
       candidate_terms<S, R, IN>(m, in, c, g.r, cfd, Dw, post, bd, mu);
-      ws.cD[c] = Dw; ws.cpost[c] = post; ws.cbd[c] = bd; ws.cmu[c] = mu;
+      ws.cD()[c] = Dw; ws.cpost()[c] = post; ws.cbd()[c] = bd; ws.cmu()[c] = mu;
     }
   }
   gr.sync();
   int nr = 0;
   for (int c = 0; c < nc; ++c) {
-    int n = ws.incl[c];
-    if (gr.lane == 0) { ws.rowstart[c] = nr; for (int e = 0; e < n; ++e) ws.rowcand[nr + e] = 4 * c + e; }
+    int n = ws.incl()[c];
+    if (gr.lane == 0) { ws.rowstart()[c] = nr; for (int e = 0; e < n; ++e) ws.rowcand()[nr + e] = 4 * c + e; }
     nr += n;
   }
   gr.sync();
@@ -371,26 +387,26 @@ DMX_D int build_rows(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, bool c
   // Jacobian entries: one (candidate, dof) item yields that candidate's 1 or 4 row entries
   for (int it = gr.lane; it < nc * nv; it += G) {
     int c = it / nv, j = it - c * nv;
-    int n = ws.incl[c];
+    int n = ws.incl()[c];
     if (n == 0) continue;
-    int r0 = ws.rowstart[c];
-    V3<S> d = rel_twist<S, R>(m, ws, j, m.ct_b1[c], m.ct_b2[c], ld3(ws.cpos, c));
-    S nd = dot(ld3(ws.cn, c), d);
-    if (n == 1) ws.J[r0 * nv + j] = nd;
+    int r0 = ws.rowstart()[c];
+    V3<S> d = rel_twist<WS, R>(m, ws, j, m.ct_b1[c], m.ct_b2[c], ld3(ws.cpos(), c));
+    S nd = dot(ld3(ws.cn(), c), d);
+    if (n == 1) ws.J()[r0 * nv + j] = nd;
     else {
-      S mu = ws.cmu[c];
-      S t1d = mu * dot(ld3(ws.ct1, c), d), t2d = mu * dot(ld3(ws.ct2, c), d);
-      ws.J[r0 * nv + j] = nd + t1d; ws.J[(r0 + 1) * nv + j] = nd - t1d;
-      ws.J[(r0 + 2) * nv + j] = nd + t2d; ws.J[(r0 + 3) * nv + j] = nd - t2d;
+      S mu = ws.cmu()[c];
+      S t1d = mu * dot(ld3(ws.ct1(), c), d), t2d = mu * dot(ld3(ws.ct2(), c), d);
+      ws.J()[r0 * nv + j] = nd + t1d; ws.J()[(r0 + 1) * nv + j] = nd - t1d;
+      ws.J()[(r0 + 2) * nv + j] = nd + t2d; ws.J()[(r0 + 3) * nv + j] = nd - t2d;
     }
   }
   gr.sync();
   for (int i = gr.lane; i < nr; i += G) {
-    int c = ws.rowcand[i] >> 2;
+    int c = ws.rowcand()[i] >> 2;
     S Jv(0.0);
-    for (int j = 0; j < nv; ++j) Jv = Jv + ws.J[i * nv + j] * in.v(j);
-    ws.aref[i] = ws.cpost[c] - ws.cbd[c] * Jv;
-    ws.D[i] = ws.cD[c];
+    for (int j = 0; j < nv; ++j) Jv = Jv + ws.J()[i * nv + j] * in.v(j);
+    ws.aref()[i] = ws.cpost()[c] - ws.cbd()[c] * Jv;
+    ws.D()[i] = ws.cD()[c];
   }
   gr.sync();
   return nr;
@@ -400,42 +416,42 @@ DMX_D int build_rows(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, bool c
 //   Phi(x) = 1/2 (x-a0)^T M (x-a0) + 1/2 sum_i D_i min(0, J_i x - aref_i)^2
 // (iterations / ls_iterations PAPER.md:515, 539).
 // Returns true when the last step was a full step inside an unchanged active set.
-template <class S, int G>
-DMX_D bool newton(int nv, int nr, int n_it, int n_ls, const Ws<S>& ws, const Grp<G>& gr) {
-  for (int j = gr.lane; j < nv; j += G) ws.x[j] = ws.a0[j];
+template <class WS, int G>
+DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G>& gr) {
+  typedef typename WS::S S;
+  for (int j = gr.lane; j < nv; j += G) ws.x()[j] = ws.a0()[j];
   gr.sync();
   if (nr == 0) return true;
   bool conv = false;
   for (int it = 0; it < n_it; ++it) {
     for (int i = gr.lane; i < nr; i += G) {
       S t(0.0);
-      for (int j = 0; j < nv; ++j) t = t + ws.J[i * nv + j] * ws.x[j];
-      ws.s[i] = t - ws.aref[i];
+      for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.x()[j];
+      ws.s()[i] = t - ws.aref()[i];
     }
-    for (int j = gr.lane; j < nv; j += G) ws.xa[j] = ws.x[j] - ws.a0[j];
+    for (int j = gr.lane; j < nv; j += G) ws.xa()[j] = ws.x()[j] - ws.a0()[j];
     gr.sync();
     for (int a = gr.lane; a < nv; a += G) {
       S t(0.0);
-      for (int b = 0; b < nv; ++b) t = t + ws.M[a * nv + b] * ws.xa[b];
-      for (int i = 0; i < nr; ++i) if (val(ws.s[i]) < 0) t = t + ws.J[i * nv + a] * ws.D[i] * ws.s[i];
-      ws.g[a] = t; ws.dl[a] = -t;
+      for (int b = 0; b < nv; ++b) t = t + ws.M()[a * nv + b] * ws.xa()[b];
+      for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.J()[i * nv + a] * ws.D()[i] * ws.s()[i];
+      ws.g()[a] = t; ws.dl()[a] = -t;
     }
     for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
-      int a = 0; while ((a + 1) * (a + 2) / 2 <= e) ++a;
-      int b = e - a * (a + 1) / 2;
-      S t = ws.M[a * nv + b];
-      for (int i = 0; i < nr; ++i) if (val(ws.s[i]) < 0) t = t + ws.D[i] * ws.J[i * nv + a] * ws.J[i * nv + b];
-      ws.Hc[a * nv + b] = t;
+      int a, b; tri_index(e, a, b);
+      S t = ws.M()[a * nv + b];
+      for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.D()[i] * ws.J()[i * nv + a] * ws.J()[i * nv + b];
+      ws.Hc()[a * nv + b] = t;
     }
     gr.sync();
-    if (!cholesky<S, G>(ws.Hc, nv, gr)) break;
-    chol_solve<S, G>(ws.Hc, nv, ws.dl, gr);
+    if (!cholesky(ws.Hc(), nv, gr)) break;
+    chol_solve(ws.Hc(), nv, ws.dl(), gr);
     bool same = true;
     for (int i = gr.lane; i < nr; i += G) {
       S t(0.0);
-      for (int j = 0; j < nv; ++j) t = t + ws.J[i * nv + j] * ws.dl[j];
-      ws.pr[i] = t;
-      if ((val(ws.s[i]) < 0) != (val(ws.s[i] + t) < 0)) same = false;
+      for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.dl()[j];
+      ws.pr()[i] = t;
+      if ((val(ws.s()[i]) < 0) != (val(ws.s()[i] + t) < 0)) same = false;
     }
     same = gr.all(same);
     gr.sync();
@@ -445,16 +461,16 @@ DMX_D bool newton(int nv, int nr, int n_it, int n_ls, const Ws<S>& ws, const Grp
       // scalar line search redundantly in row order (same summation order as a serial code)
       for (int a = gr.lane; a < nv; a += G) {
         S t(0.0);
-        for (int b = 0; b < nv; ++b) t = t + ws.M[a * nv + b] * ws.dl[b];
-        ws.Md[a] = t;
+        for (int b = 0; b < nv; ++b) t = t + ws.M()[a * nv + b] * ws.dl()[b];
+        ws.Md()[a] = t;
       }
       gr.sync();
       S dMd(0.0), dMxa(0.0);
-      for (int a = 0; a < nv; ++a) { dMd = dMd + ws.dl[a] * ws.Md[a]; dMxa = dMxa + ws.Md[a] * ws.xa[a]; }
+      for (int a = 0; a < nv; ++a) { dMd = dMd + ws.dl()[a] * ws.Md()[a]; dMxa = dMxa + ws.Md()[a] * ws.xa()[a]; }
       S lo(0.0), hi(0.0), a(0.0), d2, d1a; bool hi_inf = true, frozen = false;
       {
         d1a = dMxa; d2 = dMd;
-        for (int i = 0; i < nr; ++i) { S si = ws.s[i]; if (val(si) < 0) { d1a = d1a + ws.D[i] * ws.pr[i] * si; d2 = d2 + ws.D[i] * ws.pr[i] * ws.pr[i]; } }
+        for (int i = 0; i < nr; ++i) { S si = ws.s()[i]; if (val(si) < 0) { d1a = d1a + ws.D()[i] * ws.pr()[i] * si; d2 = d2 + ws.D()[i] * ws.pr()[i] * ws.pr()[i]; } }
       }
       for (int ls = 0; ls < n_ls && !frozen; ++ls) {
         S an = (ls == 0) ? S(1.0) : a - d1a / d2;
@@ -464,63 +480,63 @@ DMX_D bool newton(int nv, int nr, int n_it, int n_ls, const Ws<S>& ws, const Grp
         a = an;
         d1a = dMxa + a * dMd; d2 = dMd;
         for (int i = 0; i < nr; ++i) {
-          S si = ws.s[i] + a * ws.pr[i];
-          if (val(si) < 0) { d1a = d1a + ws.D[i] * ws.pr[i] * si; d2 = d2 + ws.D[i] * ws.pr[i] * ws.pr[i]; }
+          S si = ws.s()[i] + a * ws.pr()[i];
+          if (val(si) < 0) { d1a = d1a + ws.D()[i] * ws.pr()[i] * si; d2 = d2 + ws.D()[i] * ws.pr()[i] * ws.pr()[i]; }
         }
         if (val(d1a) < 0) lo = a; else if (val(d1a) > 0) { hi = a; hi_inf = false; } else frozen = true;
       }
       alpha = a;
     }
-    for (int j = gr.lane; j < nv; j += G) ws.x[j] = ws.x[j] + alpha * ws.dl[j];
+    for (int j = gr.lane; j < nv; j += G) ws.x()[j] = ws.x()[j] + alpha * ws.dl()[j];
     gr.sync();
     if (same) { conv = true; break; }
   }
   return conv;
 }
 
-// ---- F (cfd=false) or F~ (cfd=true) at one state: result in ws.x, rows and M left in ws ----------
+// ---- F (cfd=false) or F~ (cfd=true) at one state: result in ws.x(), rows and M left in ws ----------
 // returns nr >= 0, or -1 when M is not positive definite / the result is not finite
-template <class S, class R, int G, class IN>
-DMX_D int vector_field(const ModelDev<R>& m, const IN& in, const Ws<S>& ws, bool cfd, bool& conv, const Grp<G>& gr) {
+template <class WS, class R, int G, class IN>
+DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, bool& conv, const Grp<G>& gr) {
   const int nv = m.nv;
-  kinematics<S, R, G, IN, false>(m, in, ws, gr);
-  dynamics<S, R, G, IN>(m, in, ws, gr);
-  for (int e = gr.lane; e < nv * nv; e += G) ws.Hc[e] = ws.M[e];
-  for (int j = gr.lane; j < nv; j += G) ws.a0[j] = ws.tau[j] - ws.c[j];
+  kinematics<WS, R, G, IN, false>(m, in, ws, gr);
+  dynamics<WS, R, G, IN>(m, in, ws, gr);
+  for (int e = gr.lane; e < nv * nv; e += G) ws.Hc()[e] = ws.M()[e];
+  for (int j = gr.lane; j < nv; j += G) ws.a0()[j] = ws.tau()[j] - ws.c()[j];
   gr.sync();
   conv = true;
-  if (!cholesky<S, G>(ws.Hc, nv, gr)) return -1;
-  chol_solve<S, G>(ws.Hc, nv, ws.a0, gr);
-  int nr = build_rows<S, R, G, IN>(m, in, ws, cfd, gr);
-  conv = newton<S, G>(nv, nr, m.newton_iters, m.ls_iters, ws, gr);
+  if (!cholesky(ws.Hc(), nv, gr)) return -1;
+  chol_solve(ws.Hc(), nv, ws.a0(), gr);
+  int nr = build_rows<WS, R, G, IN>(m, in, ws, cfd, gr);
+  conv = newton<WS, G>(nv, nr, m.newton_iters, m.ls_iters, ws, gr);
   bool fin = true;
-  for (int j = gr.lane; j < nv; j += G) if (!isfinite(val(ws.x[j]))) fin = false;
+  for (int j = gr.lane; j < nv; j += G) if (!isfinite(val(ws.x()[j]))) fin = false;
   if (!gr.all(fin)) return -1;
   return nr;
 }
 
 // ---- S11/S12, cooperative part: final active set A, H = M + J_A^T D_A J_A, w = H^-1 kappa ---------
-// ws.kap holds kappa on entry and w on exit.  Returns false if H is not positive definite.
-template <class S, int G>
-DMX_D bool vjp_prepare(int nv, int nr, const Ws<S>& ws, const Grp<G>& gr) {
+// ws.kap() holds kappa on entry and w on exit.  Returns false if H is not positive definite.
+template <class WS, int G>
+DMX_DN bool vjp_prepare(int nv, int nr, const WS& ws, const Grp<G>& gr) {
+  typedef typename WS::S S;
   for (int i = gr.lane; i < nr; i += G) {
     S t(0.0);
-    for (int j = 0; j < nv; ++j) t = t + ws.J[i * nv + j] * ws.x[j];
-    t = t - ws.aref[i];
-    ws.s[i] = t;
-    ws.active[i] = val(t) < 0 ? 1 : 0;
+    for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.x()[j];
+    t = t - ws.aref()[i];
+    ws.s()[i] = t;
+    ws.active()[i] = val(t) < 0 ? 1 : 0;
   }
   gr.sync();
   for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
-    int a = 0; while ((a + 1) * (a + 2) / 2 <= e) ++a;
-    int b = e - a * (a + 1) / 2;
-    S t = ws.M[a * nv + b];
-    for (int i = 0; i < nr; ++i) if (ws.active[i]) t = t + ws.D[i] * ws.J[i * nv + a] * ws.J[i * nv + b];
-    ws.Hc[a * nv + b] = t;
+    int a, b; tri_index(e, a, b);
+    S t = ws.M()[a * nv + b];
+    for (int i = 0; i < nr; ++i) if (ws.active()[i]) t = t + ws.D()[i] * ws.J()[i * nv + a] * ws.J()[i * nv + b];
+    ws.Hc()[a * nv + b] = t;
   }
   gr.sync();
-  if (!cholesky<S, G>(ws.Hc, nv, gr)) return false;
-  chol_solve<S, G>(ws.Hc, nv, ws.kap, gr);
+  if (!cholesky(ws.Hc(), nv, gr)) return false;
+  chol_solve(ws.Hc(), nv, ws.kap(), gr);
   return true;
 }
 
@@ -531,25 +547,25 @@ DMX_D bool vjp_prepare(int nv, int nr, const Ws<S>& ws, const Grp<G>& gr) {
 // cooperative pass.  Uses the virtual-work identity  w^T ID = sum_b vel_w(com_b).F_b + omega_w(b).N_b
 // and, for the rows,  J_i y = dir_i . relvel_y(pos_i)  with y in {x*, v, w}.
 // dws: this lane's tangent workspace (frames only).
-template <class R, class IN>
-DMX_D R residual_tangent(const ModelDev<R>& m, const IN& in, const Ws<Dual<R> >& dws, const Arr<R>& w,
-                         const Arr<int>& incl, const Arr<int>& rowstart, const Arr<int>& active, bool cfd) {
+template <class R, class IN, class DWS, int ST>
+DMX_DN R residual_tangent(const ModelDev<R>& m, const IN& in, const DWS& dws, const Arr<R, ST>& w,
+                          const Arr<int, ST>& incl, const Arr<int, ST>& rowstart, const Arr<int, ST>& active, bool cfd) {
   typedef Dual<R> S;
   const int nv = m.nv;
   Grp<1> g1; g1.lane = 0; g1.mask = 0;
-  kinematics<S, R, 1, IN, true>(m, in, dws, g1);
+  kinematics<DWS, R, 1, IN, true>(m, in, dws, g1);
   S acc(R(0));
   for (int b = 1; b < m.nbody; ++b) {
     V3<S> Fb, Nb; M3<S> Iw;
-    body_wrench<S, R, IN>(m, in, dws, b, Fb, Nb, Iw);
-    V3<S> comb = ld3(dws.com, b);
+    body_wrench<DWS, R, IN>(m, in, dws, b, Fb, Nb, Iw);
+    V3<S> comb = ld3(dws.com(), b);
     S z(R(0));
     V3<S> vw = mk3<S>(z, z, z), ow = vw;
     for (int e = m.tw_ptr[b]; e < m.tw_ptr[b + 1]; ++e) {
       int j = m.tw_dof[e], rot = m.dof_rot[j];
       S wj(w[j]);
       vw = vw + twist_lin(dws, j, rot, comb) * wj;
-      if (rot) ow = ow + ld3(dws.dax, j) * wj;
+      if (rot) ow = ow + ld3(dws.dax(), j) * wj;
     }
     acc = acc + dot(vw, Fb) + dot(ow, Nb);
   }
@@ -570,7 +586,7 @@ DMX_D R residual_tangent(const ModelDev<R>& m, const IN& in, const Ws<Dual<R> >&
     bool any = false;
     for (int e = 0; e < n; ++e) any = any || active[r0 + e];
     if (!any) continue;
-    GeoT<S> g = collide<S, R>(m, dws, c);
+    GeoT<S> g = collide<DWS, R>(m, dws, c);
     S Dw, post, bd, mu;
     candidate_terms<S, R, IN>(m, in, c, g.r, cfd, Dw, post, bd, mu);
     S z(R(0));
@@ -578,7 +594,7 @@ DMX_D R residual_tangent(const ModelDev<R>& m, const IN& in, const Ws<Dual<R> >&
     int b1 = m.ct_b1[c], b2 = m.ct_b2[c];
     for (int j = 0; j < nv; ++j) {
       if (m.tw_idx[b2 * nv + j] < 0 && m.tw_idx[b1 * nv + j] < 0) continue;
-      V3<S> d = rel_twist<S, R>(m, dws, j, b1, b2, g.pos);
+      V3<S> d = rel_twist<DWS, R>(m, dws, j, b1, b2, g.pos);
       S nd = dot(g.n, d);
       S xj = in.a(j), vj = in.v(j), wj(w[j]);
       nX = nX + nd * xj; nV = nV + nd * vj; nW = nW + nd * wj;
@@ -604,8 +620,8 @@ DMX_D R residual_tangent(const ModelDev<R>& m, const IN& in, const Ws<Dual<R> >&
 }
 
 // tangent of q (+) eps e_d at eps = 0: fills the seed of an InDual
-template <class R>
-DMX_DI void seed_direction(const ModelDev<R>& m, InDual<R>& in, int d) {
+template <class R, int ST>
+DMX_DI void seed_direction(const ModelDev<R>& m, InDual<R, ST>& in, int d) {
   const int nv = m.nv;
   in.dq0 = R(1); in.dq1 = in.dq2 = in.dq3 = R(0);
   if (d < nv) {

@@ -9,25 +9,27 @@ namespace dmx {
 // ---- S11/S12: (qbar,vbar,ubar,pbar) = kappa^T dF/d(q,v,u,p), F~ when cfd (Eq. 4) ----------
 // Cooperative solve for x*, the active set and w = H^-1 kappa; then one tangent direction per lane.
 template <class R, int G>
-DMX_D bool vjp_stage(const ModelDev<R>& m, const Arr<R>& Yqr, const Arr<R>& Vr, const R* u, const R* p, const Arr<double>& kappa,
-                     bool cfd, bool want_p, const Ws<R>& ws, const Ws<Dual<R> >& dws, const Rk& rk, const Grp<G>& gr) {
+DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yqr, const Arr<R, StrideOf<G>::value>& Vr, const R* u, const R* p,
+                      const Arr<double, StrideOf<G>::value>& kappa, bool cfd, bool want_p, const Ws<R, StrideOf<G>::value>& ws,
+                      const Ws<Dual<R>, 32>& dws, const Rk<StrideOf<G>::value>& rk, const Grp<G>& gr) {
+  const int ST = StrideOf<G>::value;
   const int nv = m.nv;
-  InPlain<R> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
+  InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
   bool conv;
-  int nr = vector_field<R, R, G, InPlain<R> >(m, in, ws, cfd, conv, gr);
+  int nr = vector_field<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, cfd, conv, gr);
   if (nr < 0) return false;
-  for (int j = gr.lane; j < nv; j += G) ws.kap[j] = (R)kappa[j];
+  for (int j = gr.lane; j < nv; j += G) ws.kap()[j] = (R)kappa[j];
   gr.sync();
-  if (!vjp_prepare<R, G>(nv, nr, ws, gr)) return false;
+  if (!vjp_prepare<Ws<R, ST>, G>(nv, nr, ws, gr)) return false;
   const int ndir = 2 * nv + m.nu + (want_p ? m.np : 0);
   for (int d = gr.lane; d < ndir; d += G) {
-    InDual<R> din; din.qa = Yqr; din.va = Vr; din.aa = ws.x; din.ua = u; din.pa = p;
-    seed_direction<R>(m, din, d);
-    double s = -(double)residual_tangent<R, InDual<R> >(m, din, dws, ws.kap, ws.incl, ws.rowstart, ws.active, cfd);
-    if (d < nv) rk.qbar[d] = s;
-    else if (d < 2 * nv) rk.vbar[d - nv] = s;
-    else if (d < 2 * nv + m.nu) rk.ubar[d - 2 * nv] = s;
-    else rk.pbar[d - 2 * nv - m.nu] = s;
+    InDual<R, ST> din; din.qa = Yqr; din.va = Vr; din.aa = ws.x(); din.ua = u; din.pa = p;
+    seed_direction<R, ST>(m, din, d);
+    double s = -(double)residual_tangent<R, InDual<R, ST>, Ws<Dual<R>, 32>, ST>(m, din, dws, ws.kap(), ws.incl(), ws.rowstart(), ws.active(), cfd);
+    if (d < nv) rk.qbar()[d] = s;
+    else if (d < 2 * nv) rk.vbar()[d - nv] = s;
+    else if (d < 2 * nv + m.nu) rk.ubar()[d - 2 * nv] = s;
+    else rk.pbar()[d - 2 * nv - m.nu] = s;
   }
   gr.sync();
   return true;
@@ -46,21 +48,25 @@ template <class R> struct BackwardArgs {
 };
 
 template <class R>
-DMX_DI Ws<Dual<R> > bind_scratch(Dual<R>* scratch, int res_size, const WsLayout& rwl) {
-  Ws<Dual<R> > dws;
+DMX_DI Ws<Dual<R>, 32> bind_scratch(Dual<R>* scratch, int res_size, const WsLayout* rwl) {
+  Ws<Dual<R>, 32> dws;
   size_t gwarp = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  dws.bind(rwl, scratch + gwarp * (size_t)res_size * 32 + (threadIdx.x & 31), 32, nullptr, 0);
+  dws.b = scratch + gwarp * (size_t)res_size * 32 + (threadIdx.x & 31); dws.ib = nullptr; dws.L = rwl;
   return dws;
 }
 
 // ---- S10: reverse sweep over the tape, frozen step sizes ---------------------------
 template <class R, int G>
-__global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ ModelDev<R> m, const __grid_constant__ BackwardArgs<R> a) {
+__global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ BackwardArgs<R> a) {
   extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ CtaConst<R> cc;
+  load_cta_const<R>(cc, m_, a.wl, a.rwl, a.rl);
+  const ModelDev<R>& m = cc.m;
+  const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
-  Rk rk; Ws<R> ws; Arr<R> Yqr, Vr;
-  bind_shared<R, G>(smem, a.rl.size_bwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, a.rl, a.wl);
-  Ws<Dual<R> > dws = bind_scratch<R>(a.scratch, a.res_size, a.rwl);
+  Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
+  bind_shared<R, G>(smem, a.rl.size_bwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
+  Ws<Dual<R>, 32> dws = bind_scratch<R>(a.scratch, a.res_size, &cc.rwl);
   const int nq = m.nq, nv = m.nv, nu = m.nu, np = m.np, nx = nq + nv, tab = a.so.tableau, rec = nx + 2;
   const bool has_ctrl = a.ctrl != nullptr && a.nknot > 0 && nu > 0;
   const int nknot = has_ctrl ? a.nknot : 0;
@@ -86,15 +92,15 @@ __global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ M
           s = (-w1 * e0 - w2 * e1 - w3 * e2) * (double)gT[qa + 3] + (w0 * e0 + w2 * e2 - w3 * e1) * (double)gT[qa + 4] +
               (w0 * e1 - w1 * e2 + w3 * e0) * (double)gT[qa + 5] + (w0 * e2 + w1 * e1 - w2 * e0) * (double)gT[qa + 6];
         }
-        rk.lam[d] = s; rk.lam[nv + d] = (double)gT[nq + d];
+        rk.lam()[d] = s; rk.lam()[nv + d] = (double)gT[nq + d];
       }
-      for (int i = gr.lane; i < np; i += G) rk.gp[i] = 0.0;
+      for (int i = gr.lane; i < np; i += G) rk.gp()[i] = 0.0;
       gr.sync();
     }
     for (int n = N - 1; n >= 0 && good; --n) {
       const R* r = a.tape + ((size_t)e * a.tape_cap + n) * rec;
-      for (int j = gr.lane; j < nq; j += G) rk.q[j] = (double)r[j];
-      for (int j = gr.lane; j < nv; j += G) rk.v[j] = (double)r[nq + j];
+      for (int j = gr.lane; j < nq; j += G) rk.q()[j] = (double)r[j];
+      for (int j = gr.lane; j < nv; j += G) rk.v()[j] = (double)r[nq + j];
       double hs = (double)r[nx + 1], h = fabs(hs);
       if (hs < 0) knot--;
       const R* u = has_ctrl ? a.ctrl + ((size_t)e * nknot + knot) * nu : a.zero_u;
@@ -103,42 +109,42 @@ __global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ M
       rk_attempt<R, G, true>(m, tab, rk, Yqr, Vr, u, p, h, false, ws, ok, unc, gr);   // recompute the stages with F
       // y_{n+1} = (q_n (+) h sum b_i K_i, v_n + h sum b_i A_i), b = row 6 of a
       for (int j = gr.lane; j < nv; j += G) {
-        double s = 0; for (int i = 0; i < 6; ++i) s += TAB_A[tab][6][i] * rk.K[i * nv + j];
-        rk.delta[j] = h * s; rk.dbar[j] = 0; rk.qb[j] = 0; rk.vb[j] = rk.lam[nv + j];
+        double s = 0; for (int i = 0; i < 6; ++i) s += TAB_A[tab][6][i] * rk.K()[i * nv + j];
+        rk.delta()[j] = h * s; rk.dbar()[j] = 0; rk.qb()[j] = 0; rk.vb()[j] = rk.lam()[nv + j];
       }
       gr.sync();
-      for (int jn = gr.lane; jn < m.njnt; jn += G) retract_pullback_joint<R>(m, jn, rk.delta, rk.lam, rk.qb, rk.dbar);
+      for (int jn = gr.lane; jn < m.njnt; jn += G) retract_pullback_joint(m, jn, rk.delta(), rk.lam(), rk.qb(), rk.dbar());
       gr.sync();
       for (int j = gr.lane; j < nv; j += G)
-        for (int i = 0; i < 6; ++i) { rk.Kb[i * nv + j] = h * TAB_A[tab][6][i] * rk.dbar[j]; rk.Ab[i * nv + j] = h * TAB_A[tab][6][i] * rk.lam[nv + j]; }
+        for (int i = 0; i < 6; ++i) { rk.Kb()[i * nv + j] = h * TAB_A[tab][6][i] * rk.dbar()[j]; rk.Ab()[i * nv + j] = h * TAB_A[tab][6][i] * rk.lam()[nv + j]; }
       gr.sync();
       for (int i = 5; i >= 0 && good; --i) {
-        for (int j = gr.lane; j < nv; j += G) { rk.Vb[j] = 0; rk.dbar[j] = 0; }
+        for (int j = gr.lane; j < nv; j += G) { rk.Vb()[j] = 0; rk.dbar()[j] = 0; }
         gr.sync();
-        for (int jn = gr.lane; jn < m.njnt; jn += G) chart_pullback_joint<R>(m, jn, rk.sDl.at(i * nv), rk.sV.at(i * nv), rk.Kb.at(i * nv), rk.Vb, rk.dbar);
-        for (int j = gr.lane; j < nq; j += G) Yqr[j] = (R)rk.sYq[i * nq + j];
-        for (int j = gr.lane; j < nv; j += G) Vr[j] = (R)rk.sV[i * nv + j];
+        for (int jn = gr.lane; jn < m.njnt; jn += G) chart_pullback_joint(m, jn, rk.sDl().at(i * nv), rk.sV().at(i * nv), rk.Kb().at(i * nv), rk.Vb(), rk.dbar());
+        for (int j = gr.lane; j < nq; j += G) Yqr[j] = (R)rk.sYq()[i * nq + j];
+        for (int j = gr.lane; j < nv; j += G) Vr[j] = (R)rk.sV()[i * nv + j];
         gr.sync();
         // A_i = F(Y_i), or F~ for the straight-through estimator (Eq. 4)
-        if (!vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.Ab.at(i * nv), a.cfd != 0, a.want_p != 0, ws, dws, rk, gr)) { good = false; break; }
-        for (int j = gr.lane; j < nv; j += G) rk.Vb[j] += rk.vbar[j];
-        if (a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nu; c += G) a.dLdctrl[((size_t)e * nknot + knot) * nu + c] += (R)rk.ubar[c];
-        if (a.want_p) for (int c = gr.lane; c < np; c += G) rk.gp[c] += rk.pbar[c];
+        if (!vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.Ab().at(i * nv), a.cfd != 0, a.want_p != 0, ws, dws, rk, gr)) { good = false; break; }
+        for (int j = gr.lane; j < nv; j += G) rk.Vb()[j] += rk.vbar()[j];
+        if (a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nu; c += G) a.dLdctrl[((size_t)e * nknot + knot) * nu + c] += (R)rk.ubar()[c];
+        if (a.want_p) for (int c = gr.lane; c < np; c += G) rk.gp()[c] += rk.pbar()[c];
         gr.sync();
-        for (int jn = gr.lane; jn < m.njnt; jn += G) retract_pullback_joint<R>(m, jn, rk.sDl.at(i * nv), rk.qbar, rk.qb, rk.dbar);
+        for (int jn = gr.lane; jn < m.njnt; jn += G) retract_pullback_joint(m, jn, rk.sDl().at(i * nv), rk.qbar(), rk.qb(), rk.dbar());
         gr.sync();
         for (int j = gr.lane; j < nv; j += G) {
-          rk.vb[j] += rk.Vb[j];
-          for (int l = 0; l < i; ++l) { rk.Kb[l * nv + j] += h * TAB_A[tab][i][l] * rk.dbar[j]; rk.Ab[l * nv + j] += h * TAB_A[tab][i][l] * rk.Vb[j]; }
+          rk.vb()[j] += rk.Vb()[j];
+          for (int l = 0; l < i; ++l) { rk.Kb()[l * nv + j] += h * TAB_A[tab][i][l] * rk.dbar()[j]; rk.Ab()[l * nv + j] += h * TAB_A[tab][i][l] * rk.Vb()[j]; }
         }
         gr.sync();
       }
-      for (int j = gr.lane; j < nv; j += G) { rk.lam[j] = rk.qb[j]; rk.lam[nv + j] = rk.vb[j]; }
+      for (int j = gr.lane; j < nv; j += G) { rk.lam()[j] = rk.qb()[j]; rk.lam()[nv + j] = rk.vb()[j]; }
       gr.sync();
     }
     R* g0 = a.dLdx0 + (size_t)e * 2 * nv;
-    for (int j = gr.lane; j < 2 * nv; j += G) g0[j] = good ? (R)rk.lam[j] : R(0);
-    if (a.dLdparams) for (int c = gr.lane; c < np; c += G) a.dLdparams[(size_t)e * np + c] = good ? (R)rk.gp[c] : R(0);
+    for (int j = gr.lane; j < 2 * nv; j += G) g0[j] = good ? (R)rk.lam()[j] : R(0);
+    if (a.dLdparams) for (int c = gr.lane; c < np; c += G) a.dLdparams[(size_t)e * np + c] = good ? (R)rk.gp()[c] : R(0);
     if (!good && a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nknot * nu; c += G) a.dLdctrl[(size_t)e * nknot * nu + c] = R(0);
     gr.sync();
   }
@@ -153,11 +159,15 @@ template <class R> struct FieldArgs {
   WsLayout wl, rwl; RkLayout rl;
 };
 template <class R, int G>
-__global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ ModelDev<R> m, const __grid_constant__ FieldArgs<R> a) {
+__global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ FieldArgs<R> a) {
   extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ CtaConst<R> cc;
+  load_cta_const<R>(cc, m_, a.wl, a.rwl, a.rl);
+  const ModelDev<R>& m = cc.m;
+  const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
-  Rk rk; Ws<R> ws; Arr<R> Yqr, Vr;
-  bind_shared<R, G>(smem, a.rl.size_bwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, a.rl, a.wl);
+  Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
+  bind_shared<R, G>(smem, a.rl.size_bwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
   const int nq = m.nq, nv = m.nv, nx = nq + nv;
   const int ngr = (gridDim.x * blockDim.x) / G;
   for (int e = (blockIdx.x * blockDim.x + threadIdx.x) / G; e < a.n; e += ngr) {
@@ -168,20 +178,20 @@ __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ Mode
     for (int j = gr.lane; j < nv; j += G) Vr[j] = x[nq + j];
     gr.sync();
     if (!a.kappa) {
-      InPlain<R> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
+      InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
       bool conv;
-      int nr = vector_field<R, R, G, InPlain<R> >(m, in, ws, a.cfd != 0, conv, gr);
-      for (int j = gr.lane; j < nv; j += G) a.acc[(size_t)e * nv + j] = nr < 0 ? R(nan("")) : ws.x[j];
+      int nr = vector_field<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, a.cfd != 0, conv, gr);
+      for (int j = gr.lane; j < nv; j += G) a.acc[(size_t)e * nv + j] = nr < 0 ? R(nan("")) : ws.x()[j];
       if (gr.lane == 0 && a.nrow) a.nrow[e] = nr;
     } else {
-      Ws<Dual<R> > dws = bind_scratch<R>(a.scratch, a.res_size, a.rwl);
-      for (int j = gr.lane; j < nv; j += G) rk.lam[j] = (double)a.kappa[(size_t)e * nv + j];
+      Ws<Dual<R>, 32> dws = bind_scratch<R>(a.scratch, a.res_size, &cc.rwl);
+      for (int j = gr.lane; j < nv; j += G) rk.lam()[j] = (double)a.kappa[(size_t)e * nv + j];
       gr.sync();
-      bool ok = vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.lam, a.cfd != 0, a.want_p != 0, ws, dws, rk, gr);
+      bool ok = vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.lam(), a.cfd != 0, a.want_p != 0, ws, dws, rk, gr);
       R bad = R(nan(""));
-      for (int j = gr.lane; j < nv; j += G) { a.qbar[(size_t)e * nv + j] = ok ? (R)rk.qbar[j] : bad; a.vbar[(size_t)e * nv + j] = ok ? (R)rk.vbar[j] : bad; }
-      for (int j = gr.lane; j < m.nu; j += G) a.ubar[(size_t)e * m.nu + j] = ok ? (R)rk.ubar[j] : bad;
-      if (a.want_p) for (int j = gr.lane; j < m.np; j += G) a.pbar[(size_t)e * m.np + j] = ok ? (R)rk.pbar[j] : bad;
+      for (int j = gr.lane; j < nv; j += G) { a.qbar[(size_t)e * nv + j] = ok ? (R)rk.qbar()[j] : bad; a.vbar[(size_t)e * nv + j] = ok ? (R)rk.vbar()[j] : bad; }
+      for (int j = gr.lane; j < m.nu; j += G) a.ubar[(size_t)e * m.nu + j] = ok ? (R)rk.ubar()[j] : bad;
+      if (a.want_p) for (int j = gr.lane; j < m.np; j += G) a.pbar[(size_t)e * m.np + j] = ok ? (R)rk.pbar()[j] : bad;
     }
     gr.sync();
   }
@@ -189,35 +199,39 @@ __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ Mode
 
 // ---- A^: w(b) = mean diagonal of the translational block of Jc_b M(qpos0)^-1 Jc_b^T -------
 template <class R, int G>
-__global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ ModelDev<R> m, const R* qpos0, const R* zero_v, R* body_w,
+__global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ ModelDev<R> m_, const R* qpos0, const R* zero_v, R* body_w,
                                                         const __grid_constant__ WsLayout wl, const __grid_constant__ RkLayout rl) {
   extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ CtaConst<R> cc;
+  load_cta_const<R>(cc, m_, wl, wl, rl);
+  const ModelDev<R>& m = cc.m;
+  const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
-  Rk rk; Ws<R> ws; Arr<R> Yqr, Vr;
-  bind_shared<R, G>(smem, rl.size_bwd, wl.size + rl.rsize, wl.isize, rk, ws, Yqr, Vr, rl, wl);
+  Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
+  bind_shared<R, G>(smem, rl.size_bwd, wl.size + rl.rsize, wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
   if (blockIdx.x != 0 || threadIdx.x >= G) return;
   const int nv = m.nv;
   for (int j = gr.lane; j < m.nq; j += G) Yqr[j] = qpos0[j];
   for (int j = gr.lane; j < nv; j += G) Vr[j] = R(0);
   gr.sync();
-  InPlain<R> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = zero_v; in.pa = m.p_default;
-  kinematics<R, R, G, InPlain<R>, false>(m, in, ws, gr);
-  dynamics<R, R, G, InPlain<R> >(m, in, ws, gr);
-  for (int e = gr.lane; e < nv * nv; e += G) ws.Hc[e] = ws.M[e];
+  InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = zero_v; in.pa = m.p_default;
+  kinematics<Ws<R, ST>, R, G, InPlain<R, ST>, false>(m, in, ws, gr);
+  dynamics<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, gr);
+  for (int e = gr.lane; e < nv * nv; e += G) ws.Hc()[e] = ws.M()[e];
   gr.sync();
-  bool pd = cholesky<R, G>(ws.Hc, nv, gr);
+  bool pd = cholesky(ws.Hc(), nv, gr);
   for (int b = 0; b < m.nbody; ++b) {
     R tr = R(0);
     for (int c = 0; c < 3 && pd && b > 0; ++c) {
       for (int j = gr.lane; j < nv; j += G) {
         int e = m.tw_idx[b * nv + j];
         R val_ = R(0);
-        if (e >= 0) { V3<R> l = ld3(ws.tw, e); val_ = c == 0 ? l.x : (c == 1 ? l.y : l.z); }
-        ws.g[j] = val_; ws.dl[j] = val_;
+        if (e >= 0) { V3<R> l = ld3(ws.tw(), e); val_ = c == 0 ? l.x : (c == 1 ? l.y : l.z); }
+        ws.g()[j] = val_; ws.dl()[j] = val_;
       }
       gr.sync();
-      chol_solve<R, G>(ws.Hc, nv, ws.dl, gr);
-      for (int j = 0; j < nv; ++j) tr += ws.g[j] * ws.dl[j];
+      chol_solve(ws.Hc(), nv, ws.dl(), gr);
+      for (int j = 0; j < nv; ++j) tr += ws.g()[j] * ws.dl()[j];
       gr.sync();
     }
     if (gr.lane == 0) body_w[b] = pd ? tr / R(3) : R(nan(""));

@@ -16,6 +16,11 @@ namespace dmx {
 
 #define DMX_DI __device__ __forceinline__
 #define DMX_D __device__
+#ifdef DMX_NOINLINE
+#define DMX_DN __device__ __noinline__
+#else
+#define DMX_DN __device__
+#endif
 
 // ---- tangent scalar: value and one directional derivative -------------------------------
 template <class T> struct Dual {
@@ -65,15 +70,16 @@ template <class T> DMX_DI Dual<T> m_pow(const Dual<T>& a, const Dual<T>& b) {
   return Dual<T>(f, b.v * m_pow(a.v, b.v - T(1)) * a.d + f * m_log(a.v) * b.d);
 }
 
-// ---- strided array view: element i lives at p[i*st] ---------------------------------------
-// st == 1: contiguous per-group workspace in shared memory; st == 32: per-lane workspaces of a
-// warp interleaved so that lanes touching the same index coalesce (G == 1 instantiations).
-template <class S> struct Arr {
-  S* p; int st;
+// ---- strided array view: element i lives at p[i*ST] ----------------------------------------
+// ST == 1: contiguous per-group workspace in shared memory; ST == 32: per-lane workspaces of a
+// warp interleaved so that lanes touching the same index coalesce (G == 1 instantiations and the
+// per-lane tangent workspaces of the VJP).  The stride is a compile-time constant.
+template <class S, int ST> struct Arr {
+  S* p;
   DMX_DI Arr() {}
-  DMX_DI Arr(S* p_, int st_) : p(p_), st(st_) {}
-  DMX_DI S& operator[](int i) const { return p[(size_t)i * st]; }
-  DMX_DI Arr<S> at(int o) const { return Arr<S>(p + (size_t)o * st, st); }
+  DMX_DI explicit Arr(S* p_) : p(p_) {}
+  DMX_DI S& operator[](int i) const { return p[i * ST]; }
+  DMX_DI Arr<S, ST> at(int o) const { return Arr<S, ST>(p + o * ST); }
 };
 
 // ---- lane group ----------------------------------------------------------------------------
@@ -123,13 +129,13 @@ template <class S> DMX_DI M3<S> operator*(const M3<S>& A, const M3<S>& B) {
 }
 template <class S> DMX_DI V3<S> colv(const M3<S>& A, int k) { return mk3<S>(A.m[k], A.m[3 + k], A.m[6 + k]); }
 
-template <class S> DMX_DI V3<S> ld3(const Arr<S>& a, int i) { return mk3<S>(a[3 * i], a[3 * i + 1], a[3 * i + 2]); }
-template <class S> DMX_DI void st3(const Arr<S>& a, int i, const V3<S>& v) { a[3 * i] = v.x; a[3 * i + 1] = v.y; a[3 * i + 2] = v.z; }
-template <class S> DMX_DI M3<S> ld9(const Arr<S>& a, int i) { M3<S> A;
+template <class S, int ST> DMX_DI V3<S> ld3(const Arr<S, ST>& a, int i) { return mk3<S>(a[3 * i], a[3 * i + 1], a[3 * i + 2]); }
+template <class S, int ST> DMX_DI void st3(const Arr<S, ST>& a, int i, const V3<S>& v) { a[3 * i] = v.x; a[3 * i + 1] = v.y; a[3 * i + 2] = v.z; }
+template <class S, int ST> DMX_DI M3<S> ld9(const Arr<S, ST>& a, int i) { M3<S> A;
 #pragma unroll
   for (int k = 0; k < 9; ++k) A.m[k] = a[9 * i + k];
   return A; }
-template <class S> DMX_DI void st9(const Arr<S>& a, int i, const M3<S>& A) {
+template <class S, int ST> DMX_DI void st9(const Arr<S, ST>& a, int i, const M3<S>& A) {
 #pragma unroll
   for (int k = 0; k < 9; ++k) a[9 * i + k] = A.m[k]; }
 // constants of the model (real type R) lifted to the scalar S

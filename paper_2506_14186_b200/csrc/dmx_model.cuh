@@ -48,23 +48,19 @@ struct WsLayout {
   int i_incl, i_rowstart, i_rowcand, i_active, isize;
 };
 
-template <class S> struct Ws {
-  Arr<S> fp, fR, fw, fal, fvp, fap, com, dax, dan, Fb, Nb, Iw, Isub, tw, M, Hc, tau, c, a0, x, g, dl, Md, xa, kap;
-  Arr<S> cr, cn, cpos, ct1, ct2, cD, cpost, cbd, cmu, J, aref, D, s, pr;
-  Arr<int> incl, rowstart, rowcand, active;
-  DMX_DI void bind(const WsLayout& L, S* base, int st, int* ibase, int ist) {
-    Arr<S> b(base, st);
-    fp = b.at(L.fp); fR = b.at(L.fR); fw = b.at(L.fw); fal = b.at(L.fal); fvp = b.at(L.fvp); fap = b.at(L.fap);
-    com = b.at(L.com); dax = b.at(L.dax); dan = b.at(L.dan);
-    Fb = b.at(L.Fb); Nb = b.at(L.Nb); Iw = b.at(L.Iw); Isub = b.at(L.Isub); tw = b.at(L.tw);
-    M = b.at(L.M); Hc = b.at(L.Hc); tau = b.at(L.tau); c = b.at(L.c); a0 = b.at(L.a0); x = b.at(L.x); g = b.at(L.g);
-    dl = b.at(L.dl); Md = b.at(L.Md); xa = b.at(L.xa); kap = b.at(L.kap);
-    cr = b.at(L.cr); cn = b.at(L.cn); cpos = b.at(L.cpos); ct1 = b.at(L.ct1); ct2 = b.at(L.ct2);
-    cD = b.at(L.cD); cpost = b.at(L.cpost); cbd = b.at(L.cbd); cmu = b.at(L.cmu);
-    J = b.at(L.J); aref = b.at(L.aref); D = b.at(L.D); s = b.at(L.s); pr = b.at(L.pr);
-    Arr<int> ib(ibase, ist);
-    incl = ib.at(L.i_incl); rowstart = ib.at(L.i_rowstart); rowcand = ib.at(L.i_rowcand); active = ib.at(L.i_active);
-  }
+// View of one workspace: base pointer + layout (kept in shared memory); arrays are resolved on use.
+#define DMX_WS_ARR(name) DMX_DI Arr<S, ST> name() const { return Arr<S, ST>(b + L->name * ST); }
+#define DMX_WS_INT(name) DMX_DI Arr<int, ST> name() const { return Arr<int, ST>(ib + L->i_##name * ST); }
+template <class S_, int ST_> struct Ws {
+  typedef S_ S;
+  static const int ST = ST_;
+  S* b; int* ib; const WsLayout* L;
+  DMX_WS_ARR(fp) DMX_WS_ARR(fR) DMX_WS_ARR(fw) DMX_WS_ARR(fal) DMX_WS_ARR(fvp) DMX_WS_ARR(fap) DMX_WS_ARR(com) DMX_WS_ARR(dax) DMX_WS_ARR(dan)
+  DMX_WS_ARR(Fb) DMX_WS_ARR(Nb) DMX_WS_ARR(Iw) DMX_WS_ARR(Isub) DMX_WS_ARR(tw)
+  DMX_WS_ARR(M) DMX_WS_ARR(Hc) DMX_WS_ARR(tau) DMX_WS_ARR(c) DMX_WS_ARR(a0) DMX_WS_ARR(x) DMX_WS_ARR(g) DMX_WS_ARR(dl) DMX_WS_ARR(Md) DMX_WS_ARR(xa) DMX_WS_ARR(kap)
+  DMX_WS_ARR(cr) DMX_WS_ARR(cn) DMX_WS_ARR(cpos) DMX_WS_ARR(ct1) DMX_WS_ARR(ct2) DMX_WS_ARR(cD) DMX_WS_ARR(cpost) DMX_WS_ARR(cbd) DMX_WS_ARR(cmu)
+  DMX_WS_ARR(J) DMX_WS_ARR(aref) DMX_WS_ARR(D) DMX_WS_ARR(s) DMX_WS_ARR(pr)
+  DMX_WS_INT(incl) DMX_WS_INT(rowstart) DMX_WS_INT(rowcand) DMX_WS_INT(active)
 };
 
 }  // namespace dmx

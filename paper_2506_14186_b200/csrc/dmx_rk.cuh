@@ -44,9 +44,8 @@ DMX_DI void cross3(const double* a, const double* b, double* r) {
   r[0] = a[1] * b[2] - a[2] * b[1]; r[1] = a[2] * b[0] - a[0] * b[2]; r[2] = a[0] * b[1] - a[1] * b[0];
 }
 // joint jn of: qout = q (+) delta and K = chart_rate(delta, V)
-template <class R>
-DMX_DI void retract_joint(const ModelDev<R>& m, int jn, const Arr<double>& q, const Arr<double>& delta, const Arr<double>& V,
-                          const Arr<double>& qout, const Arr<double>& K) {
+template <class R, class AD>
+DMX_DI void retract_joint(const ModelDev<R>& m, int jn, const AD& q, const AD& delta, const AD& V, const AD& qout, const AD& K) {
   int qa = m.jnt_qadr[jn], va = m.jnt_vadr[jn];
   if (m.jnt_type[jn] != JNT_FREE) { qout[qa] = q[qa] + delta[va]; K[va] = V[va]; return; }
   double d[3], w[3], e[4], a[4], r[4];
@@ -72,9 +71,8 @@ DMX_DI void rot_AB(const double* d, double& A, double& B, double& C) {
   C = sm ? 1.0 / 6.0 - th2 / 120.0 : (th - s) / (th2 * th);
 }
 // joint jn of: base += T^T Qbar (T = blockdiag(I, R(exp delta)^T)), dbar += Jr(delta)^T Qbar
-template <class R>
-DMX_DI void retract_pullback_joint(const ModelDev<R>& m, int jn, const Arr<double>& delta, const Arr<double>& Qbar,
-                                   const Arr<double>& base, const Arr<double>& dbar) {
+template <class R, class AD>
+DMX_DI void retract_pullback_joint(const ModelDev<R>& m, int jn, const AD& delta, const AD& Qbar, const AD& base, const AD& dbar) {
   int va = m.jnt_vadr[jn];
   if (m.jnt_type[jn] != JNT_FREE) { base[va] += Qbar[va]; dbar[va] += Qbar[va]; return; }
   double d[3], qb[3];
@@ -85,9 +83,8 @@ DMX_DI void retract_pullback_joint(const ModelDev<R>& m, int jn, const Arr<doubl
   for (int c = 0; c < 3; ++c) { base[va + 3 + c] += qb[c] + A * k1[c] + B * k2[c]; dbar[va + 3 + c] += qb[c] + B * k1[c] + C * k2[c]; }
 }
 // joint jn of: Vbar += (dK/dV)^T Kbar, dbar += (dK/dTheta)^T Kbar
-template <class R>
-DMX_DI void chart_pullback_joint(const ModelDev<R>& m, int jn, const Arr<double>& delta, const Arr<double>& V, const Arr<double>& Kbar,
-                                 const Arr<double>& Vbar, const Arr<double>& dbar) {
+template <class R, class AD>
+DMX_DI void chart_pullback_joint(const ModelDev<R>& m, int jn, const AD& delta, const AD& V, const AD& Kbar, const AD& Vbar, const AD& dbar) {
   int va = m.jnt_vadr[jn];
   if (m.jnt_type[jn] != JNT_FREE) { Vbar[va] += Kbar[va]; return; }
   double th[3], w[3], kb[3];
@@ -107,77 +104,79 @@ struct RkLayout {
   int size_fwd, size_bwd;
   int Yqr, Vr, rsize;                        // stage inputs in the real type R
 };
-struct Rk {
-  Arr<double> q, v, Yq, V, Dl, K, A, err, sYq, sV, sDl, Kb, Ab, qb, vb, dbar, Vb, lam, delta, qbar, vbar, ubar, pbar, gp;
-  DMX_DI void bind(const RkLayout& L, double* base, int st) {
-    Arr<double> b(base, st);
-    q = b.at(L.q); v = b.at(L.v); Yq = b.at(L.Yq); V = b.at(L.V); Dl = b.at(L.Dl); K = b.at(L.K); A = b.at(L.A); err = b.at(L.err);
-    sYq = b.at(L.sYq); sV = b.at(L.sV); sDl = b.at(L.sDl); Kb = b.at(L.Kb); Ab = b.at(L.Ab); qb = b.at(L.qb); vb = b.at(L.vb);
-    dbar = b.at(L.dbar); Vb = b.at(L.Vb); lam = b.at(L.lam); delta = b.at(L.delta); qbar = b.at(L.qbar); vbar = b.at(L.vbar);
-    ubar = b.at(L.ubar); pbar = b.at(L.pbar); gp = b.at(L.gp);
-  }
+#define DMX_RK_ARR(name) DMX_DI Arr<double, ST> name() const { return Arr<double, ST>(b + L->name * ST); }
+template <int ST_> struct Rk {
+  static const int ST = ST_;
+  double* b; const RkLayout* L;
+  DMX_RK_ARR(q) DMX_RK_ARR(v) DMX_RK_ARR(Yq) DMX_RK_ARR(V) DMX_RK_ARR(Dl) DMX_RK_ARR(K) DMX_RK_ARR(A) DMX_RK_ARR(err)
+  DMX_RK_ARR(sYq) DMX_RK_ARR(sV) DMX_RK_ARR(sDl) DMX_RK_ARR(Kb) DMX_RK_ARR(Ab) DMX_RK_ARR(qb) DMX_RK_ARR(vb) DMX_RK_ARR(dbar)
+  DMX_RK_ARR(Vb) DMX_RK_ARR(lam) DMX_RK_ARR(delta) DMX_RK_ARR(qbar) DMX_RK_ARR(vbar) DMX_RK_ARR(ubar) DMX_RK_ARR(pbar) DMX_RK_ARR(gp)
 };
+// stride of the cooperative workspaces: contiguous per group, warp-interleaved for one-lane groups
+template <int G> struct StrideOf { static const int value = (G == 1) ? 32 : 1; };
 
 // ---- S7: one attempted step: stages 1..7 (stage 1 reused when have_k1), proposal, error vector -----
 // KEEP: also store every stage's (Yq, V, Dl) for the reverse sweep.
 template <class R, int G, bool KEEP>
-DMX_D void rk_attempt(const ModelDev<R>& m, int tab, const Rk& rk, const Arr<R>& Yqr, const Arr<R>& Vr, const R* u, const R* p,
-                      double h, bool have_k1, const Ws<R>& ws, bool& ok, int& unconverged, const Grp<G>& gr) {
+DMX_DN void rk_attempt(const ModelDev<R>& m, int tab, const Rk<StrideOf<G>::value>& rk, const Arr<R, StrideOf<G>::value>& Yqr,
+                       const Arr<R, StrideOf<G>::value>& Vr, const R* u, const R* p, double h, bool have_k1,
+                       const Ws<R, StrideOf<G>::value>& ws, bool& ok, int& unconverged, const Grp<G>& gr) {
+  const int ST = StrideOf<G>::value;
   const int nv = m.nv, nq = m.nq;
   ok = true; unconverged = 0;
   const int ns = KEEP ? 6 : 7;     // the reverse sweep needs stages 1..6 only
   for (int i = 0; i < ns; ++i) {
     for (int j = gr.lane; j < nv; j += G) {
       double sq = 0, sv = 0;
-      for (int l = 0; l < i; ++l) { sq += TAB_A[tab][i][l] * rk.K[l * nv + j]; sv += TAB_A[tab][i][l] * rk.A[l * nv + j]; }
-      rk.Dl[j] = h * sq; rk.V[j] = rk.v[j] + h * sv;
+      for (int l = 0; l < i; ++l) { sq += TAB_A[tab][i][l] * rk.K()[l * nv + j]; sv += TAB_A[tab][i][l] * rk.A()[l * nv + j]; }
+      rk.Dl()[j] = h * sq; rk.V()[j] = rk.v()[j] + h * sv;
     }
     gr.sync();
-    for (int jn = gr.lane; jn < m.njnt; jn += G) retract_joint<R>(m, jn, rk.q, rk.Dl, rk.V, rk.Yq, rk.K.at(i * nv));
+    for (int jn = gr.lane; jn < m.njnt; jn += G) retract_joint(m, jn, rk.q(), rk.Dl(), rk.V(), rk.Yq(), rk.K().at(i * nv));
     gr.sync();
-    for (int j = gr.lane; j < nq; j += G) { Yqr[j] = (R)rk.Yq[j]; if (KEEP && i < 6) rk.sYq[i * nq + j] = rk.Yq[j]; }
+    for (int j = gr.lane; j < nq; j += G) { Yqr[j] = (R)rk.Yq()[j]; if (KEEP && i < 6) rk.sYq()[i * nq + j] = rk.Yq()[j]; }
     for (int j = gr.lane; j < nv; j += G) {
-      Vr[j] = (R)rk.V[j];
-      if (KEEP && i < 6) { rk.sV[i * nv + j] = rk.V[j]; rk.sDl[i * nv + j] = rk.Dl[j]; }
+      Vr[j] = (R)rk.V()[j];
+      if (KEEP && i < 6) { rk.sV()[i * nv + j] = rk.V()[j]; rk.sDl()[i * nv + j] = rk.Dl()[j]; }
     }
     gr.sync();
     if (i == 0 && have_k1) continue;
-    InPlain<R> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
+    InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
     bool conv;
-    int nr = vector_field<R, R, G, InPlain<R> >(m, in, ws, false, conv, gr);
-    if (nr < 0) { ok = false; for (int j = gr.lane; j < nv; j += G) rk.A[i * nv + j] = nan(""); }
-    else { for (int j = gr.lane; j < nv; j += G) rk.A[i * nv + j] = (double)ws.x[j]; if (nr > 0 && !conv) unconverged++; }
+    int nr = vector_field<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, false, conv, gr);
+    if (nr < 0) { ok = false; for (int j = gr.lane; j < nv; j += G) rk.A()[i * nv + j] = nan(""); }
+    else { for (int j = gr.lane; j < nv; j += G) rk.A()[i * nv + j] = (double)ws.x()[j]; if (nr > 0 && !conv) unconverged++; }
     gr.sync();
   }
   if (!KEEP) {
     // row 6 of a is b: stage 7 is the proposal y_{n+1} = (Yq, V) and k7 = (V, A[6]) (FSAL)
     for (int j = gr.lane; j < nv; j += G) {
       double eq = 0, ev = 0;
-      for (int i = 0; i < 7; ++i) { eq += TAB_E[tab][i] * rk.K[i * nv + j]; ev += TAB_E[tab][i] * rk.A[i * nv + j]; }
-      rk.err[j] = h * eq; rk.err[nv + j] = h * ev;
+      for (int i = 0; i < 7; ++i) { eq += TAB_E[tab][i] * rk.K()[i * nv + j]; ev += TAB_E[tab][i] * rk.A()[i * nv + j]; }
+      rk.err()[j] = h * eq; rk.err()[nv + j] = h * ev;
     }
     gr.sync();
   }
 }
 
 // ---- S8: scaled RMS error in index order with plain adds; every lane computes it -------
-template <class R>
-DMX_D double error_norm(const ModelDev<R>& m, const Rk& rk, double rtol, double atol, bool& finite) {
+template <class R, int ST>
+DMX_DN double error_norm(const ModelDev<R>& m, const Rk<ST>& rk, double rtol, double atol, bool& finite) {
   const int nv = m.nv;
   double acc = 0.0;
   for (int d = 0; d < nv; ++d) {
     int j = m.dof_jnt[d], c = d - m.jnt_vadr[j];
     double mag = 1.0;
-    if (m.jnt_type[j] != JNT_FREE || c < 3) { int qi = m.jnt_qadr[j] + c; mag = fmax(fabs(rk.q[qi]), fabs(rk.Yq[qi])); }
-    double e = rk.err[d];
+    if (m.jnt_type[j] != JNT_FREE || c < 3) { int qi = m.jnt_qadr[j] + c; mag = fmax(fabs(rk.q()[qi]), fabs(rk.Yq()[qi])); }
+    double e = rk.err()[d];
     if (!isfinite(e)) finite = false;
     double r = __ddiv_rn(e, __dadd_rn(atol, __dmul_rn(rtol, mag)));
     acc = __dadd_rn(acc, __dmul_rn(r, r));
   }
   for (int d = 0; d < nv; ++d) {
-    double e = rk.err[nv + d];
+    double e = rk.err()[nv + d];
     if (!isfinite(e)) finite = false;
-    double r = __ddiv_rn(e, __dadd_rn(atol, __dmul_rn(rtol, fmax(fabs(rk.v[d]), fabs(rk.V[d])))));
+    double r = __ddiv_rn(e, __dadd_rn(atol, __dmul_rn(rtol, fmax(fabs(rk.v()[d]), fabs(rk.V()[d])))));
     acc = __dadd_rn(acc, __dmul_rn(r, r));
   }
   return sqrt(acc / (2 * nv));
@@ -199,31 +198,46 @@ template <class R> struct RolloutArgs {
   WsLayout wl; RkLayout rl;
 };
 
+// Shared-memory copies of the model header and the layouts (one per CTA), so that the non-inlined device
+// functions read them with plain shared loads.
+template <class R> struct CtaConst { ModelDev<R> m; WsLayout wl, rwl; RkLayout rl; };
+template <class R>
+DMX_DI void load_cta_const(CtaConst<R>& c, const ModelDev<R>& m, const WsLayout& wl, const WsLayout& rwl, const RkLayout& rl) {
+  const int* src[4] = {reinterpret_cast<const int*>(&m), reinterpret_cast<const int*>(&wl), reinterpret_cast<const int*>(&rwl), reinterpret_cast<const int*>(&rl)};
+  int* dst[4] = {reinterpret_cast<int*>(&c.m), reinterpret_cast<int*>(&c.wl), reinterpret_cast<int*>(&c.rwl), reinterpret_cast<int*>(&c.rl)};
+  const int n[4] = {(int)(sizeof(ModelDev<R>) / 4), (int)(sizeof(WsLayout) / 4), (int)(sizeof(WsLayout) / 4), (int)(sizeof(RkLayout) / 4)};
+  for (int k = 0; k < 4; ++k) for (int i = threadIdx.x; i < n[k]; i += blockDim.x) dst[k][i] = src[k][i];
+  __syncthreads();
+}
+
 // workspace bases of this thread's lane group inside the CTA's dynamic shared memory:
 // [doubles | reals | ints], each region holding all groups of the CTA
 template <class R, int G>
-DMX_DI void bind_shared(unsigned char* smem, int nd, int nr_, int ni, Rk& rk, Ws<R>& ws, Arr<R>& Yqr, Arr<R>& Vr,
-                        const RkLayout& rl, const WsLayout& wl) {
-  const int ngr = blockDim.x / G;
+DMX_DI void bind_shared(unsigned char* smem, int nd, int nr_, int ni, Rk<StrideOf<G>::value>& rk, Ws<R, StrideOf<G>::value>& ws,
+                        Arr<R, StrideOf<G>::value>& Yqr, Arr<R, StrideOf<G>::value>& Vr, const RkLayout* rl, const WsLayout* wl) {
+  const int ST = StrideOf<G>::value;
+  const int ngr = (G == 1) ? blockDim.x : blockDim.x / G;
   double* dreg = reinterpret_cast<double*>(smem);
   R* rreg = reinterpret_cast<R*>(smem + (size_t)ngr * nd * sizeof(double));
   int* ireg = reinterpret_cast<int*>(smem + (size_t)ngr * nd * sizeof(double) + (size_t)ngr * nr_ * sizeof(R));
-  int st; size_t gi;
-  if (G == 1) { st = 32; int w = threadIdx.x >> 5, l = threadIdx.x & 31; dreg += (size_t)w * 32 * nd + l; rreg += (size_t)w * 32 * nr_ + l; ireg += (size_t)w * 32 * ni + l; }
-  else { st = 1; gi = threadIdx.x / G; dreg += gi * nd; rreg += gi * nr_; ireg += gi * ni; }
-  rk.bind(rl, dreg, st);
-  ws.bind(wl, rreg, st, ireg, st);
-  Arr<R> rb(rreg, st);
-  Yqr = rb.at(rl.Yqr); Vr = rb.at(rl.Vr);
+  if (G == 1) { int w = threadIdx.x >> 5, l = threadIdx.x & 31; dreg += (size_t)w * 32 * nd + l; rreg += (size_t)w * 32 * nr_ + l; ireg += (size_t)w * 32 * ni + l; }
+  else { size_t gi = threadIdx.x / G; dreg += gi * nd; rreg += gi * nr_; ireg += gi * ni; }
+  rk.b = dreg; rk.L = rl;
+  ws.b = rreg; ws.ib = ireg; ws.L = wl;
+  Yqr = Arr<R, ST>(rreg + rl->Yqr * ST); Vr = Arr<R, ST>(rreg + rl->Vr * ST);
 }
 
 // ---- forward rollout: persistent lane groups pulling environments from a global queue --------------
 template <class R, int G>
-__global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ ModelDev<R> m, const __grid_constant__ RolloutArgs<R> a) {
+__global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ RolloutArgs<R> a) {
   extern __shared__ __align__(16) unsigned char smem[];
+  __shared__ CtaConst<R> cc;
+  load_cta_const<R>(cc, m_, a.wl, a.wl, a.rl);
+  const ModelDev<R>& m = cc.m;
+  const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
-  Rk rk; Ws<R> ws; Arr<R> Yqr, Vr;
-  bind_shared<R, G>(smem, a.rl.size_fwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, a.rl, a.wl);
+  Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
+  bind_shared<R, G>(smem, a.rl.size_fwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
   const int nq = m.nq, nv = m.nv, nu = m.nu, nx = nq + nv, tab = a.so.tableau, rec = nx + 2;
   const bool has_ctrl = a.ctrl != nullptr && a.nknot > 0 && nu > 0;
   const int nknot = has_ctrl ? a.nknot : 0;
@@ -234,8 +248,8 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
     if (e >= a.nenv) break;
     const R* x0 = a.x0 + (size_t)e * nx;
     const R* p = a.params ? a.params + (size_t)e * m.np : m.p_default;
-    for (int j = gr.lane; j < nq; j += G) rk.q[j] = (double)x0[j];
-    for (int j = gr.lane; j < nv; j += G) rk.v[j] = (double)x0[nq + j];
+    for (int j = gr.lane; j < nq; j += G) rk.q()[j] = (double)x0[j];
+    for (int j = gr.lane; j < nv; j += G) rk.v()[j] = (double)x0[nq + j];
     gr.sync();
     double t = 0.0, hprop = a.so.h0, Eprev = 1.0, hmin = INFINITY, hmax = 0.0;
     int knot = 0, attempts = 0, ir = 0, status = 0, n_acc = 0, n_rej = 0, n_feval = 0, n_unc = 0;
@@ -262,7 +276,7 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
       n_feval += have_k1 ? 6 : 7; n_unc += unc;
       have_k1 = true;
       bool finite = ok;
-      double E = error_norm<R>(m, rk, a.so.rtol, a.so.atol, finite);
+      double E = error_norm<R, ST>(m, rk, a.so.rtol, a.so.atol, finite);
       bool accept = true;
       last_nonfinite = !finite;
       if (!hr) {
@@ -277,24 +291,24 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
       bool knot_up = hits && tb < a.horizon;
       if (tape) {   // S9: checkpoint record (y_n, t_n, +-h_n); a negative h marks a step that ends a control interval
         R* r = tape + (size_t)n_acc * rec;
-        for (int j = gr.lane; j < nq; j += G) r[j] = (R)rk.q[j];
-        for (int j = gr.lane; j < nv; j += G) r[nq + j] = (R)rk.v[j];
+        for (int j = gr.lane; j < nq; j += G) r[j] = (R)rk.q()[j];
+        for (int j = gr.lane; j < nv; j += G) r[nq + j] = (R)rk.v()[j];
         if (gr.lane == 0) { r[nx] = (R)t; r[nx + 1] = (R)(knot_up ? -h : h); }
       }
       gr.sync();
-      for (int j = gr.lane; j < nq; j += G) rk.q[j] = rk.Yq[j];
-      for (int j = gr.lane; j < nv; j += G) rk.v[j] = rk.V[j];
+      for (int j = gr.lane; j < nq; j += G) rk.q()[j] = rk.Yq()[j];
+      for (int j = gr.lane; j < nv; j += G) rk.v()[j] = rk.V()[j];
       n_acc++; hmin = fmin(hmin, h); hmax = fmax(hmax, h);
       if (hits) {
         t = tb;
         if (knot_up) { knot++; have_k1 = false; }
       } else t += h;
-      if (have_k1) for (int j = gr.lane; j < nv; j += G) rk.A[j] = rk.A[6 * nv + j];
+      if (have_k1) for (int j = gr.lane; j < nv; j += G) rk.A()[j] = rk.A()[6 * nv + j];
       gr.sync();
     }
     R* xT = a.xT + (size_t)e * nx;
-    for (int j = gr.lane; j < nq; j += G) xT[j] = (R)rk.q[j];
-    for (int j = gr.lane; j < nv; j += G) xT[nq + j] = (R)rk.v[j];
+    for (int j = gr.lane; j < nq; j += G) xT[j] = (R)rk.q()[j];
+    for (int j = gr.lane; j < nv; j += G) xT[nq + j] = (R)rk.v()[j];
     if (gr.lane == 0) {
       if (a.n_accept) a.n_accept[e] = n_acc;
       if (a.n_reject) a.n_reject[e] = n_rej;
