@@ -157,6 +157,10 @@ int dmx_vjp_field(const dmx_model *m, int n, const void *x, const void *u, const
  * measured FLOP/s (2 per FMA) in *flops_per_s.  Synchronises. */
 int dmx_fma_peak(int precision, int iters, double *flops_per_s, double *ms);
 
+/* Diagnostics: per-phase SM-clock counters of the kernels (32 slots, summed over lane groups since the last call);
+ * all zero unless the library was compiled with -DDMX_PROF.  Synchronises. */
+int dmx_debug_counters(const dmx_model *m, unsigned long long *host32);
+
 const char *dmx_last_error(void);
 
 #ifdef __cplusplus

@@ -14,7 +14,7 @@ LIB_PATH = os.environ.get("DMX_LIB", os.path.join(_HERE, "libdmx.so"))
 
 SYMBOLS = ["dmx_model_create", "dmx_model_destroy", "dmx_model_np", "dmx_model_nc", "dmx_model_default_params",
            "dmx_model_lanes", "dmx_tape_bytes", "dmx_rollout", "dmx_rollout_grad", "dmx_rollout_backward",
-           "dmx_vector_field", "dmx_vjp_field", "dmx_fma_peak", "dmx_last_error"]
+           "dmx_vector_field", "dmx_vjp_field", "dmx_fma_peak", "dmx_debug_counters", "dmx_last_error"]
 
 _pd, _pi = C.POINTER(C.c_double), C.POINTER(C.c_int)
 _INT_FIELDS = ["nbody", "njnt", "nq", "nv", "nu", "ngeom", "npair"]
@@ -73,6 +73,7 @@ def load():
         L.dmx_vector_field.argtypes = [vp, i, vp, vp, vp, i, vp, vp, vp]
         L.dmx_vjp_field.argtypes = [vp, i, vp, vp, vp, vp, i, vp, vp, vp, vp, vp]
         L.dmx_fma_peak.argtypes = [i, i, _pd, _pd]
+        L.dmx_debug_counters.argtypes = [vp, vp]
         _lib = L
     return _lib
 
@@ -147,6 +148,12 @@ class Model:
         p = np.zeros(self.np_)
         load().dmx_model_default_params(self.h, p.ctypes.data_as(C.c_void_p))
         return p
+
+    def debug_counters(self):
+        a = np.zeros(32, dtype=np.uint64)
+        if load().dmx_debug_counters(self.h, a.ctypes.data_as(C.c_void_p)) != 0:
+            raise RuntimeError("dmx_debug_counters: " + _err())
+        return a
 
     def tape_bytes(self, nenv, tape_steps):
         return int(load().dmx_tape_bytes(self.h, int(nenv), int(tape_steps)))

@@ -25,12 +25,13 @@ template <class R> struct Launchers {
   cudaError_t (*backward)(const ModelDev<R>&, const BackwardArgs<R>&, LaunchCfg, cudaStream_t);
   cudaError_t (*field)(const ModelDev<R>&, const FieldArgs<R>&, LaunchCfg, cudaStream_t);
   cudaError_t (*invweight)(const ModelDev<R>&, const R*, const R*, R*, const WsLayout&, const RkLayout&, LaunchCfg, cudaStream_t);
-  cudaError_t (*occupancy)(int, size_t, size_t, int*, int*);
+  cudaError_t (*occupancy)(int, size_t, size_t, size_t, int*, int*, int*);
+  cudaError_t (*prof_dump)(unsigned long long*, cudaStream_t);
 };
 template <class R, int G> Launchers<R> make_launchers() {
   Launchers<R> l;
   l.rollout = &launch_rollout<R, G>; l.backward = &launch_backward<R, G>; l.field = &launch_field<R, G>;
-  l.invweight = &launch_invweight<R, G>; l.occupancy = &kernel_occupancy<R, G>;
+  l.invweight = &launch_invweight<R, G>; l.occupancy = &kernel_occupancy<R, G>; l.prof_dump = &launch_prof_dump<R, G>;
   return l;
 }
 template <class R> Launchers<R> launchers_for(int G) {
@@ -56,7 +57,7 @@ struct Arena {
 struct HostModel {   // flattened description, doubles
   int nbody, njnt, nq, nv, nu, npair, nc, np, nlevel, ntw, nmp, nrmax, newton_iters, ls_iters;
   std::vector<int> body_parent, body_jnt, level_ptr, level_body, jnt_type, jnt_qadr, jnt_vadr, jnt_body, dof_jnt, dof_body, dof_rot,
-      tw_ptr, tw_body, tw_dof, tw_idx, sub_ptr, sub_body, mp_i, mp_j, mp_deep, ct_kind, ct_b1, ct_b2, ct_condim, ct_pair, act_type, act_jnt;
+      tw_ptr, tw_body, tw_dof, tw_idx, sub_ptr, sub_body, child_ptr, child_idx, mp_i, mp_j, mp_deep, ct_kind, ct_b1, ct_b2, ct_condim, ct_pair, act_type, act_jnt;
   std::vector<double> body_pos, body_rot, body_ipos, body_irot, body_iunit, jnt_axis, jnt_pos, jnt_damping, jnt_armature, ct_p1, ct_p2,
       ct_rho1, ct_rho2, ct_n, ct_t1, ct_t2, pair_invweight, pair_solimp_cfd, pair_cfd_beta, act_gear, act_kp, act_kd, p_default, qpos0;
   std::vector<int> pair_body1, pair_body2;
@@ -118,6 +119,9 @@ void flatten(const dmx_model_desc* d, HostModel& h) {
     if (b > 0) for (int c = b; c < nb; ++c) if (anc(b, c)) h.sub_body.push_back(c);
   }
   h.tw_ptr[nb] = (int)h.tw_dof.size(); h.sub_ptr[nb] = (int)h.sub_body.size(); h.ntw = (int)h.tw_dof.size();
+  h.child_ptr.assign(nb + 1, 0);
+  for (int b = 0; b < nb; ++b) { h.child_ptr[b] = (int)h.child_idx.size(); for (int c = b + 1; c < nb; ++c) if (h.body_parent[c] == b) h.child_idx.push_back(c); }
+  h.child_ptr[nb] = (int)h.child_idx.size();
   for (int i = 0; i < nv; ++i) for (int j = 0; j <= i; ++j) {
     int bi = h.dof_body[i], bj = h.dof_body[j];
     h.mp_i.push_back(i); h.mp_j.push_back(j);
@@ -211,7 +215,7 @@ template <class R> void build_dev(const HostModel& h, Arena& ar, ModelDev<R>& m,
   if (!patch) {
     offs.clear();
     const std::vector<int>* iv[] = {&h.body_parent, &h.body_jnt, &h.level_ptr, &h.level_body, &h.jnt_type, &h.jnt_qadr, &h.jnt_vadr, &h.jnt_body,
-                                    &h.dof_jnt, &h.dof_body, &h.dof_rot, &h.tw_ptr, &h.tw_body, &h.tw_dof, &h.tw_idx, &h.sub_ptr, &h.sub_body,
+                                    &h.dof_jnt, &h.dof_body, &h.dof_rot, &h.tw_ptr, &h.tw_body, &h.tw_dof, &h.tw_idx, &h.sub_ptr, &h.sub_body, &h.child_ptr, &h.child_idx,
                                     &h.mp_i, &h.mp_j, &h.mp_deep, &h.ct_kind, &h.ct_b1, &h.ct_b2, &h.ct_condim, &h.ct_pair, &h.act_type, &h.act_jnt};
     for (auto v : iv) offs.push_back(add_int(ar, *v));
     const std::vector<double>* rv[] = {&h.body_pos, &h.body_rot, &h.body_ipos, &h.body_irot, &h.body_iunit, &h.jnt_axis, &h.jnt_pos, &h.jnt_damping,
@@ -228,7 +232,7 @@ template <class R> void build_dev(const HostModel& h, Arena& ar, ModelDev<R>& m,
   auto ip = [&]() { return reinterpret_cast<const int*>(ar.dev + offs[k++]); };
   auto rp = [&]() { return reinterpret_cast<const R*>(ar.dev + offs[k++]); };
   m.body_parent = ip(); m.body_jnt = ip(); m.level_ptr = ip(); m.level_body = ip(); m.jnt_type = ip(); m.jnt_qadr = ip(); m.jnt_vadr = ip(); m.jnt_body = ip();
-  m.dof_jnt = ip(); m.dof_body = ip(); m.dof_rot = ip(); m.tw_ptr = ip(); m.tw_body = ip(); m.tw_dof = ip(); m.tw_idx = ip(); m.sub_ptr = ip(); m.sub_body = ip();
+  m.dof_jnt = ip(); m.dof_body = ip(); m.dof_rot = ip(); m.tw_ptr = ip(); m.tw_body = ip(); m.tw_dof = ip(); m.tw_idx = ip(); m.sub_ptr = ip(); m.sub_body = ip(); m.child_ptr = ip(); m.child_idx = ip();
   m.mp_i = ip(); m.mp_j = ip(); m.mp_deep = ip(); m.ct_kind = ip(); m.ct_b1 = ip(); m.ct_b2 = ip(); m.ct_condim = ip(); m.ct_pair = ip(); m.act_type = ip(); m.act_jnt = ip();
   m.body_pos = rp(); m.body_rot = rp(); m.body_ipos = rp(); m.body_irot = rp(); m.body_iunit = rp(); m.jnt_axis = rp(); m.jnt_pos = rp(); m.jnt_damping = rp();
   m.jnt_armature = rp(); m.ct_p1 = rp(); m.ct_p2 = rp(); m.ct_rho1 = rp(); m.ct_rho2 = rp(); m.ct_n = rp(); m.ct_t1 = rp(); m.ct_t2 = rp(); m.pair_invweight = rp();
@@ -239,12 +243,13 @@ template <class R> void build_dev(const HostModel& h, Arena& ar, ModelDev<R>& m,
 
 // ---- the model object -------------------------------------------------------------------------------------
 struct dmx_model {
-  int precision, G, block, sm_count;
+  int precision, G, sm_count, max_smem;
   HostModel h;
   Arena arena;
   ModelDev<double> md; ModelDev<float> mf;
   WsLayout wl, rwl; RkLayout rl;
-  size_t smem_fwd, smem_bwd; int occ_fwd, occ_bwd;
+  struct Cfg { int block = 0, occ = 0; size_t smem = 0; } cf, cb, cx;   // forward, backward, field kernels
+  void* rk_scratch = nullptr; size_t rk_scratch_bytes = 0;              // backward integrator arrays (global memory)
   int* queue = nullptr;            // [4] work-queue counters
   void* zero_u = nullptr;          // zeros: controls when ctrl == NULL, velocities at create
   void* scratch = nullptr; size_t scratch_bytes = 0;   // tangent workspaces of the VJP lanes
@@ -254,15 +259,26 @@ namespace {
 
 size_t rsize(const dmx_model* m) { return m->precision == 64 ? sizeof(double) : sizeof(float); }
 
-size_t group_bytes(const dmx_model* m, bool bwd) {
-  return (size_t)(bwd ? m->rl.size_bwd : m->rl.size_fwd) * sizeof(double) + (size_t)(m->wl.size + m->rl.rsize) * rsize(m) +
-         (size_t)m->wl.isize * sizeof(int);
+// shared memory of one lane group: kind 0 forward (integrator arrays + field workspace), 1 backward (field workspace
+// only; the integrator / adjoint arrays live in global memory), 2 field kernels (both)
+size_t group_bytes(const dmx_model* m, int kind) {
+  size_t rk = kind == 0 ? m->rl.size_fwd : (kind == 1 ? 0 : m->rl.size_bwd);
+  return rk * sizeof(double) + (size_t)(m->wl.size + m->rl.rsize) * rsize(m) + (size_t)m->wl.isize * sizeof(int);
 }
-int groups_per_block(const dmx_model* m) { return m->G == 1 ? m->block : m->block / m->G; }
+int groups_per_block(const dmx_model* m, int block) { return m->G == 1 ? block : block / m->G; }
 
-int ensure_scratch(dmx_model* m, int grid) {
+int ensure_scratch(dmx_model* m, int grid, int block, bool rk) {
+  if (rk) {
+    size_t need2 = (size_t)grid * block * (size_t)m->rl.size_bwd * sizeof(double);   // >= groups * size_bwd
+    if (need2 > m->rk_scratch_bytes) {
+      if (m->rk_scratch) cudaFree(m->rk_scratch);
+      m->rk_scratch = nullptr; m->rk_scratch_bytes = 0;
+      CUDA_OK(cudaMalloc(&m->rk_scratch, need2));
+      m->rk_scratch_bytes = need2;
+    }
+  }
   size_t dual = 2 * rsize(m);
-  size_t need = (size_t)grid * (m->block / 32) * 32 * (size_t)m->rwl.size * dual;
+  size_t need = (size_t)grid * (block / 32) * 32 * (size_t)m->rwl.size * dual;
   if (need <= m->scratch_bytes) return 0;
   if (m->scratch) cudaFree(m->scratch);
   m->scratch = nullptr; m->scratch_bytes = 0;
@@ -296,7 +312,7 @@ int create_typed(dmx_model* m) {
   R *dq0 = nullptr, *dw = nullptr;
   CUDA_OK(cudaMalloc(&dq0, sizeof(R) * h.nq)); CUDA_OK(cudaMalloc(&dw, sizeof(R) * h.nbody));
   CUDA_OK(cudaMemcpy(dq0, q0.data(), sizeof(R) * h.nq, cudaMemcpyHostToDevice));
-  LaunchCfg c; c.block = 32; c.grid = 1; c.smem = (m->G == 1 ? 32 : 32 / m->G) * group_bytes(m, true);
+  LaunchCfg c; c.block = 32; c.grid = 1; c.smem = groups_per_block(m, 32) * group_bytes(m, 2);
   CUDA_OK(L.invweight(dev, dq0, (const R*)m->zero_u, dw, m->wl, m->rl, c, 0));
   CUDA_OK(cudaDeviceSynchronize());
   std::vector<R> bw(h.nbody);
@@ -307,8 +323,25 @@ int create_typed(dmx_model* m) {
   for (int i = 0; i < h.npair; ++i) { h.pair_invweight[i] = (double)bw[h.pair_body1[i]] + (double)bw[h.pair_body2[i]]; pw[i] = (R)h.pair_invweight[i]; }
   if (h.npair) CUDA_OK(cudaMemcpy(const_cast<R*>(dev.pair_invweight), pw.data(), sizeof(R) * h.npair, cudaMemcpyHostToDevice));
   if (sizeof(R) == 8) std::memcpy(&m->md, &dev, sizeof(dev)); else std::memcpy(&m->mf, &dev, sizeof(dev));
-  CUDA_OK(L.occupancy(m->block, m->smem_fwd, m->smem_bwd, &m->occ_fwd, &m->occ_bwd));
-  if (m->occ_fwd < 1 || m->occ_bwd < 1) return fail("kernel does not fit on an SM (shared memory / registers)");
+  // block size per kernel: the one that keeps the most lane groups resident on an SM
+  const int blocks[3] = {128, 64, 32};
+  for (int bi = 0; bi < 3; ++bi) {
+    int blk = blocks[bi], g = groups_per_block(m, blk);
+    size_t sf = g * group_bytes(m, 0), sb = g * group_bytes(m, 1), sx = g * group_bytes(m, 2);
+    int of = 0, ob = 0, ox = 0;
+    size_t lim = (size_t)m->max_smem - 2048;     // room for the static shared constants
+    CUDA_OK(L.occupancy(blk, std::min(sf, lim), std::min(sb, lim), std::min(sx, lim), &of, &ob, &ox));
+    if (sf <= lim && of * g > m->cf.occ * groups_per_block(m, std::max(m->cf.block, 1))) { m->cf.block = blk; m->cf.occ = of; m->cf.smem = sf; }
+    if (sb <= lim && ob * g > m->cb.occ * groups_per_block(m, std::max(m->cb.block, 1))) { m->cb.block = blk; m->cb.occ = ob; m->cb.smem = sb; }
+    if (sx <= lim && ox * g > m->cx.occ * groups_per_block(m, std::max(m->cx.block, 1))) { m->cx.block = blk; m->cx.occ = ox; m->cx.smem = sx; }
+  }
+  if (m->cf.occ < 1 || m->cb.occ < 1 || m->cx.occ < 1) return fail("model too large for the per-environment shared-memory workspace (try DMX_LANES=32)");
+  if (std::getenv("DMX_VERBOSE"))
+    std::fprintf(stderr, "dmx: lanes %d | fwd block %d x occ %d smem %zu | bwd block %d x occ %d smem %zu | field block %d x occ %d smem %zu | group bytes f/b %zu/%zu\n",
+                 m->G, m->cf.block, m->cf.occ, m->cf.smem, m->cb.block, m->cb.occ, m->cb.smem, m->cx.block, m->cx.occ, m->cx.smem, group_bytes(m, 0), group_bytes(m, 1));
+  // the occupancy queries above left the largest attribute set; restore the chosen sizes
+  int d0, d1, d2;
+  CUDA_OK(L.occupancy(m->cf.block, m->cf.smem, m->cb.smem, m->cx.smem, &d0, &d1, &d2));
   return 0;
 }
 
@@ -340,9 +373,9 @@ int rollout_typed(const dmx_model* m, int nenv, const void* x0, const void* ctrl
             a.h_min = st->h_min; a.h_max = st->h_max; a.t_end = st->t_end; }
   a.queue = m->queue; a.wl = m->wl; a.rl = m->rl;
   CUDA_OK(cudaMemsetAsync(m->queue, 0, sizeof(int), s));
-  LaunchCfg c; c.block = m->block; c.smem = m->smem_fwd;
-  int gpb = groups_per_block(m);
-  c.grid = std::max(1, std::min(m->occ_fwd * m->sm_count, (nenv + gpb - 1) / gpb));
+  LaunchCfg c; c.block = m->cf.block; c.smem = m->cf.smem;
+  int gpb = groups_per_block(m, c.block);
+  c.grid = std::max(1, std::min(m->cf.occ * m->sm_count, (nenv + gpb - 1) / gpb));
   CUDA_OK(launchers_for<R>(m->G).rollout(dev_of<R>(m), a, c, s));
   return 0;
 }
@@ -356,16 +389,17 @@ int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const vo
   size_t hdr = tape_header_bytes(nenv);
   if (!tape || tape_bytes < hdr + (size_t)nenv * rec * sizeof(R)) return fail("tape missing or too small");
   a.nenv = nenv; a.nknot = nknot; a.want_p = dLdparams != nullptr; a.cfd = cfd_on;
+  { const char* e = std::getenv("DMX_DBG"); a.dbg = e ? std::atoi(e) : 0; }   // timing experiments only (results invalid when set)
   a.tape_cap = (int)std::min<size_t>((tape_bytes - hdr) / ((size_t)nenv * rec * sizeof(R)), (size_t)1 << 30);
   a.tape_hdr = (const int*)tape; a.tape = (const R*)((const unsigned char*)tape + hdr);
   a.ctrl = (const R*)ctrl; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u; a.xT = (const R*)xT; a.dLdxT = (const R*)dLdxT;
   a.status = status; a.so = opts_of(opts); a.dLdx0 = (R*)dLdx0; a.dLdctrl = (R*)dLdctrl; a.dLdparams = (R*)dLdparams;
   a.queue = m->queue + 1; a.wl = m->wl; a.rwl = m->rwl; a.rl = m->rl; a.res_size = m->rwl.size;
-  LaunchCfg c; c.block = m->block; c.smem = m->smem_bwd;
-  int gpb = groups_per_block(m);
-  c.grid = std::max(1, std::min(m->occ_bwd * m->sm_count, (nenv + gpb - 1) / gpb));
-  if (ensure_scratch(m, c.grid)) return -1;
-  a.scratch = (Dual<R>*)m->scratch;
+  LaunchCfg c; c.block = m->cb.block; c.smem = m->cb.smem;
+  int gpb = groups_per_block(m, c.block);
+  c.grid = std::max(1, std::min(m->cb.occ * m->sm_count, (nenv + gpb - 1) / gpb));
+  if (ensure_scratch(m, c.grid, c.block, true)) return -1;
+  a.scratch = (Dual<R>*)m->scratch; a.rk_scratch = (double*)m->rk_scratch;
   CUDA_OK(cudaMemsetAsync(m->queue + 1, 0, sizeof(int), s));
   if (dLdctrl && nknot > 0 && m->h.nu > 0) CUDA_OK(cudaMemsetAsync(dLdctrl, 0, (size_t)nenv * nknot * m->h.nu * sizeof(R), s));
   CUDA_OK(launchers_for<R>(m->G).backward(dev_of<R>(m), a, c, s));
@@ -379,10 +413,10 @@ int field_typed(dmx_model* m, int n, const void* x, const void* u, const void* p
   a.n = n; a.cfd = cfd; a.want_p = pbar != nullptr; a.x = (const R*)x; a.u = (const R*)u; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u;
   a.kappa = (const R*)kappa; a.acc = (R*)acc; a.nrow = nrow; a.qbar = (R*)qbar; a.vbar = (R*)vbar; a.ubar = (R*)ubar; a.pbar = (R*)pbar;
   a.wl = m->wl; a.rwl = m->rwl; a.rl = m->rl; a.res_size = m->rwl.size;
-  LaunchCfg c; c.block = m->block; c.smem = m->smem_bwd;
-  int gpb = groups_per_block(m);
-  c.grid = std::max(1, std::min(m->occ_bwd * m->sm_count, (n + gpb - 1) / gpb));
-  if (kappa) { if (ensure_scratch(m, c.grid)) return -1; a.scratch = (Dual<R>*)m->scratch; }
+  LaunchCfg c; c.block = m->cx.block; c.smem = m->cx.smem;
+  int gpb = groups_per_block(m, c.block);
+  c.grid = std::max(1, std::min(m->cx.occ * m->sm_count, (n + gpb - 1) / gpb));
+  if (kappa) { if (ensure_scratch(m, c.grid, c.block, false)) return -1; a.scratch = (Dual<R>*)m->scratch; }
   CUDA_OK(launchers_for<R>(m->G).field(dev_of<R>(m), a, c, s));
   return 0;
 }
@@ -433,17 +467,7 @@ int dmx_model_create(const dmx_model_desc* desc, int precision, dmx_model** out)
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
     fail("no CUDA device: the dmx library has no CPU fallback"); delete m; return -1;
   }
-  int max_smem = 0; cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-  m->block = m->G == 1 ? 32 : 128;
-  for (;;) {
-    m->smem_fwd = groups_per_block(m) * group_bytes(m, false); m->smem_bwd = groups_per_block(m) * group_bytes(m, true);
-    if ((int)m->smem_bwd <= max_smem || m->block == 32) break;
-    m->block /= 2;
-  }
-  if ((int)m->smem_bwd > max_smem) {
-    if (m->G < 32) { fail("model too large for shared memory at this lane count; set DMX_LANES=32"); delete m; return -1; }
-    fail("model too large for the per-environment shared-memory workspace"); delete m; return -1;
-  }
+  m->max_smem = 0; cudaDeviceGetAttribute(&m->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   size_t zbytes = sizeof(double) * (size_t)std::max(std::max(m->h.nu, m->h.nv), 1);
   if (cudaMalloc(&m->zero_u, zbytes) != cudaSuccess || cudaMemset(m->zero_u, 0, zbytes) != cudaSuccess ||
       cudaMalloc(&m->queue, 4 * sizeof(int)) != cudaSuccess) { fail("cudaMalloc failed"); dmx_model_destroy(m); return -1; }
@@ -459,6 +483,7 @@ void dmx_model_destroy(dmx_model* m) {
   if (m->queue) cudaFree(m->queue);
   if (m->zero_u) cudaFree(m->zero_u);
   if (m->scratch) cudaFree(m->scratch);
+  if (m->rk_scratch) cudaFree(m->rk_scratch);
   delete m;
 }
 
@@ -530,6 +555,17 @@ int dmx_vjp_field(const dmx_model* m, int n, const void* x, const void* u, const
   cudaStream_t s = (cudaStream_t)cuda_stream;
   return m->precision == 64 ? field_typed<double>(mm, n, x, u, params, kappa, cfd, nullptr, nullptr, qbar, vbar, ubar, pbar, s)
                             : field_typed<float>(mm, n, x, u, params, kappa, cfd, nullptr, nullptr, qbar, vbar, ubar, pbar, s);
+}
+
+int dmx_debug_counters(const dmx_model* m, unsigned long long* host32) {
+  if (!m || !host32) return fail("null argument");
+  unsigned long long* d = nullptr;
+  CUDA_OK(cudaMalloc(&d, 32 * sizeof(unsigned long long)));
+  cudaError_t e = m->precision == 64 ? launchers_for<double>(m->G).prof_dump(d, 0) : launchers_for<float>(m->G).prof_dump(d, 0);
+  if (e == cudaSuccess) e = cudaMemcpy(host32, d, 32 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  CUDA_OK(e);
+  return 0;
 }
 
 int dmx_fma_peak(int precision, int iters, double* flops_per_s, double* ms) {

@@ -122,7 +122,9 @@ DMX_DN void kinematics(const ModelDev<R>& m, const IN& in, const WS& ws, const G
     st9(ws.fR(), 0, I);
   }
   gr.sync();
+#pragma unroll 1
   for (int lv = 0; lv < m.nlevel; ++lv) {
+#pragma unroll 1
     for (int i = m.level_ptr[lv] + gr.lane; i < m.level_ptr[lv + 1]; i += G) body_kin<WS, R, IN, ACC>(m, in, ws, m.level_body[i]);
     gr.sync();
   }
@@ -167,27 +169,33 @@ template <class WS, class R, int G, class IN>
 DMX_DN void dynamics(const ModelDev<R>& m, const IN& in, const WS& ws, const Grp<G>& gr) {
   typedef typename WS::S S;
   const int nv = m.nv, nb = m.nbody;
+#pragma unroll 1
   for (int b = 1 + gr.lane; b < nb; b += G) {
     V3<S> Fb, Nb; M3<S> Iw;
     body_wrench<WS, R, IN>(m, in, ws, b, Fb, Nb, Iw);
     st3(ws.Fb(), b, Fb); st3(ws.Nb(), b, Nb); st9(ws.Iw(), b, Iw);
   }
+#pragma unroll 1
   for (int e = gr.lane; e < m.ntw; e += G) {
     int j = m.tw_dof[e];
     st3(ws.tw(), e, twist_lin(ws, j, m.dof_rot[j], ld3(ws.com(), m.tw_body[e])));
   }
   gr.sync();
+#pragma unroll 1
   for (int i = gr.lane; i < 9 * (nb - 1); i += G) {
     int b = 1 + i / 9, k = i % 9;
     S acc(0.0);
+#pragma unroll 1
     for (int t = m.sub_ptr[b]; t < m.sub_ptr[b + 1]; ++t) acc = acc + ws.Iw()[9 * m.sub_body[t] + k];
     ws.Isub()[9 * b + k] = acc;
   }
   gr.sync();
+#pragma unroll 1
   for (int e = gr.lane; e < m.nmp; e += G) {
     int i = m.mp_i[e], j = m.mp_j[e], deep = m.mp_deep[e];
     S acc(0.0);
     if (deep >= 0) {
+#pragma unroll 1
       for (int t = m.sub_ptr[deep]; t < m.sub_ptr[deep + 1]; ++t) {
         int b = m.sub_body[t];
         acc = acc + in.p(b) * dot(ld3(ws.tw(), m.tw_idx[b * nv + i]), ld3(ws.tw(), m.tw_idx[b * nv + j]));
@@ -197,10 +205,12 @@ DMX_DN void dynamics(const ModelDev<R>& m, const IN& in, const WS& ws, const Grp
     }
     ws.M()[i * nv + j] = acc; ws.M()[j * nv + i] = acc;
   }
+#pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) {
     int bj = m.dof_body[j], rot = m.dof_rot[j];
     V3<S> ax = ld3(ws.dax(), j);
     S acc(0.0);
+#pragma unroll 1
     for (int t = m.sub_ptr[bj]; t < m.sub_ptr[bj + 1]; ++t) {
       int b = m.sub_body[t];
       acc = acc + dot(ld3(ws.tw(), m.tw_idx[b * nv + j]), ld3(ws.Fb(), b));
@@ -208,6 +218,7 @@ DMX_DN void dynamics(const ModelDev<R>& m, const IN& in, const WS& ws, const Grp
     }
     ws.c()[j] = acc;
     S tau = -(S(m.jnt_damping[m.dof_jnt[j]]) * in.v(j));
+#pragma unroll 1
     for (int i = 0; i < m.nu; ++i) {
       int jn = m.act_jnt[i];
       if (m.jnt_vadr[jn] != j) continue;
@@ -229,9 +240,12 @@ DMX_DI void tri_index(int e, int& a, int& b) {
 
 // ---- dense Cholesky on the lower triangle, one column at a time, lanes over rows ---------------
 template <class S, int ST, int G> DMX_DN bool cholesky(const Arr<S, ST>& A, int n, const Grp<G>& gr) {
+#pragma unroll 1
   for (int j = 0; j < n; ++j) {
+#pragma unroll 1
     for (int i = j + gr.lane; i < n; i += G) {
       S t = A[i * n + j];
+#pragma unroll 1
       for (int k = 0; k < j; ++k) t = t - A[i * n + k] * A[j * n + k];
       A[i * n + j] = t;
     }
@@ -240,6 +254,7 @@ template <class S, int ST, int G> DMX_DN bool cholesky(const Arr<S, ST>& A, int 
     if (!(val(s) > 0)) return false;       // uniform over the group
     S l = m_sqrt(s);
     gr.sync();
+#pragma unroll 1
     for (int i = j + gr.lane; i < n; i += G) A[i * n + j] = (i == j) ? l : A[i * n + j] / l;
     gr.sync();
   }
@@ -247,18 +262,24 @@ template <class S, int ST, int G> DMX_DN bool cholesky(const Arr<S, ST>& A, int 
 }
 // b <- (L L^T)^-1 b; column-oriented substitutions
 template <class S, int ST, int G> DMX_DN void chol_solve(const Arr<S, ST>& L, int n, const Arr<S, ST>& b, const Grp<G>& gr) {
+#pragma unroll 1
   for (int i = 0; i < n; ++i) {
     S bi = b[i] / L[i * n + i];
+#pragma unroll 1
     for (int k = i + 1 + gr.lane; k < n; k += G) b[k] = b[k] - L[k * n + i] * bi;
     gr.sync();
   }
+#pragma unroll 1
   for (int i = gr.lane; i < n; i += G) b[i] = b[i] / L[i * n + i];
   gr.sync();
+#pragma unroll 1
   for (int i = n - 1; i >= 0; --i) {
     S bi = b[i] / L[i * n + i];
+#pragma unroll 1
     for (int k = gr.lane; k < i; k += G) b[k] = b[k] - L[i * n + k] * bi;
     gr.sync();
   }
+#pragma unroll 1
   for (int i = gr.lane; i < n; i += G) b[i] = b[i] / L[i * n + i];
   gr.sync();
 }
@@ -364,6 +385,7 @@ template <class WS, class R, int G, class IN>
 DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, const Grp<G>& gr) {
   typedef typename WS::S S;
   const int nv = m.nv, nc = m.nc;
+#pragma unroll 1
   for (int c = gr.lane; c < nc; c += G) {
     GeoT<S> g = collide<WS, R>(m, ws, c);
     ws.cr()[c] = g.r; st3(ws.cn(), c, g.n); st3(ws.cpos(), c, g.pos); st3(ws.ct1(), c, g.t1); st3(ws.ct2(), c, g.t2);
@@ -377,6 +399,7 @@ DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
   }
   gr.sync();
   int nr = 0;
+#pragma unroll 1
   for (int c = 0; c < nc; ++c) {
     int n = ws.incl()[c];
     if (gr.lane == 0) { ws.rowstart()[c] = nr; for (int e = 0; e < n; ++e) ws.rowcand()[nr + e] = 4 * c + e; }
@@ -385,6 +408,7 @@ DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
   gr.sync();
   if (nr == 0) return 0;
   // Jacobian entries: one (candidate, dof) item yields that candidate's 1 or 4 row entries
+#pragma unroll 1
   for (int it = gr.lane; it < nc * nv; it += G) {
     int c = it / nv, j = it - c * nv;
     int n = ws.incl()[c];
@@ -401,9 +425,11 @@ DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
     }
   }
   gr.sync();
+#pragma unroll 1
   for (int i = gr.lane; i < nr; i += G) {
     int c = ws.rowcand()[i] >> 2;
     S Jv(0.0);
+#pragma unroll 1
     for (int j = 0; j < nv; ++j) Jv = Jv + ws.J()[i * nv + j] * in.v(j);
     ws.aref()[i] = ws.cpost()[c] - ws.cbd()[c] * Jv;
     ws.D()[i] = ws.cD()[c];
@@ -419,27 +445,37 @@ DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
 template <class WS, int G>
 DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G>& gr) {
   typedef typename WS::S S;
+#pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) ws.x()[j] = ws.a0()[j];
   gr.sync();
   if (nr == 0) return true;
   bool conv = false;
+#pragma unroll 1
   for (int it = 0; it < n_it; ++it) {
+#pragma unroll 1
     for (int i = gr.lane; i < nr; i += G) {
       S t(0.0);
+#pragma unroll 1
       for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.x()[j];
       ws.s()[i] = t - ws.aref()[i];
     }
+#pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) ws.xa()[j] = ws.x()[j] - ws.a0()[j];
     gr.sync();
+#pragma unroll 1
     for (int a = gr.lane; a < nv; a += G) {
       S t(0.0);
+#pragma unroll 1
       for (int b = 0; b < nv; ++b) t = t + ws.M()[a * nv + b] * ws.xa()[b];
+#pragma unroll 1
       for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.J()[i * nv + a] * ws.D()[i] * ws.s()[i];
       ws.g()[a] = t; ws.dl()[a] = -t;
     }
+#pragma unroll 1
     for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
       int a, b; tri_index(e, a, b);
       S t = ws.M()[a * nv + b];
+#pragma unroll 1
       for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.D()[i] * ws.J()[i * nv + a] * ws.J()[i * nv + b];
       ws.Hc()[a * nv + b] = t;
     }
@@ -447,8 +483,10 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
     if (!cholesky(ws.Hc(), nv, gr)) break;
     chol_solve(ws.Hc(), nv, ws.dl(), gr);
     bool same = true;
+#pragma unroll 1
     for (int i = gr.lane; i < nr; i += G) {
       S t(0.0);
+#pragma unroll 1
       for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.dl()[j];
       ws.pr()[i] = t;
       if ((val(ws.s()[i]) < 0) != (val(ws.s()[i] + t) < 0)) same = false;
@@ -459,19 +497,24 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
     if (!same) {
       // D1: phi'(a) = dl^T M (x + a dl - a0) + sum_i D_i p_i min(0, s_i + a p_i); every lane runs the
       // scalar line search redundantly in row order (same summation order as a serial code)
+#pragma unroll 1
       for (int a = gr.lane; a < nv; a += G) {
         S t(0.0);
+#pragma unroll 1
         for (int b = 0; b < nv; ++b) t = t + ws.M()[a * nv + b] * ws.dl()[b];
         ws.Md()[a] = t;
       }
       gr.sync();
       S dMd(0.0), dMxa(0.0);
+#pragma unroll 1
       for (int a = 0; a < nv; ++a) { dMd = dMd + ws.dl()[a] * ws.Md()[a]; dMxa = dMxa + ws.Md()[a] * ws.xa()[a]; }
       S lo(0.0), hi(0.0), a(0.0), d2, d1a; bool hi_inf = true, frozen = false;
       {
         d1a = dMxa; d2 = dMd;
+#pragma unroll 1
         for (int i = 0; i < nr; ++i) { S si = ws.s()[i]; if (val(si) < 0) { d1a = d1a + ws.D()[i] * ws.pr()[i] * si; d2 = d2 + ws.D()[i] * ws.pr()[i] * ws.pr()[i]; } }
       }
+#pragma unroll 1
       for (int ls = 0; ls < n_ls && !frozen; ++ls) {
         S an = (ls == 0) ? S(1.0) : a - d1a / d2;
         if (ls > 0 && val(an) == val(a)) break;      // no representable progress: the root of phi' is reached
@@ -479,6 +522,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
         if (!inside) an = hi_inf ? S(2.0) * (val(a) > 1 ? a : S(1.0)) : S(0.5) * (lo + hi);
         a = an;
         d1a = dMxa + a * dMd; d2 = dMd;
+#pragma unroll 1
         for (int i = 0; i < nr; ++i) {
           S si = ws.s()[i] + a * ws.pr()[i];
           if (val(si) < 0) { d1a = d1a + ws.D()[i] * ws.pr()[i] * si; d2 = d2 + ws.D()[i] * ws.pr()[i] * ws.pr()[i]; }
@@ -487,6 +531,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
       }
       alpha = a;
     }
+#pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) ws.x()[j] = ws.x()[j] + alpha * ws.dl()[j];
     gr.sync();
     if (same) { conv = true; break; }
@@ -499,17 +544,26 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
 template <class WS, class R, int G, class IN>
 DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, bool& conv, const Grp<G>& gr) {
   const int nv = m.nv;
+  DMX_T0;
   kinematics<WS, R, G, IN, false>(m, in, ws, gr);
+  DMX_TICK(gr, 0);
   dynamics<WS, R, G, IN>(m, in, ws, gr);
+  DMX_TICK(gr, 1);
+#pragma unroll 1
   for (int e = gr.lane; e < nv * nv; e += G) ws.Hc()[e] = ws.M()[e];
+#pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) ws.a0()[j] = ws.tau()[j] - ws.c()[j];
   gr.sync();
   conv = true;
   if (!cholesky(ws.Hc(), nv, gr)) return -1;
   chol_solve(ws.Hc(), nv, ws.a0(), gr);
+  DMX_TICK(gr, 2);
   int nr = build_rows<WS, R, G, IN>(m, in, ws, cfd, gr);
+  DMX_TICK(gr, 3);
   conv = newton<WS, G>(nv, nr, m.newton_iters, m.ls_iters, ws, gr);
+  DMX_TICK(gr, 4);
   bool fin = true;
+#pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) if (!isfinite(val(ws.x()[j]))) fin = false;
   if (!gr.all(fin)) return -1;
   return nr;
@@ -520,17 +574,21 @@ DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool c
 template <class WS, int G>
 DMX_DN bool vjp_prepare(int nv, int nr, const WS& ws, const Grp<G>& gr) {
   typedef typename WS::S S;
+#pragma unroll 1
   for (int i = gr.lane; i < nr; i += G) {
     S t(0.0);
+#pragma unroll 1
     for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.x()[j];
     t = t - ws.aref()[i];
     ws.s()[i] = t;
     ws.active()[i] = val(t) < 0 ? 1 : 0;
   }
   gr.sync();
+#pragma unroll 1
   for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
     int a, b; tri_index(e, a, b);
     S t = ws.M()[a * nv + b];
+#pragma unroll 1
     for (int i = 0; i < nr; ++i) if (ws.active()[i]) t = t + ws.D()[i] * ws.J()[i * nv + a] * ws.J()[i * nv + b];
     ws.Hc()[a * nv + b] = t;
   }
@@ -540,81 +598,222 @@ DMX_DN bool vjp_prepare(int nv, int nr, const WS& ws, const Grp<G>& gr) {
   return true;
 }
 
-// ---- S11/S12, tangent part: one lane, one direction ----------------------------------------------
-// Directional derivative of  w^T g(z; x*)  with
-//   g = ID(q,v,x*) - tau(q,v,u) + sum_{i in A} J_i^T D_i (J_i x* - aref_i)      (stationarity of Eq. 2)
-// along the direction carried by `in`; x*, A, w and the row inclusion decisions are those of the
-// cooperative pass.  Uses the virtual-work identity  w^T ID = sum_b vel_w(com_b).F_b + omega_w(b).N_b
-// and, for the rows,  J_i y = dir_i . relvel_y(pos_i)  with y in {x*, v, w}.
-// dws: this lane's tangent workspace (frames only).
-template <class R, class IN, class DWS, int ST>
-DMX_DN R residual_tangent(const ModelDev<R>& m, const IN& in, const DWS& dws, const Arr<R, ST>& w,
-                          const Arr<int, ST>& incl, const Arr<int, ST>& rowstart, const Arr<int, ST>& active, bool cfd) {
+// ---- S11/S12: derivative of  S = w^T g(z; x*),  g = ID(q,v,x*) - tau(q,v,u) + sum_{i in A} J_i^T D_i (J_i x* - aref_i)
+// (stationarity of Eq. 2 at the final active set A; x*, A and w = H^-1 kappa are constants).  The VJP of the
+// vector field is minus the gradient of S.  With the virtual-work identity
+//   w^T ID = sum_b velw(com_b).F_b + omegaw(b).N_b            (velw, omegaw: body velocities under joint rates w)
+// and  J_i y = dir_i . relvel_y(pos_i)  for y in {x*, v, w}, the gradient splits into
+//   u : closed form;   v : one reverse sweep over the tree (geometry fixed) + closed-form row / damping terms;
+//   q : one tangent pass per dof over the subtree below that dof;   p : tangent passes without kinematics.
+
+// velocity part, cooperative: vbar = -dS/dv.  Needs in ws: frames (any acceleration), tw, Iw, J, D, cbd, active,
+// w in ws.kap.  Uses ws.Fb/ws.Nb for velw/omegaw, ws.Isub for the body adjoints, ws.pr for J_i w.
+template <class WS, class R, int G, class IN, class AOUT>
+DMX_D void vjp_velocity(const ModelDev<R>& m, const IN& in, const WS& ws, int nr, const AOUT& vbar, const Grp<G>& gr) {
+  typedef typename WS::S S;
+  const int nv = m.nv, nb = m.nbody;
+  // seeds: cotangents of (omega_b, alpha_b, ap_b) from F_b = m (ac_b - g), N_b = I alpha + omega x I omega
+#pragma unroll 1
+  for (int b = 1 + gr.lane; b < nb; b += G) {
+    S z(0.0);
+    V3<S> vw = mk3<S>(z, z, z), ow = vw, comb = ld3(ws.com(), b);
+#pragma unroll 1
+    for (int e = m.tw_ptr[b]; e < m.tw_ptr[b + 1]; ++e) {
+      int j = m.tw_dof[e];
+      S wj = ws.kap()[j];
+      vw = vw + ld3(ws.tw(), e) * wj;
+      if (m.dof_rot[j]) ow = ow + ld3(ws.dax(), j) * wj;
+    }
+    st3(ws.Fb(), b, vw); st3(ws.Nb(), b, ow);
+    V3<S> om = ld3(ws.fw(), b), rc = comb - ld3(ws.fp(), b);
+    M3<S> I = ld9(ws.Iw(), b);
+    V3<S> acb = vw * in.p(b);
+    V3<S> alb = cross(rc, acb) + I * ow;
+    V3<S> omb = cross(cross(om, rc), acb) + cross(rc, cross(acb, om)) + cross(I * om, ow) + I * cross(ow, om);
+    st3(ws.Isub(), 3 * b, omb); st3(ws.Isub(), 3 * b + 1, alb); st3(ws.Isub(), 3 * b + 2, acb);
+  }
+#pragma unroll 1
+  for (int i = gr.lane; i < nr; i += G) {
+    S t(0.0);
+    if (ws.active()[i]) for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.kap()[j];
+    ws.pr()[i] = t;
+  }
+  gr.sync();
+  // leaves to root: every body gathers its children's cotangents through their joints
+#pragma unroll 1
+  for (int lv = m.nlevel - 1; lv >= 0; --lv) {
+#pragma unroll 1
+    for (int i = m.level_ptr[lv] + gr.lane; i < m.level_ptr[lv + 1]; i += G) {
+      int b = m.level_body[i];
+      V3<S> omb = ld3(ws.Isub(), 3 * b), alb = ld3(ws.Isub(), 3 * b + 1), apb = ld3(ws.Isub(), 3 * b + 2);
+      V3<S> wp = ld3(ws.fw(), b), pp = ld3(ws.fp(), b);
+#pragma unroll 1
+      for (int t = m.child_ptr[b]; t < m.child_ptr[b + 1]; ++t) {
+        int c = m.child_idx[t], j = m.body_jnt[c];
+        V3<S> oc = ld3(ws.Isub(), 3 * c), ac = ld3(ws.Isub(), 3 * c + 1), pc = ld3(ws.Isub(), 3 * c + 2);
+        V3<S> E = ld3(ws.fp(), c) - pp;
+        if (j >= 0 && m.jnt_type[j] == JNT_HINGE) {
+          int va = m.jnt_vadr[j];
+          V3<S> ax = ld3(ws.dax(), va), o = ld3(ws.dan(), va), wc = ld3(ws.fw(), c);
+          V3<S> d = ld3(ws.fp(), c) - o;
+          ac = ac + cross(d, pc);
+          oc = oc + cross(cross(wc, d), pc) + cross(d, cross(pc, wc));
+          E = o - pp;
+          omb = omb + cross(ax, ac) * in.v(va);
+        } else if (j >= 0 && m.jnt_type[j] == JNT_SLIDE) {
+          int va = m.jnt_vadr[j];
+          omb = omb + cross(ld3(ws.dax(), va), pc) * (S(2.0) * in.v(va));
+        }
+        omb = omb + oc + cross(cross(wp, E), pc) + cross(E, cross(pc, wp));
+        alb = alb + ac + cross(E, pc);
+        apb = apb + pc;
+      }
+      st3(ws.Isub(), 3 * b, omb); st3(ws.Isub(), 3 * b + 1, alb); st3(ws.Isub(), 3 * b + 2, apb);
+    }
+    gr.sync();
+  }
+  // joint rates: Coriolis part through each body's own joint, damping / PD and the rows' -b J v term
+#pragma unroll 1
+  for (int j = gr.lane; j < nv; j += G) {
+    int jn = m.dof_jnt[j], b = m.dof_body[j], jt = m.jnt_type[jn], par = m.body_parent[b];
+    V3<S> omb = ld3(ws.Isub(), 3 * b), alb = ld3(ws.Isub(), 3 * b + 1), apb = ld3(ws.Isub(), 3 * b + 2);
+    V3<S> ax = ld3(ws.dax(), j), wp = ld3(ws.fw(), par);
+    S g(0.0);
+    if (jt == JNT_HINGE) {
+      V3<S> d = ld3(ws.fp(), b) - ld3(ws.dan(), j), wc = ld3(ws.fw(), b);
+      V3<S> a2 = alb + cross(d, apb);
+      V3<S> o2 = omb + cross(cross(wc, d), apb) + cross(d, cross(apb, wc));
+      g = dot(o2, ax) + dot(a2, cross(wp, ax));
+    } else if (jt == JNT_SLIDE) g = S(2.0) * dot(cross(wp, ax), apb);
+    else if (m.dof_rot[j]) g = dot(omb, ax);
+    S kd(m.jnt_damping[jn]);
+#pragma unroll 1
+    for (int i = 0; i < m.nu; ++i) if (m.act_type[i] == ACT_PD && m.jnt_vadr[m.act_jnt[i]] == j) kd = kd + S(m.act_kd[i]);
+    g = g + ws.kap()[j] * kd;
+#pragma unroll 1
+    for (int i = 0; i < nr; ++i) if (ws.active()[i]) g = g + ws.pr()[i] * ws.D()[i] * ws.cbd()[ws.rowcand()[i] >> 2] * ws.J()[i * nv + j];
+    vbar[j] = -(double)g;
+  }
+  gr.sync();
+}
+
+// copy body b's frame and the axes / anchors of its ancestor dofs from the cooperative workspace (values at
+// acceleration x*) into a lane's tangent workspace, with zero tangent
+template <class R, class WS, class DWS>
+DMX_DI void lift_body(const ModelDev<R>& m, const WS& ws, const DWS& dws, int b) {
+  typedef Dual<R> S;
+#pragma unroll 1
+  for (int k = 0; k < 3; ++k) {
+    dws.fp()[3 * b + k] = S(ws.fp()[3 * b + k]); dws.fw()[3 * b + k] = S(ws.fw()[3 * b + k]); dws.fal()[3 * b + k] = S(ws.fal()[3 * b + k]);
+    dws.fvp()[3 * b + k] = S(ws.fvp()[3 * b + k]); dws.fap()[3 * b + k] = S(ws.fap()[3 * b + k]); dws.com()[3 * b + k] = S(ws.com()[3 * b + k]);
+  }
+#pragma unroll 1
+  for (int k = 0; k < 9; ++k) dws.fR()[9 * b + k] = S(ws.fR()[9 * b + k]);
+#pragma unroll 1
+  for (int e = m.tw_ptr[b]; e < m.tw_ptr[b + 1]; ++e) {
+    int j = m.tw_dof[e];
+#pragma unroll 1
+    for (int k = 0; k < 3; ++k) { dws.dax()[3 * j + k] = S(ws.dax()[3 * j + k]); dws.dan()[3 * j + k] = S(ws.dan()[3 * j + k]); }
+  }
+}
+// velw(com_b).F_b + omegaw(b).N_b in the tangent workspace
+template <class R, class IN, class DWS, class AW>
+DMX_DI Dual<R> body_term(const ModelDev<R>& m, const IN& in, const DWS& dws, const AW& w, int b) {
+  typedef Dual<R> S;
+  V3<S> Fb, Nb; M3<S> Iw;
+  body_wrench<DWS, R, IN>(m, in, dws, b, Fb, Nb, Iw);
+  V3<S> comb = ld3(dws.com(), b);
+  S z(R(0));
+  V3<S> vw = mk3<S>(z, z, z), ow = vw;
+#pragma unroll 1
+  for (int e = m.tw_ptr[b]; e < m.tw_ptr[b + 1]; ++e) {
+    int j = m.tw_dof[e], rot = m.dof_rot[j];
+    S wj(w[j]);
+    vw = vw + twist_lin(dws, j, rot, comb) * wj;
+    if (rot) ow = ow + ld3(dws.dax(), j) * wj;
+  }
+  return dot(vw, Fb) + dot(ow, Nb);
+}
+// sum over the active rows of candidate c of (J_i w) D_i (J_i x* - aref_i) in the tangent workspace
+template <class R, class IN, class DWS, class AW, class AI>
+DMX_DI Dual<R> contact_term(const ModelDev<R>& m, const IN& in, const DWS& dws, const AW& w, int c, int n, int r0, const AI& active, bool cfd) {
   typedef Dual<R> S;
   const int nv = m.nv;
-  Grp<1> g1; g1.lane = 0; g1.mask = 0;
-  kinematics<DWS, R, 1, IN, true>(m, in, dws, g1);
-  S acc(R(0));
-  for (int b = 1; b < m.nbody; ++b) {
-    V3<S> Fb, Nb; M3<S> Iw;
-    body_wrench<DWS, R, IN>(m, in, dws, b, Fb, Nb, Iw);
-    V3<S> comb = ld3(dws.com(), b);
-    S z(R(0));
-    V3<S> vw = mk3<S>(z, z, z), ow = vw;
-    for (int e = m.tw_ptr[b]; e < m.tw_ptr[b + 1]; ++e) {
-      int j = m.tw_dof[e], rot = m.dof_rot[j];
-      S wj(w[j]);
-      vw = vw + twist_lin(dws, j, rot, comb) * wj;
-      if (rot) ow = ow + ld3(dws.dax(), j) * wj;
-    }
-    acc = acc + dot(vw, Fb) + dot(ow, Nb);
-  }
+  GeoT<S> g = collide<DWS, R>(m, dws, c);
+  S Dw, post, bd, mu;
+  candidate_terms<S, R, IN>(m, in, c, g.r, cfd, Dw, post, bd, mu);
+  S z(R(0));
+  S nX = z, t1X = z, t2X = z, nV = z, t1V = z, t2V = z, nW = z, t1W = z, t2W = z;
+  int b1 = m.ct_b1[c], b2 = m.ct_b2[c];
+#pragma unroll 1
   for (int j = 0; j < nv; ++j) {
-    S tau = -(S(m.jnt_damping[m.dof_jnt[j]]) * in.v(j));
-    for (int i = 0; i < m.nu; ++i) {
-      int jn = m.act_jnt[i];
-      if (m.jnt_vadr[jn] != j) continue;
-      if (m.act_type[i] == ACT_MOTOR) tau = tau + S(m.act_gear[i]) * in.u(i);
-      else tau = tau + S(m.act_kp[i]) * (in.u(i) - in.q(m.jnt_qadr[jn])) - S(m.act_kd[i]) * in.v(j);
+    if (m.tw_idx[b2 * nv + j] < 0 && m.tw_idx[b1 * nv + j] < 0) continue;
+    V3<S> d = rel_twist<DWS, R>(m, dws, j, b1, b2, g.pos);
+    S nd = dot(g.n, d);
+    S xj = in.a(j), vj = in.v(j), wj(w[j]);
+    nX = nX + nd * xj; nV = nV + nd * vj; nW = nW + nd * wj;
+    if (n == 4) {
+      S t1d = dot(g.t1, d), t2d = dot(g.t2, d);
+      t1X = t1X + t1d * xj; t1V = t1V + t1d * vj; t1W = t1W + t1d * wj;
+      t2X = t2X + t2d * xj; t2V = t2V + t2d * vj; t2W = t2W + t2d * wj;
     }
-    acc = acc + S(w[j]) * (S(m.jnt_armature[m.dof_jnt[j]]) * in.a(j) - tau);
   }
+  S acc = z;
+#pragma unroll 1
+  for (int e = 0; e < n; ++e) {
+    if (!active[r0 + e]) continue;
+    S JX = nX, JV = nV, JW = nW;
+    if (n == 4) {
+      S sg = (e & 1) ? -mu : mu;
+      if (e < 2) { JX = JX + sg * t1X; JV = JV + sg * t1V; JW = JW + sg * t1W; }
+      else { JX = JX + sg * t2X; JV = JV + sg * t2V; JW = JW + sg * t2W; }
+    }
+    acc = acc + JW * (Dw * (JX - (post - bd * JV)));
+  }
+  return acc;
+}
+
+// one lane, one direction: dS/d(direction) for a configuration dof (in.kind 0, dof d) or a parameter (in.kind 3).
+// ws: cooperative workspace holding the frames at acceleration x*; dws: this lane's tangent workspace.
+// Configuration dof: tangent kinematics over the subtree below the dof, wrenches of those bodies, rows touching
+// them.  Body mass: that body's wrench only.  Pair parameter: that pair's rows only.  (One code path, so that
+// the body / row terms are emitted once.)
+template <class R, class IN, class WS, class DWS>
+DMX_D R residual_tangent(const ModelDev<R>& m, const IN& in, const WS& ws, const DWS& dws, int d, bool cfd) {
+  typedef Dual<R> S;
+  const int nv = m.nv;
+  S acc(R(0));
+  int b0 = -1, bm = -1, pr = -1, t0 = 0, t1 = 0;
+  if (in.kind == 0) { b0 = m.dof_body[d]; bm = m.body_parent[b0]; t0 = m.sub_ptr[b0]; t1 = m.sub_ptr[b0 + 1]; }
+  else if (in.idx < m.nbody) { bm = in.idx; t1 = bm > 0 ? 1 : 0; }
+  else pr = in.idx < m.p_solref ? in.idx - m.p_fric : (in.idx < m.p_solimp ? (in.idx - m.p_solref) / 2 : (in.idx - m.p_solimp) / 5);
+  if (bm >= 0) lift_body<R>(m, ws, dws, bm);
+#pragma unroll 1
+  for (int t = t0; t < t1; ++t) {
+    int b = b0 >= 0 ? m.sub_body[t] : bm;
+    if (b0 >= 0) body_kin<DWS, R, IN, true>(m, in, dws, b);
+    acc = acc + body_term<R>(m, in, dws, ws.kap(), b);
+  }
+  if (b0 >= 0) {
+    int jn = m.dof_jnt[d];
+    if (m.jnt_type[jn] != JNT_FREE)
+      for (int i = 0; i < m.nu; ++i) if (m.act_type[i] == ACT_PD && m.act_jnt[i] == jn) acc = acc - S(ws.kap()[d]) * (S(m.act_kp[i]) * (in.u(i) - in.q(m.jnt_qadr[jn])));
+  }
+  if (bm > 0 && b0 < 0) return acc.d;
+#pragma unroll 1
   for (int c = 0; c < m.nc; ++c) {
-    int n = incl[c];
+    int n = ws.incl()[c];
     if (n == 0) continue;
-    int r0 = rowstart[c];
-    bool any = false;
-    for (int e = 0; e < n; ++e) any = any || active[r0 + e];
-    if (!any) continue;
-    GeoT<S> g = collide<DWS, R>(m, dws, c);
-    S Dw, post, bd, mu;
-    candidate_terms<S, R, IN>(m, in, c, g.r, cfd, Dw, post, bd, mu);
-    S z(R(0));
-    S nX = z, t1X = z, t2X = z, nV = z, t1V = z, t2V = z, nW = z, t1W = z, t2W = z;
     int b1 = m.ct_b1[c], b2 = m.ct_b2[c];
-    for (int j = 0; j < nv; ++j) {
-      if (m.tw_idx[b2 * nv + j] < 0 && m.tw_idx[b1 * nv + j] < 0) continue;
-      V3<S> d = rel_twist<DWS, R>(m, dws, j, b1, b2, g.pos);
-      S nd = dot(g.n, d);
-      S xj = in.a(j), vj = in.v(j), wj(w[j]);
-      nX = nX + nd * xj; nV = nV + nd * vj; nW = nW + nd * wj;
-      if (n == 4) {
-        S t1d = dot(g.t1, d), t2d = dot(g.t2, d);
-        t1X = t1X + t1d * xj; t1V = t1V + t1d * vj; t1W = t1W + t1d * wj;
-        t2X = t2X + t2d * xj; t2V = t2V + t2d * vj; t2W = t2W + t2d * wj;
-      }
-    }
-    for (int e = 0; e < n; ++e) {
-      if (!active[r0 + e]) continue;
-      S JX = nX, JV = nV, JW = nW;
-      if (n == 4) {
-        S sg = (e & 1) ? -mu : mu;
-        if (e < 2) { JX = JX + sg * t1X; JV = JV + sg * t1V; JW = JW + sg * t1W; }
-        else { JX = JX + sg * t2X; JV = JV + sg * t2V; JW = JW + sg * t2W; }
-      }
-      S s = JX - (post - bd * JV);
-      acc = acc + JW * (Dw * s);
-    }
+    bool in1 = b0 >= 0 && m.tw_idx[b1 * nv + d] >= 0, in2 = b0 >= 0 && m.tw_idx[b2 * nv + d] >= 0;
+    if (b0 >= 0 ? !(in1 || in2) : m.ct_pair[c] != pr) continue;
+    int r0 = ws.rowstart()[c];
+    bool any = false;
+    for (int e = 0; e < n; ++e) any = any || ws.active()[r0 + e];
+    if (!any) continue;
+#pragma unroll 1
+    for (int k = 0; k < 2; ++k) if (!(k ? in2 : in1)) lift_body<R>(m, ws, dws, k ? b2 : b1);
+    acc = acc + contact_term<R>(m, in, dws, ws.kap(), c, n, r0, ws.active(), cfd);
   }
   return acc.d;
 }

@@ -30,14 +30,22 @@ template <class R, int G> cudaError_t launch_invweight(const ModelDev<R>& m, con
   invweight_kernel<R, G><<<1, c.block, c.smem, s>>>(m, qpos0, zero_v, body_w, wl, rl);
   return cudaGetLastError();
 }
-template <class R, int G> cudaError_t kernel_occupancy(int block, size_t smem_fwd, size_t smem_bwd, int* occ_fwd, int* occ_bwd) {
+template <class R, int G> cudaError_t launch_prof_dump(unsigned long long* out, cudaStream_t s) {
+  prof_dump_kernel<R, G><<<1, 32, 0, s>>>(out);
+  return cudaGetLastError();
+}
+template <class R, int G> cudaError_t kernel_occupancy(int block, size_t smem_fwd, size_t smem_bwd, size_t smem_field, int* occ_fwd, int* occ_bwd, int* occ_field) {
   cudaError_t e = cudaFuncSetAttribute(rollout_kernel<R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_fwd);
   if (e != cudaSuccess) return e;
   e = cudaFuncSetAttribute(backward_kernel<R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bwd);
   if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(field_kernel<R, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_field);
+  if (e != cudaSuccess) return e;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_fwd, rollout_kernel<R, G>, block, smem_fwd);
   if (e != cudaSuccess) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_bwd, backward_kernel<R, G>, block, smem_bwd);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_bwd, backward_kernel<R, G>, block, smem_bwd);
+  if (e != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(occ_field, field_kernel<R, G>, block, smem_field);
 }
 
 }  // namespace dmx
@@ -48,4 +56,5 @@ template <class R, int G> cudaError_t kernel_occupancy(int block, size_t smem_fw
   template cudaError_t dmx::launch_field<R, G>(const dmx::ModelDev<R>&, const dmx::FieldArgs<R>&, dmx::LaunchCfg, cudaStream_t);       \
   template cudaError_t dmx::launch_invweight<R, G>(const dmx::ModelDev<R>&, const R*, const R*, R*, const dmx::WsLayout&,             \
                                                    const dmx::RkLayout&, dmx::LaunchCfg, cudaStream_t);                             \
-  template cudaError_t dmx::kernel_occupancy<R, G>(int, size_t, size_t, int*, int*);
+  template cudaError_t dmx::launch_prof_dump<R, G>(unsigned long long*, cudaStream_t);                                              \
+  template cudaError_t dmx::kernel_occupancy<R, G>(int, size_t, size_t, size_t, int*, int*, int*);

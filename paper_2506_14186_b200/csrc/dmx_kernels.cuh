@@ -11,32 +11,46 @@ namespace dmx {
 template <class R, int G>
 DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yqr, const Arr<R, StrideOf<G>::value>& Vr, const R* u, const R* p,
                       const Arr<double, StrideOf<G>::value>& kappa, bool cfd, bool want_p, const Ws<R, StrideOf<G>::value>& ws,
-                      const Ws<Dual<R>, 32>& dws, const Rk<StrideOf<G>::value>& rk, const Grp<G>& gr) {
+                      const Ws<Dual<R>, 32>& dws, const Rk<StrideOf<G>::value>& rk, const Grp<G>& gr, int dbg = 0) {
   const int ST = StrideOf<G>::value;
   const int nv = m.nv;
+  if (dbg & 4) return true;
+  DMX_T0;
   InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
-  bool conv;
-  int nr = vector_field<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, cfd, conv, gr);
+  int conv;
+  int nr = field_eval<R, G>(u, p, cfd ? 1 : 0, &conv);
   if (nr < 0) return false;
+  DMX_TICK(gr, 8);
+#pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) ws.kap()[j] = (R)kappa[j];
   gr.sync();
   if (!vjp_prepare<Ws<R, ST>, G>(nv, nr, ws, gr)) return false;
-  const int ndir = 2 * nv + m.nu + (want_p ? m.np : 0);
+  DMX_TICK(gr, 9);
+  // u: closed form; v: reverse sweep over the tree; then the frames at acceleration x* for the tangent passes
+#pragma unroll 1
+  for (int i = gr.lane; i < m.nu; i += G)
+    rk.ubar()[i] = (double)(ws.kap()[m.jnt_vadr[m.act_jnt[i]]] * (m.act_type[i] == ACT_MOTOR ? m.act_gear[i] : m.act_kp[i]));
+  if (!(dbg & 2)) vjp_velocity<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, nr, rk.vbar(), gr);
+  DMX_TICK(gr, 10);
+  in.aa = ws.x();
+  kinematics<Ws<R, ST>, R, G, InPlain<R, ST>, true>(m, in, ws, gr);
+  DMX_TICK(gr, 11);
+  const int ndir = (dbg & 1) ? 0 : nv + (want_p ? m.np : 0);
+#pragma unroll 1
   for (int d = gr.lane; d < ndir; d += G) {
     InDual<R, ST> din; din.qa = Yqr; din.va = Vr; din.aa = ws.x(); din.ua = u; din.pa = p;
-    seed_direction<R, ST>(m, din, d);
-    double s = -(double)residual_tangent<R, InDual<R, ST>, Ws<Dual<R>, 32>, ST>(m, din, dws, ws.kap(), ws.incl(), ws.rowstart(), ws.active(), cfd);
-    if (d < nv) rk.qbar()[d] = s;
-    else if (d < 2 * nv) rk.vbar()[d - nv] = s;
-    else if (d < 2 * nv + m.nu) rk.ubar()[d - 2 * nv] = s;
-    else rk.pbar()[d - 2 * nv - m.nu] = s;
+    if (d < nv) seed_direction<R, ST>(m, din, d);
+    else { din.kind = 3; din.idx = d - nv; din.dq0 = din.dq1 = din.dq2 = din.dq3 = R(0); }
+    double s = -(double)residual_tangent<R, InDual<R, ST>, Ws<R, ST>, Ws<Dual<R>, 32> >(m, din, ws, dws, d, cfd);
+    if (d < nv) rk.qbar()[d] = s; else rk.pbar()[d - nv] = s;
   }
   gr.sync();
+  DMX_TICK(gr, 12);
   return true;
 }
 
 template <class R> struct BackwardArgs {
-  int nenv, nknot, want_p, cfd, tape_cap;
+  int nenv, nknot, want_p, cfd, tape_cap, dbg;
   const R *ctrl, *params, *zero_u, *xT, *dLdxT;
   const int* status;
   SolverOpts so;
@@ -44,6 +58,7 @@ template <class R> struct BackwardArgs {
   const int* tape_hdr; const R* tape;
   int* queue;
   Dual<R>* scratch; int res_size;
+  double* rk_scratch;       // integrator / adjoint arrays of every resident group (global memory: touched once per stage)
   WsLayout wl, rwl; RkLayout rl;
 };
 
@@ -58,18 +73,21 @@ DMX_DI Ws<Dual<R>, 32> bind_scratch(Dual<R>* scratch, int res_size, const WsLayo
 // ---- S10: reverse sweep over the tape, frozen step sizes ---------------------------
 template <class R, int G>
 __global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ BackwardArgs<R> a) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  __shared__ CtaConst<R> cc;
-  load_cta_const<R>(cc, m_, a.wl, a.rwl, a.rl);
+  unsigned char* smem = dyn_smem;
+  CtaConst<R>& cc = cta_const<R>();
+  load_cta_const<R>(cc, m_, a.wl, a.rwl, a.rl, 0);
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
   Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
-  bind_shared<R, G>(smem, a.rl.size_bwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
+  bind_shared<R, G>(smem, 0, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
+  if (G == 1) rk.b = a.rk_scratch + ((size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32 * (size_t)a.rl.size_bwd + (threadIdx.x & 31);
+  else rk.b = a.rk_scratch + ((size_t)blockIdx.x * (blockDim.x / G) + threadIdx.x / G) * (size_t)a.rl.size_bwd;
   Ws<Dual<R>, 32> dws = bind_scratch<R>(a.scratch, a.res_size, &cc.rwl);
   const int nq = m.nq, nv = m.nv, nu = m.nu, np = m.np, nx = nq + nv, tab = a.so.tableau, rec = nx + 2;
   const bool has_ctrl = a.ctrl != nullptr && a.nknot > 0 && nu > 0;
   const int nknot = has_ctrl ? a.nknot : 0;
+#pragma unroll 1
   for (;;) {
     int e = 0;
     if (gr.lane == 0) e = atomicAdd(a.queue, 1);
@@ -82,6 +100,7 @@ __global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ M
     if (good) {
       // ambient gradient at x_T -> tangent cotangent: lam = E(q_T)^T g
       const R* xT = a.xT + (size_t)e * nx; const R* gT = a.dLdxT + (size_t)e * nx;
+#pragma unroll 1
       for (int d = gr.lane; d < nv; d += G) {
         int j = m.dof_jnt[d], c = d - m.jnt_vadr[j], qa = m.jnt_qadr[j];
         double s;
@@ -94,12 +113,16 @@ __global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ M
         }
         rk.lam()[d] = s; rk.lam()[nv + d] = (double)gT[nq + d];
       }
+#pragma unroll 1
       for (int i = gr.lane; i < np; i += G) rk.gp()[i] = 0.0;
       gr.sync();
     }
+#pragma unroll 1
     for (int n = N - 1; n >= 0 && good; --n) {
       const R* r = a.tape + ((size_t)e * a.tape_cap + n) * rec;
+#pragma unroll 1
       for (int j = gr.lane; j < nq; j += G) rk.q()[j] = (double)r[j];
+#pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) rk.v()[j] = (double)r[nq + j];
       double hs = (double)r[nx + 1], h = fabs(hs);
       if (hs < 0) knot--;
@@ -108,41 +131,56 @@ __global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ M
       bool ok; int unc;
       rk_attempt<R, G, true>(m, tab, rk, Yqr, Vr, u, p, h, false, ws, ok, unc, gr);   // recompute the stages with F
       // y_{n+1} = (q_n (+) h sum b_i K_i, v_n + h sum b_i A_i), b = row 6 of a
+#pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) {
         double s = 0; for (int i = 0; i < 6; ++i) s += TAB_A[tab][6][i] * rk.K()[i * nv + j];
         rk.delta()[j] = h * s; rk.dbar()[j] = 0; rk.qb()[j] = 0; rk.vb()[j] = rk.lam()[nv + j];
       }
       gr.sync();
+#pragma unroll 1
       for (int jn = gr.lane; jn < m.njnt; jn += G) retract_pullback_joint(m, jn, rk.delta(), rk.lam(), rk.qb(), rk.dbar());
       gr.sync();
+#pragma unroll 1
       for (int j = gr.lane; j < nv; j += G)
+#pragma unroll 1
         for (int i = 0; i < 6; ++i) { rk.Kb()[i * nv + j] = h * TAB_A[tab][6][i] * rk.dbar()[j]; rk.Ab()[i * nv + j] = h * TAB_A[tab][6][i] * rk.lam()[nv + j]; }
       gr.sync();
+#pragma unroll 1
       for (int i = 5; i >= 0 && good; --i) {
+#pragma unroll 1
         for (int j = gr.lane; j < nv; j += G) { rk.Vb()[j] = 0; rk.dbar()[j] = 0; }
         gr.sync();
+#pragma unroll 1
         for (int jn = gr.lane; jn < m.njnt; jn += G) chart_pullback_joint(m, jn, rk.sDl().at(i * nv), rk.sV().at(i * nv), rk.Kb().at(i * nv), rk.Vb(), rk.dbar());
+#pragma unroll 1
         for (int j = gr.lane; j < nq; j += G) Yqr[j] = (R)rk.sYq()[i * nq + j];
+#pragma unroll 1
         for (int j = gr.lane; j < nv; j += G) Vr[j] = (R)rk.sV()[i * nv + j];
         gr.sync();
         // A_i = F(Y_i), or F~ for the straight-through estimator (Eq. 4)
-        if (!vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.Ab().at(i * nv), a.cfd != 0, a.want_p != 0, ws, dws, rk, gr)) { good = false; break; }
+        if (!vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.Ab().at(i * nv), a.cfd != 0, a.want_p != 0, ws, dws, rk, gr, a.dbg)) { good = false; break; }
+#pragma unroll 1
         for (int j = gr.lane; j < nv; j += G) rk.Vb()[j] += rk.vbar()[j];
         if (a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nu; c += G) a.dLdctrl[((size_t)e * nknot + knot) * nu + c] += (R)rk.ubar()[c];
         if (a.want_p) for (int c = gr.lane; c < np; c += G) rk.gp()[c] += rk.pbar()[c];
         gr.sync();
+#pragma unroll 1
         for (int jn = gr.lane; jn < m.njnt; jn += G) retract_pullback_joint(m, jn, rk.sDl().at(i * nv), rk.qbar(), rk.qb(), rk.dbar());
         gr.sync();
+#pragma unroll 1
         for (int j = gr.lane; j < nv; j += G) {
           rk.vb()[j] += rk.Vb()[j];
+#pragma unroll 1
           for (int l = 0; l < i; ++l) { rk.Kb()[l * nv + j] += h * TAB_A[tab][i][l] * rk.dbar()[j]; rk.Ab()[l * nv + j] += h * TAB_A[tab][i][l] * rk.Vb()[j]; }
         }
         gr.sync();
       }
+#pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) { rk.lam()[j] = rk.qb()[j]; rk.lam()[nv + j] = rk.vb()[j]; }
       gr.sync();
     }
     R* g0 = a.dLdx0 + (size_t)e * 2 * nv;
+#pragma unroll 1
     for (int j = gr.lane; j < 2 * nv; j += G) g0[j] = good ? (R)rk.lam()[j] : R(0);
     if (a.dLdparams) for (int c = gr.lane; c < np; c += G) a.dLdparams[(size_t)e * np + c] = good ? (R)rk.gp()[c] : R(0);
     if (!good && a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nknot * nu; c += G) a.dLdctrl[(size_t)e * nknot * nu + c] = R(0);
@@ -160,9 +198,9 @@ template <class R> struct FieldArgs {
 };
 template <class R, int G>
 __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ FieldArgs<R> a) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  __shared__ CtaConst<R> cc;
-  load_cta_const<R>(cc, m_, a.wl, a.rwl, a.rl);
+  unsigned char* smem = dyn_smem;
+  CtaConst<R>& cc = cta_const<R>();
+  load_cta_const<R>(cc, m_, a.wl, a.rwl, a.rl, a.rl.size_bwd);
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
@@ -170,26 +208,32 @@ __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ Mode
   bind_shared<R, G>(smem, a.rl.size_bwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
   const int nq = m.nq, nv = m.nv, nx = nq + nv;
   const int ngr = (gridDim.x * blockDim.x) / G;
+#pragma unroll 1
   for (int e = (blockIdx.x * blockDim.x + threadIdx.x) / G; e < a.n; e += ngr) {
     const R* x = a.x + (size_t)e * nx;
     const R* u = (a.u && m.nu > 0) ? a.u + (size_t)e * m.nu : a.zero_u;
     const R* p = a.params ? a.params + (size_t)e * m.np : m.p_default;
+#pragma unroll 1
     for (int j = gr.lane; j < nq; j += G) Yqr[j] = x[j];
+#pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) Vr[j] = x[nq + j];
     gr.sync();
     if (!a.kappa) {
-      InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
-      bool conv;
-      int nr = vector_field<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, a.cfd != 0, conv, gr);
+      int conv;
+      int nr = field_eval<R, G>(u, p, a.cfd, &conv);
+#pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) a.acc[(size_t)e * nv + j] = nr < 0 ? R(nan("")) : ws.x()[j];
       if (gr.lane == 0 && a.nrow) a.nrow[e] = nr;
     } else {
       Ws<Dual<R>, 32> dws = bind_scratch<R>(a.scratch, a.res_size, &cc.rwl);
+#pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) rk.lam()[j] = (double)a.kappa[(size_t)e * nv + j];
       gr.sync();
       bool ok = vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.lam(), a.cfd != 0, a.want_p != 0, ws, dws, rk, gr);
       R bad = R(nan(""));
+#pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) { a.qbar[(size_t)e * nv + j] = ok ? (R)rk.qbar()[j] : bad; a.vbar[(size_t)e * nv + j] = ok ? (R)rk.vbar()[j] : bad; }
+#pragma unroll 1
       for (int j = gr.lane; j < m.nu; j += G) a.ubar[(size_t)e * m.nu + j] = ok ? (R)rk.ubar()[j] : bad;
       if (a.want_p) for (int j = gr.lane; j < m.np; j += G) a.pbar[(size_t)e * m.np + j] = ok ? (R)rk.pbar()[j] : bad;
     }
@@ -201,9 +245,9 @@ __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ Mode
 template <class R, int G>
 __global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ ModelDev<R> m_, const R* qpos0, const R* zero_v, R* body_w,
                                                         const __grid_constant__ WsLayout wl, const __grid_constant__ RkLayout rl) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  __shared__ CtaConst<R> cc;
-  load_cta_const<R>(cc, m_, wl, wl, rl);
+  unsigned char* smem = dyn_smem;
+  CtaConst<R>& cc = cta_const<R>();
+  load_cta_const<R>(cc, m_, wl, wl, rl, rl.size_bwd);
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
@@ -211,18 +255,24 @@ __global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ 
   bind_shared<R, G>(smem, rl.size_bwd, wl.size + rl.rsize, wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
   if (blockIdx.x != 0 || threadIdx.x >= G) return;
   const int nv = m.nv;
+#pragma unroll 1
   for (int j = gr.lane; j < m.nq; j += G) Yqr[j] = qpos0[j];
+#pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) Vr[j] = R(0);
   gr.sync();
   InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = zero_v; in.pa = m.p_default;
   kinematics<Ws<R, ST>, R, G, InPlain<R, ST>, false>(m, in, ws, gr);
   dynamics<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, gr);
+#pragma unroll 1
   for (int e = gr.lane; e < nv * nv; e += G) ws.Hc()[e] = ws.M()[e];
   gr.sync();
   bool pd = cholesky(ws.Hc(), nv, gr);
+#pragma unroll 1
   for (int b = 0; b < m.nbody; ++b) {
     R tr = R(0);
+#pragma unroll 1
     for (int c = 0; c < 3 && pd && b > 0; ++c) {
+#pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) {
         int e = m.tw_idx[b * nv + j];
         R val_ = R(0);
@@ -231,11 +281,16 @@ __global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ 
       }
       gr.sync();
       chol_solve(ws.Hc(), nv, ws.dl(), gr);
+#pragma unroll 1
       for (int j = 0; j < nv; ++j) tr += ws.g()[j] * ws.dl()[j];
       gr.sync();
     }
     if (gr.lane == 0) body_w[b] = pd ? tr / R(3) : R(nan(""));
   }
+}
+
+template <class R, int G> __global__ void prof_dump_kernel(unsigned long long* out) {
+  if (threadIdx.x < 32) { out[threadIdx.x] = g_prof[threadIdx.x]; g_prof[threadIdx.x] = 0; }
 }
 
 // ---- host launchers (defined per instantiation in dmx_inst.cuh) -----------------------------------------
@@ -246,6 +301,7 @@ template <class R, int G> cudaError_t launch_backward(const ModelDev<R>& m, cons
 template <class R, int G> cudaError_t launch_field(const ModelDev<R>& m, const FieldArgs<R>& a, LaunchCfg c, cudaStream_t s);
 template <class R, int G> cudaError_t launch_invweight(const ModelDev<R>& m, const R* qpos0, const R* zero_v, R* body_w, const WsLayout& wl,
                                                        const RkLayout& rl, LaunchCfg c, cudaStream_t s);
-template <class R, int G> cudaError_t kernel_occupancy(int block, size_t smem_fwd, size_t smem_bwd, int* occ_fwd, int* occ_bwd);
+template <class R, int G> cudaError_t launch_prof_dump(unsigned long long* out, cudaStream_t s);
+template <class R, int G> cudaError_t kernel_occupancy(int block, size_t smem_fwd, size_t smem_bwd, size_t smem_field, int* occ_fwd, int* occ_bwd, int* occ_field);
 
 }  // namespace dmx

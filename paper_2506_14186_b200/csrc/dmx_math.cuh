@@ -22,6 +22,16 @@ namespace dmx {
 #define DMX_DN __device__
 #endif
 
+// ---- optional phase counters (compile with -DDMX_PROF; read back with dmx_debug_counters) ----------
+static __device__ unsigned long long g_prof[32];
+#ifdef DMX_PROF
+#define DMX_T0 long long t0_ = clock64()
+#define DMX_TICK(gr, id) do { long long t1_ = clock64(); if ((gr).lane == 0) atomicAdd(&g_prof[id], (unsigned long long)(t1_ - t0_)); t0_ = clock64(); } while (0)
+#else
+#define DMX_T0 do {} while (0)
+#define DMX_TICK(gr, id) do {} while (0)
+#endif
+
 // ---- tangent scalar: value and one directional derivative -------------------------------
 template <class T> struct Dual {
   T v, d;

@@ -23,6 +23,7 @@ template <class R> struct ModelDev {
   // (body, ancestor-dof) table: entries of body b are tw_ptr[b] .. tw_ptr[b+1]
   const int *tw_ptr, *tw_body, *tw_dof, *tw_idx /* [nbody*nv] entry or -1 */;
   const int *sub_ptr, *sub_body;            // subtree lists (ascending, self included)
+  const int *child_ptr, *child_idx;         // children lists
   const int *mp_i, *mp_j, *mp_deep;         // lower-triangle entries of M; deep = -1: structurally zero
   // flattened candidate contacts
   const int *ct_kind, *ct_b1, *ct_b2, *ct_condim, *ct_pair;

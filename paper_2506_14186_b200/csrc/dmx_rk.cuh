@@ -49,7 +49,9 @@ DMX_DI void retract_joint(const ModelDev<R>& m, int jn, const AD& q, const AD& d
   int qa = m.jnt_qadr[jn], va = m.jnt_vadr[jn];
   if (m.jnt_type[jn] != JNT_FREE) { qout[qa] = q[qa] + delta[va]; K[va] = V[va]; return; }
   double d[3], w[3], e[4], a[4], r[4];
+#pragma unroll 1
   for (int c = 0; c < 3; ++c) { qout[qa + c] = q[qa + c] + delta[va + c]; K[va + c] = V[va + c]; d[c] = delta[va + 3 + c]; w[c] = V[va + 3 + c]; }
+#pragma unroll 1
   for (int c = 0; c < 4; ++c) a[c] = q[qa + 3 + c];
   rotvec_to_quat(d, e);
   r[0] = a[0] * e[0] - a[1] * e[1] - a[2] * e[2] - a[3] * e[3];
@@ -57,9 +59,11 @@ DMX_DI void retract_joint(const ModelDev<R>& m, int jn, const AD& q, const AD& d
   r[2] = a[0] * e[2] - a[1] * e[3] + a[2] * e[0] + a[3] * e[1];
   r[3] = a[0] * e[3] + a[1] * e[2] - a[2] * e[1] + a[3] * e[0];
   double n = sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2] + r[3] * r[3]);
+#pragma unroll 1
   for (int c = 0; c < 4; ++c) qout[qa + 3 + c] = r[c] / n;
   // Theta' = dexp^-1_Theta(w) truncated after the B_2 term: w + 1/2 Theta x w + 1/12 Theta x (Theta x w)
   double t1[3], t2[3]; cross3(d, w, t1); cross3(d, t1, t2);
+#pragma unroll 1
   for (int c = 0; c < 3; ++c) K[va + 3 + c] = w[c] + 0.5 * t1[c] + t2[c] / 12.0;
 }
 DMX_DI void rot_AB(const double* d, double& A, double& B, double& C) {
@@ -76,10 +80,12 @@ DMX_DI void retract_pullback_joint(const ModelDev<R>& m, int jn, const AD& delta
   int va = m.jnt_vadr[jn];
   if (m.jnt_type[jn] != JNT_FREE) { base[va] += Qbar[va]; dbar[va] += Qbar[va]; return; }
   double d[3], qb[3];
+#pragma unroll 1
   for (int c = 0; c < 3; ++c) { base[va + c] += Qbar[va + c]; dbar[va + c] += Qbar[va + c]; d[c] = delta[va + 3 + c]; qb[c] = Qbar[va + 3 + c]; }
   double A, B, C; rot_AB(d, A, B, C);
   // R qb = qb + A d x qb + B d x (d x qb);  Jr^T qb = qb + B d x qb + C d x (d x qb)   (K^T = -K)
   double k1[3], k2[3]; cross3(d, qb, k1); cross3(d, k1, k2);
+#pragma unroll 1
   for (int c = 0; c < 3; ++c) { base[va + 3 + c] += qb[c] + A * k1[c] + B * k2[c]; dbar[va + 3 + c] += qb[c] + B * k1[c] + C * k2[c]; }
 }
 // joint jn of: Vbar += (dK/dV)^T Kbar, dbar += (dK/dTheta)^T Kbar
@@ -88,11 +94,14 @@ DMX_DI void chart_pullback_joint(const ModelDev<R>& m, int jn, const AD& delta, 
   int va = m.jnt_vadr[jn];
   if (m.jnt_type[jn] != JNT_FREE) { Vbar[va] += Kbar[va]; return; }
   double th[3], w[3], kb[3];
+#pragma unroll 1
   for (int c = 0; c < 3; ++c) { Vbar[va + c] += Kbar[va + c]; th[c] = delta[va + 3 + c]; w[c] = V[va + 3 + c]; kb[c] = Kbar[va + 3 + c]; }
   double t1[3], t2[3], tw[3], a[3], b[3], c3v[3];
   cross3(th, kb, t1); cross3(th, t1, t2);
+#pragma unroll 1
   for (int c = 0; c < 3; ++c) Vbar[va + 3 + c] += kb[c] - 0.5 * t1[c] + t2[c] / 12.0;
   cross3(w, kb, a); cross3(th, w, tw); cross3(tw, kb, b); cross3(w, t1, c3v);
+#pragma unroll 1
   for (int c = 0; c < 3; ++c) dbar[va + 3 + c] += 0.5 * a[c] + b[c] / 12.0 - c3v[c] / 12.0;
 }
 
@@ -115,6 +124,8 @@ template <int ST_> struct Rk {
 // stride of the cooperative workspaces: contiguous per group, warp-interleaved for one-lane groups
 template <int G> struct StrideOf { static const int value = (G == 1) ? 32 : 1; };
 
+template <class R, int G> __device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* conv_out);
+
 // ---- S7: one attempted step: stages 1..7 (stage 1 reused when have_k1), proposal, error vector -----
 // KEEP: also store every stage's (Yq, V, Dl) for the reverse sweep.
 template <class R, int G, bool KEEP>
@@ -125,33 +136,40 @@ DMX_DN void rk_attempt(const ModelDev<R>& m, int tab, const Rk<StrideOf<G>::valu
   const int nv = m.nv, nq = m.nq;
   ok = true; unconverged = 0;
   const int ns = KEEP ? 6 : 7;     // the reverse sweep needs stages 1..6 only
+#pragma unroll 1
   for (int i = 0; i < ns; ++i) {
+#pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) {
       double sq = 0, sv = 0;
+#pragma unroll 1
       for (int l = 0; l < i; ++l) { sq += TAB_A[tab][i][l] * rk.K()[l * nv + j]; sv += TAB_A[tab][i][l] * rk.A()[l * nv + j]; }
       rk.Dl()[j] = h * sq; rk.V()[j] = rk.v()[j] + h * sv;
     }
     gr.sync();
+#pragma unroll 1
     for (int jn = gr.lane; jn < m.njnt; jn += G) retract_joint(m, jn, rk.q(), rk.Dl(), rk.V(), rk.Yq(), rk.K().at(i * nv));
     gr.sync();
+#pragma unroll 1
     for (int j = gr.lane; j < nq; j += G) { Yqr[j] = (R)rk.Yq()[j]; if (KEEP && i < 6) rk.sYq()[i * nq + j] = rk.Yq()[j]; }
+#pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) {
       Vr[j] = (R)rk.V()[j];
       if (KEEP && i < 6) { rk.sV()[i * nv + j] = rk.V()[j]; rk.sDl()[i * nv + j] = rk.Dl()[j]; }
     }
     gr.sync();
     if (i == 0 && have_k1) continue;
-    InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
-    bool conv;
-    int nr = vector_field<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, false, conv, gr);
+    int conv;
+    int nr = field_eval<R, G>(u, p, 0, &conv);
     if (nr < 0) { ok = false; for (int j = gr.lane; j < nv; j += G) rk.A()[i * nv + j] = nan(""); }
     else { for (int j = gr.lane; j < nv; j += G) rk.A()[i * nv + j] = (double)ws.x()[j]; if (nr > 0 && !conv) unconverged++; }
     gr.sync();
   }
   if (!KEEP) {
     // row 6 of a is b: stage 7 is the proposal y_{n+1} = (Yq, V) and k7 = (V, A[6]) (FSAL)
+#pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) {
       double eq = 0, ev = 0;
+#pragma unroll 1
       for (int i = 0; i < 7; ++i) { eq += TAB_E[tab][i] * rk.K()[i * nv + j]; ev += TAB_E[tab][i] * rk.A()[i * nv + j]; }
       rk.err()[j] = h * eq; rk.err()[nv + j] = h * ev;
     }
@@ -164,6 +182,7 @@ template <class R, int ST>
 DMX_DN double error_norm(const ModelDev<R>& m, const Rk<ST>& rk, double rtol, double atol, bool& finite) {
   const int nv = m.nv;
   double acc = 0.0;
+#pragma unroll 1
   for (int d = 0; d < nv; ++d) {
     int j = m.dof_jnt[d], c = d - m.jnt_vadr[j];
     double mag = 1.0;
@@ -173,6 +192,7 @@ DMX_DN double error_norm(const ModelDev<R>& m, const Rk<ST>& rk, double rtol, do
     double r = __ddiv_rn(e, __dadd_rn(atol, __dmul_rn(rtol, mag)));
     acc = __dadd_rn(acc, __dmul_rn(r, r));
   }
+#pragma unroll 1
   for (int d = 0; d < nv; ++d) {
     double e = rk.err()[nv + d];
     if (!isfinite(e)) finite = false;
@@ -200,12 +220,20 @@ template <class R> struct RolloutArgs {
 
 // Shared-memory copies of the model header and the layouts (one per CTA), so that the non-inlined device
 // functions read them with plain shared loads.
-template <class R> struct CtaConst { ModelDev<R> m; WsLayout wl, rwl; RkLayout rl; };
+template <class R> struct CtaConst { ModelDev<R> m; WsLayout wl, rwl; RkLayout rl; int nd; };
+static __shared__ CtaConst<double> g_cc64;
+static __shared__ CtaConst<float> g_cc32;
+extern __shared__ __align__(16) unsigned char dyn_smem[];
+template <class R> DMX_DI CtaConst<R>& cta_const();
+template <> DMX_DI CtaConst<double>& cta_const<double>() { return g_cc64; }
+template <> DMX_DI CtaConst<float>& cta_const<float>() { return g_cc32; }
 template <class R>
-DMX_DI void load_cta_const(CtaConst<R>& c, const ModelDev<R>& m, const WsLayout& wl, const WsLayout& rwl, const RkLayout& rl) {
+DMX_DI void load_cta_const(CtaConst<R>& c, const ModelDev<R>& m, const WsLayout& wl, const WsLayout& rwl, const RkLayout& rl, int nd) {
+  if (threadIdx.x == 0) c.nd = nd;
   const int* src[4] = {reinterpret_cast<const int*>(&m), reinterpret_cast<const int*>(&wl), reinterpret_cast<const int*>(&rwl), reinterpret_cast<const int*>(&rl)};
   int* dst[4] = {reinterpret_cast<int*>(&c.m), reinterpret_cast<int*>(&c.wl), reinterpret_cast<int*>(&c.rwl), reinterpret_cast<int*>(&c.rl)};
   const int n[4] = {(int)(sizeof(ModelDev<R>) / 4), (int)(sizeof(WsLayout) / 4), (int)(sizeof(WsLayout) / 4), (int)(sizeof(RkLayout) / 4)};
+#pragma unroll 1
   for (int k = 0; k < 4; ++k) for (int i = threadIdx.x; i < n[k]; i += blockDim.x) dst[k][i] = src[k][i];
   __syncthreads();
 }
@@ -227,12 +255,28 @@ DMX_DI void bind_shared(unsigned char* smem, int nd, int nr_, int ni, Rk<StrideO
   Yqr = Arr<R, ST>(rreg + rl->Yqr * ST); Vr = Arr<R, ST>(rreg + rl->Vr * ST);
 }
 
+// F or F~ at the stage state held in this group's (Yqr, Vr); one copy per kernel, shared by the stage recomputation
+// and the VJP.  All pointers are re-derived from the CTA's shared memory, so the accesses stay shared-space loads.
+template <class R, int G>
+__device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* conv_out) {
+  const int ST = StrideOf<G>::value;
+  CtaConst<R>& cc = cta_const<R>();
+  const Grp<G> gr = make_group<G>();
+  Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
+  bind_shared<R, G>(dyn_smem, cc.nd, cc.wl.size + cc.rl.rsize, cc.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
+  InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
+  bool conv;
+  int nr = vector_field<Ws<R, ST>, R, G, InPlain<R, ST> >(cc.m, in, ws, cfd != 0, conv, gr);
+  *conv_out = conv ? 1 : 0;
+  return nr;
+}
+
 // ---- forward rollout: persistent lane groups pulling environments from a global queue --------------
 template <class R, int G>
 __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ RolloutArgs<R> a) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  __shared__ CtaConst<R> cc;
-  load_cta_const<R>(cc, m_, a.wl, a.wl, a.rl);
+  unsigned char* smem = dyn_smem;
+  CtaConst<R>& cc = cta_const<R>();
+  load_cta_const<R>(cc, m_, a.wl, a.wl, a.rl, a.rl.size_fwd);
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
@@ -241,6 +285,7 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
   const int nq = m.nq, nv = m.nv, nu = m.nu, nx = nq + nv, tab = a.so.tableau, rec = nx + 2;
   const bool has_ctrl = a.ctrl != nullptr && a.nknot > 0 && nu > 0;
   const int nknot = has_ctrl ? a.nknot : 0;
+#pragma unroll 1
   for (;;) {
     int e = 0;
     if (gr.lane == 0) e = atomicAdd(a.queue, 1);
@@ -248,7 +293,9 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
     if (e >= a.nenv) break;
     const R* x0 = a.x0 + (size_t)e * nx;
     const R* p = a.params ? a.params + (size_t)e * m.np : m.p_default;
+#pragma unroll 1
     for (int j = gr.lane; j < nq; j += G) rk.q()[j] = (double)x0[j];
+#pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) rk.v()[j] = (double)x0[nq + j];
     gr.sync();
     double t = 0.0, hprop = a.so.h0, Eprev = 1.0, hmin = INFINITY, hmax = 0.0;
@@ -291,12 +338,16 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
       bool knot_up = hits && tb < a.horizon;
       if (tape) {   // S9: checkpoint record (y_n, t_n, +-h_n); a negative h marks a step that ends a control interval
         R* r = tape + (size_t)n_acc * rec;
+#pragma unroll 1
         for (int j = gr.lane; j < nq; j += G) r[j] = (R)rk.q()[j];
+#pragma unroll 1
         for (int j = gr.lane; j < nv; j += G) r[nq + j] = (R)rk.v()[j];
         if (gr.lane == 0) { r[nx] = (R)t; r[nx + 1] = (R)(knot_up ? -h : h); }
       }
       gr.sync();
+#pragma unroll 1
       for (int j = gr.lane; j < nq; j += G) rk.q()[j] = rk.Yq()[j];
+#pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) rk.v()[j] = rk.V()[j];
       n_acc++; hmin = fmin(hmin, h); hmax = fmax(hmax, h);
       if (hits) {
@@ -307,7 +358,9 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
       gr.sync();
     }
     R* xT = a.xT + (size_t)e * nx;
+#pragma unroll 1
     for (int j = gr.lane; j < nq; j += G) xT[j] = (R)rk.q()[j];
+#pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) xT[nq + j] = (R)rk.v()[j];
     if (gr.lane == 0) {
       if (a.n_accept) a.n_accept[e] = n_acc;
