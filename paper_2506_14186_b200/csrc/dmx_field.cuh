@@ -239,6 +239,8 @@ DMX_DI void tri_index(int e, int& a, int& b) {
 }
 
 // ---- dense Cholesky on the lower triangle, one column at a time, lanes over rows ---------------
+// The factor is stored with the RECIPROCAL of its diagonal (l_jj^-1 = rsqrt of the pivot), so the column scaling
+// and both substitutions multiply instead of divide: the dependent chain per column is one rsqrt, not sqrt + div.
 template <class S, int ST, int G> DMX_DN bool cholesky(const Arr<S, ST>& A, int n, const Grp<G>& gr) {
 #pragma unroll 1
   for (int j = 0; j < n; ++j) {
@@ -252,35 +254,35 @@ template <class S, int ST, int G> DMX_DN bool cholesky(const Arr<S, ST>& A, int 
     gr.sync();
     S s = A[j * n + j];
     if (!(val(s) > 0)) return false;       // uniform over the group
-    S l = m_sqrt(s);
+    S il = m_rsqrt(s);
     gr.sync();
 #pragma unroll 1
-    for (int i = j + gr.lane; i < n; i += G) A[i * n + j] = (i == j) ? l : A[i * n + j] / l;
+    for (int i = j + gr.lane; i < n; i += G) A[i * n + j] = (i == j) ? il : A[i * n + j] * il;
     gr.sync();
   }
   return true;
 }
-// b <- (L L^T)^-1 b; column-oriented substitutions
+// b <- (L L^T)^-1 b; column-oriented substitutions (diagonal of L holds reciprocals)
 template <class S, int ST, int G> DMX_DN void chol_solve(const Arr<S, ST>& L, int n, const Arr<S, ST>& b, const Grp<G>& gr) {
 #pragma unroll 1
   for (int i = 0; i < n; ++i) {
-    S bi = b[i] / L[i * n + i];
+    S bi = b[i] * L[i * n + i];
 #pragma unroll 1
     for (int k = i + 1 + gr.lane; k < n; k += G) b[k] = b[k] - L[k * n + i] * bi;
     gr.sync();
   }
 #pragma unroll 1
-  for (int i = gr.lane; i < n; i += G) b[i] = b[i] / L[i * n + i];
+  for (int i = gr.lane; i < n; i += G) b[i] = b[i] * L[i * n + i];
   gr.sync();
 #pragma unroll 1
   for (int i = n - 1; i >= 0; --i) {
-    S bi = b[i] / L[i * n + i];
+    S bi = b[i] * L[i * n + i];
 #pragma unroll 1
     for (int k = gr.lane; k < i; k += G) b[k] = b[k] - L[i * n + k] * bi;
     gr.sync();
   }
 #pragma unroll 1
-  for (int i = gr.lane; i < n; i += G) b[i] = b[i] / L[i * n + i];
+  for (int i = gr.lane; i < n; i += G) b[i] = b[i] * L[i * n + i];
   gr.sync();
 }
 
@@ -544,11 +546,14 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
 template <class WS, class R, int G, class IN>
 DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, bool& conv, const Grp<G>& gr) {
   const int nv = m.nv;
+  phase_sync();
   DMX_T0;
   kinematics<WS, R, G, IN, false>(m, in, ws, gr);
   DMX_TICK(gr, 0);
+  phase_sync();
   dynamics<WS, R, G, IN>(m, in, ws, gr);
   DMX_TICK(gr, 1);
+  phase_sync();
 #pragma unroll 1
   for (int e = gr.lane; e < nv * nv; e += G) ws.Hc()[e] = ws.M()[e];
 #pragma unroll 1
@@ -558,8 +563,10 @@ DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool c
   if (!cholesky(ws.Hc(), nv, gr)) return -1;
   chol_solve(ws.Hc(), nv, ws.a0(), gr);
   DMX_TICK(gr, 2);
+  phase_sync();
   int nr = build_rows<WS, R, G, IN>(m, in, ws, cfd, gr);
   DMX_TICK(gr, 3);
+  phase_sync();
   conv = newton<WS, G>(nv, nr, m.newton_iters, m.ls_iters, ws, gr);
   DMX_TICK(gr, 4);
   bool fin = true;

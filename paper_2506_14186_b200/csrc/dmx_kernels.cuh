@@ -21,20 +21,24 @@ DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yq
   int nr = field_eval<R, G>(u, p, cfd ? 1 : 0, &conv);
   if (nr < 0) return false;
   DMX_TICK(gr, 8);
+  phase_sync();
 #pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) ws.kap()[j] = (R)kappa[j];
   gr.sync();
   if (!vjp_prepare<Ws<R, ST>, G>(nv, nr, ws, gr)) return false;
   DMX_TICK(gr, 9);
+  phase_sync();
   // u: closed form; v: reverse sweep over the tree; then the frames at acceleration x* for the tangent passes
 #pragma unroll 1
   for (int i = gr.lane; i < m.nu; i += G)
     rk.ubar()[i] = (double)(ws.kap()[m.jnt_vadr[m.act_jnt[i]]] * (m.act_type[i] == ACT_MOTOR ? m.act_gear[i] : m.act_kp[i]));
   if (!(dbg & 2)) vjp_velocity<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, nr, rk.vbar(), gr);
   DMX_TICK(gr, 10);
+  phase_sync();
   in.aa = ws.x();
   kinematics<Ws<R, ST>, R, G, InPlain<R, ST>, true>(m, in, ws, gr);
   DMX_TICK(gr, 11);
+  phase_sync();
   const int ndir = (dbg & 1) ? 0 : nv + (want_p ? m.np : 0);
 #pragma unroll 1
   for (int d = gr.lane; d < ndir; d += G) {
@@ -50,7 +54,7 @@ DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yq
 }
 
 template <class R> struct BackwardArgs {
-  int nenv, nknot, want_p, cfd, tape_cap, dbg;
+  int nenv, nknot, want_p, cfd, tape_cap, dbg, lockstep;
   const R *ctrl, *params, *zero_u, *xT, *dLdxT;
   const int* status;
   SolverOpts so;
@@ -75,6 +79,7 @@ template <class R, int G>
 __global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ BackwardArgs<R> a) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
+  if (threadIdx.x == 0) g_lockstep = a.lockstep;
   load_cta_const<R>(cc, m_, a.wl, a.rwl, a.rl, 0);
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
@@ -186,6 +191,7 @@ __global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ M
     if (!good && a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nknot * nu; c += G) a.dLdctrl[(size_t)e * nknot * nu + c] = R(0);
     gr.sync();
   }
+  phase_drain();
 }
 
 // ---- building blocks for parity tests: one lane group per state --------------------------------------
@@ -200,6 +206,7 @@ template <class R, int G>
 __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ FieldArgs<R> a) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
+  if (threadIdx.x == 0) g_lockstep = 0;
   load_cta_const<R>(cc, m_, a.wl, a.rwl, a.rl, a.rl.size_bwd);
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
@@ -247,6 +254,7 @@ __global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ 
                                                         const __grid_constant__ WsLayout wl, const __grid_constant__ RkLayout rl) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
+  if (threadIdx.x == 0) g_lockstep = 0;
   load_cta_const<R>(cc, m_, wl, wl, rl, rl.size_bwd);
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;

@@ -32,6 +32,20 @@ static __device__ unsigned long long g_prof[32];
 #define DMX_TICK(gr, id) do {} while (0)
 #endif
 
+// ---- phase synchronisation of a CTA's lane groups ---------------------------------------------------
+// With lockstep on, every lane group arrives at a CTA-wide barrier before each phase of the vector field and of
+// the VJP, so that the warps of a CTA run the same (small) piece of code at the same time and share the fetched
+// instruction lines.  The barrier is the non-aligned form: groups of one warp arrive from different code
+// locations.  A group that has run out of environments keeps arriving (with done = 1) until all groups are done.
+static __shared__ int g_lockstep;
+DMX_DI int cta_barrier_and(int p) {
+  int r;
+  asm volatile("{\n\t.reg .pred q, o;\n\tsetp.ne.b32 q, %1, 0;\n\tbarrier.cta.red.and.pred o, 1, q;\n\tselp.b32 %0, 1, 0, o;\n\t}" : "=r"(r) : "r"(p) : "memory");
+  return r;
+}
+DMX_DI void phase_sync() { if (g_lockstep) cta_barrier_and(0); }
+DMX_DI void phase_drain() { if (g_lockstep) while (!cta_barrier_and(1)) {} }
+
 // ---- tangent scalar: value and one directional derivative -------------------------------
 template <class T> struct Dual {
   T v, d;
@@ -59,6 +73,8 @@ template <class T> struct RealOf<Dual<T> > { typedef T type; };
 
 DMX_DI double m_sqrt(double a) { return sqrt(a); }
 DMX_DI float m_sqrt(float a) { return sqrtf(a); }
+DMX_DI double m_rsqrt(double a) { return rsqrt(a); }
+DMX_DI float m_rsqrt(float a) { return rsqrtf(a); }
 DMX_DI double m_exp(double a) { return exp(a); }
 DMX_DI float m_exp(float a) { return expf(a); }
 DMX_DI double m_log(double a) { return log(a); }
@@ -68,6 +84,7 @@ DMX_DI float m_pow(float a, float b) { return powf(a, b); }
 DMX_DI void m_sincos(double a, double& s, double& c) { sincos(a, &s, &c); }
 DMX_DI void m_sincos(float a, float& s, float& c) { sincosf(a, &s, &c); }
 template <class T> DMX_DI Dual<T> m_sqrt(const Dual<T>& a) { T s = m_sqrt(a.v); return Dual<T>(s, a.d * (T(0.5) / s)); }
+template <class T> DMX_DI Dual<T> m_rsqrt(const Dual<T>& a) { T r = m_rsqrt(a.v); return Dual<T>(r, a.d * (T(-0.5) * r / a.v)); }
 template <class T> DMX_DI Dual<T> m_exp(const Dual<T>& a) { T e = m_exp(a.v); return Dual<T>(e, e * a.d); }
 template <class T> DMX_DI Dual<T> m_log(const Dual<T>& a) { return Dual<T>(m_log(a.v), a.d / a.v); }
 template <class T> DMX_DI void m_sincos(const Dual<T>& a, Dual<T>& s, Dual<T>& c) {

@@ -157,7 +157,7 @@ DMX_DN void rk_attempt(const ModelDev<R>& m, int tab, const Rk<StrideOf<G>::valu
       if (KEEP && i < 6) { rk.sV()[i * nv + j] = rk.V()[j]; rk.sDl()[i * nv + j] = rk.Dl()[j]; }
     }
     gr.sync();
-    if (i == 0 && have_k1) continue;
+    if (i == 0 && have_k1) { for (int k = 0; k < 5; ++k) phase_sync(); continue; }   // keep the CTA's phases aligned
     int conv;
     int nr = field_eval<R, G>(u, p, 0, &conv);
     if (nr < 0) { ok = false; for (int j = gr.lane; j < nv; j += G) rk.A()[i * nv + j] = nan(""); }
@@ -204,7 +204,7 @@ DMX_DN double error_norm(const ModelDev<R>& m, const Rk<ST>& rk, double rtol, do
 
 // ---- kernel arguments ------------------------------------------------------------------------------
 template <class R> struct RolloutArgs {
-  int nenv, nknot, n_replay, tape_cap, want_tape;
+  int nenv, nknot, n_replay, tape_cap, want_tape, lockstep;
   const R *x0, *ctrl, *params, *zero_u;
   const double* h_replay;
   double knot_dt, horizon;
@@ -276,6 +276,7 @@ template <class R, int G>
 __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ RolloutArgs<R> a) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
+  if (threadIdx.x == 0) g_lockstep = a.lockstep;
   load_cta_const<R>(cc, m_, a.wl, a.wl, a.rl, a.rl.size_fwd);
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
@@ -375,6 +376,7 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
     }
     gr.sync();
   }
+  phase_drain();
 }
 
 }  // namespace dmx
