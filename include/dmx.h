@@ -101,8 +101,13 @@ int dmx_model_default_params(const dmx_model *m, double *p_host);
 /* Lanes per environment the kernels use for this model (1, 8, 16 or 32). */
 int dmx_model_lanes(const dmx_model *m);
 
-/* Bytes of tape for nenv environments with room for tape_steps accepted steps each
- * (checkpoint record = (y_n, t_n, h_n): (nq+nv+2) reals). */
+/* Tape record per accepted step: the checkpoint (y_n, t_n, h_n), nq+nv+2 reals, and - by
+ * default - the six stage rates A_1..A_6 (6*nv reals), so that the reverse sweep rebuilds the stage states without
+ * re-evaluating F (memory for time, the checkpoint-count knob of PAPER.md:371).  on = 0 keeps the checkpoint only and
+ * the reverse sweep recomputes the stages with six F evaluations per step.  Set before sizing / writing a tape. */
+int dmx_model_set_tape_stages(dmx_model *m, int on);
+
+/* Bytes of tape for nenv environments with room for tape_steps accepted steps each. */
 size_t dmx_tape_bytes(const dmx_model *m, int nenv, int tape_steps);
 
 /* Forward rollout (PAPER.md:41 x_{k+1}=step(x_k,a_k,p); Eq. 5 at PAPER.md:422-425): integrates

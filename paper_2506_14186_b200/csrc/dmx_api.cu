@@ -243,7 +243,7 @@ template <class R> void build_dev(const HostModel& h, Arena& ar, ModelDev<R>& m,
 
 // ---- the model object -------------------------------------------------------------------------------------
 struct dmx_model {
-  int precision, G, sm_count, max_smem;
+  int precision, G, sm_count, max_smem, tape_stages = 1;
   HostModel h;
   Arena arena;
   ModelDev<double> md; ModelDev<float> mf;
@@ -359,8 +359,8 @@ int rollout_typed(const dmx_model* m, int nenv, const void* x0, const void* ctrl
                   const dmx_solver_opts* opts, const double* h_replay, int n_replay, void* xT, const dmx_stats* st, void* tape, size_t tape_bytes,
                   cudaStream_t s) {
   RolloutArgs<R> a; std::memset(&a, 0, sizeof(a));
-  const int rec = m->h.nq + m->h.nv + 2;
-  a.nenv = nenv; a.nknot = nknot; a.n_replay = h_replay ? n_replay : 0; a.want_tape = tape != nullptr;
+  const int rec = m->h.nq + m->h.nv + 2 + (m->tape_stages ? 6 * m->h.nv : 0);
+  a.nenv = nenv; a.nknot = nknot; a.n_replay = h_replay ? n_replay : 0; a.want_tape = tape != nullptr; a.tape_stages = m->tape_stages;
   if (tape) {
     size_t hdr = tape_header_bytes(nenv);
     if (tape_bytes < hdr + (size_t)nenv * rec * sizeof(R)) return fail("tape too small");
@@ -386,10 +386,10 @@ int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const vo
                    const void* dLdxT, int cfd_on, void* dLdx0, void* dLdctrl, void* dLdparams, const int* status, const void* tape,
                    size_t tape_bytes, cudaStream_t s) {
   BackwardArgs<R> a; std::memset(&a, 0, sizeof(a));
-  const int rec = m->h.nq + m->h.nv + 2;
+  const int rec = m->h.nq + m->h.nv + 2 + (m->tape_stages ? 6 * m->h.nv : 0);
   size_t hdr = tape_header_bytes(nenv);
   if (!tape || tape_bytes < hdr + (size_t)nenv * rec * sizeof(R)) return fail("tape missing or too small");
-  a.nenv = nenv; a.nknot = nknot; a.want_p = dLdparams != nullptr; a.cfd = cfd_on;
+  a.nenv = nenv; a.nknot = nknot; a.want_p = dLdparams != nullptr; a.cfd = cfd_on; a.tape_stages = m->tape_stages;
   { const char* e = std::getenv("DMX_DBG"); a.dbg = e ? std::atoi(e) : 0; }   // timing experiments only (results invalid when set)
   a.tape_cap = (int)std::min<size_t>((tape_bytes - hdr) / ((size_t)nenv * rec * sizeof(R)), (size_t)1 << 30);
   a.tape_hdr = (const int*)tape; a.tape = (const R*)((const unsigned char*)tape + hdr);
@@ -489,6 +489,11 @@ void dmx_model_destroy(dmx_model* m) {
   delete m;
 }
 
+int dmx_model_set_tape_stages(dmx_model* m, int on) {
+  if (!m) return fail("null model");
+  m->tape_stages = on ? 1 : 0;
+  return 0;
+}
 int dmx_model_np(const dmx_model* m) { return m ? m->h.np : -1; }
 int dmx_model_nc(const dmx_model* m) { return m ? m->h.nc : -1; }
 int dmx_model_lanes(const dmx_model* m) { return m ? m->G : -1; }
@@ -500,7 +505,7 @@ int dmx_model_default_params(const dmx_model* m, double* p_host) {
 
 size_t dmx_tape_bytes(const dmx_model* m, int nenv, int tape_steps) {
   if (!m || nenv <= 0 || tape_steps <= 0) return 0;
-  return tape_header_bytes(nenv) + (size_t)nenv * (size_t)tape_steps * (size_t)(m->h.nq + m->h.nv + 2) * rsize(m);
+  return tape_header_bytes(nenv) + (size_t)nenv * (size_t)tape_steps * (size_t)(m->h.nq + m->h.nv + 2 + (m->tape_stages ? 6 * m->h.nv : 0)) * rsize(m);
 }
 
 static int check_common(const dmx_model* m, int nenv, const void* x0, const dmx_solver_opts* o, double horizon) {

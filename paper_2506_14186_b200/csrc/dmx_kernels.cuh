@@ -54,7 +54,7 @@ DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yq
 }
 
 template <class R> struct BackwardArgs {
-  int nenv, nknot, want_p, cfd, tape_cap, dbg, lockstep;
+  int nenv, nknot, want_p, cfd, tape_cap, dbg, lockstep, tape_stages;
   const R *ctrl, *params, *zero_u, *xT, *dLdxT;
   const int* status;
   SolverOpts so;
@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ M
   if (G == 1) rk.b = a.rk_scratch + ((size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32 * (size_t)a.rl.size_bwd + (threadIdx.x & 31);
   else rk.b = a.rk_scratch + ((size_t)blockIdx.x * (blockDim.x / G) + threadIdx.x / G) * (size_t)a.rl.size_bwd;
   Ws<Dual<R>, 32> dws = bind_scratch<R>(a.scratch, a.res_size, &cc.rwl);
-  const int nq = m.nq, nv = m.nv, nu = m.nu, np = m.np, nx = nq + nv, tab = a.so.tableau, rec = nx + 2;
+  const int nq = m.nq, nv = m.nv, nu = m.nu, np = m.np, nx = nq + nv, tab = a.so.tableau, rec = nx + 2 + (a.tape_stages ? 6 * nv : 0);
   const bool has_ctrl = a.ctrl != nullptr && a.nknot > 0 && nu > 0;
   const int nknot = has_ctrl ? a.nknot : 0;
 #pragma unroll 1
@@ -132,9 +132,11 @@ __global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ M
       double hs = (double)r[nx + 1], h = fabs(hs);
       if (hs < 0) knot--;
       const R* u = has_ctrl ? a.ctrl + ((size_t)e * nknot + knot) * nu : a.zero_u;
+      if (a.tape_stages) for (int j = gr.lane; j < 6 * nv; j += G) rk.A()[j] = (double)r[nx + 2 + j];
       gr.sync();
       bool ok; int unc;
-      rk_attempt<R, G, true>(m, tab, rk, Yqr, Vr, u, p, h, false, ws, ok, unc, gr);   // recompute the stages with F
+      // stage states: recomputed with F from the checkpoint, or rebuilt from the taped stage rates
+      rk_attempt<R, G, true>(m, tab, rk, Yqr, Vr, u, p, h, false, ws, ok, unc, gr, a.tape_stages != 0);
       // y_{n+1} = (q_n (+) h sum b_i K_i, v_n + h sum b_i A_i), b = row 6 of a
 #pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) {

@@ -131,7 +131,7 @@ template <class R, int G> __device__ __noinline__ int field_eval(const R* u, con
 template <class R, int G, bool KEEP>
 DMX_DN void rk_attempt(const ModelDev<R>& m, int tab, const Rk<StrideOf<G>::value>& rk, const Arr<R, StrideOf<G>::value>& Yqr,
                        const Arr<R, StrideOf<G>::value>& Vr, const R* u, const R* p, double h, bool have_k1,
-                       const Ws<R, StrideOf<G>::value>& ws, bool& ok, int& unconverged, const Grp<G>& gr) {
+                       const Ws<R, StrideOf<G>::value>& ws, bool& ok, int& unconverged, const Grp<G>& gr, bool restore = false) {
   const int ST = StrideOf<G>::value;
   const int nv = m.nv, nq = m.nq;
   ok = true; unconverged = 0;
@@ -157,6 +157,7 @@ DMX_DN void rk_attempt(const ModelDev<R>& m, int tab, const Rk<StrideOf<G>::valu
       if (KEEP && i < 6) { rk.sV()[i * nv + j] = rk.V()[j]; rk.sDl()[i * nv + j] = rk.Dl()[j]; }
     }
     gr.sync();
+    if (restore) continue;       // stage rates A_i come from the tape: stage states only
     if (i == 0 && have_k1) { for (int k = 0; k < 5; ++k) phase_sync(); continue; }   // keep the CTA's phases aligned
     int conv;
     int nr = field_eval<R, G>(u, p, 0, &conv);
@@ -204,7 +205,7 @@ DMX_DN double error_norm(const ModelDev<R>& m, const Rk<ST>& rk, double rtol, do
 
 // ---- kernel arguments ------------------------------------------------------------------------------
 template <class R> struct RolloutArgs {
-  int nenv, nknot, n_replay, tape_cap, want_tape, lockstep;
+  int nenv, nknot, n_replay, tape_cap, want_tape, lockstep, tape_stages;
   const R *x0, *ctrl, *params, *zero_u;
   const double* h_replay;
   double knot_dt, horizon;
@@ -283,7 +284,7 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
   const Grp<G> gr = make_group<G>();
   Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
   bind_shared<R, G>(smem, a.rl.size_fwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
-  const int nq = m.nq, nv = m.nv, nu = m.nu, nx = nq + nv, tab = a.so.tableau, rec = nx + 2;
+  const int nq = m.nq, nv = m.nv, nu = m.nu, nx = nq + nv, tab = a.so.tableau, rec = nx + 2 + (a.tape_stages ? 6 * nv : 0);
   const bool has_ctrl = a.ctrl != nullptr && a.nknot > 0 && nu > 0;
   const int nknot = has_ctrl ? a.nknot : 0;
 #pragma unroll 1
@@ -344,6 +345,7 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
 #pragma unroll 1
         for (int j = gr.lane; j < nv; j += G) r[nq + j] = (R)rk.v()[j];
         if (gr.lane == 0) { r[nx] = (R)t; r[nx + 1] = (R)(knot_up ? -h : h); }
+        if (a.tape_stages) for (int j = gr.lane; j < 6 * nv; j += G) r[nx + 2 + j] = (R)rk.A()[j];   // stage rates A_1..A_6
       }
       gr.sync();
 #pragma unroll 1

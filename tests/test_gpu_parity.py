@@ -94,12 +94,15 @@ def test_vector_field_and_vjp_match_oracle(B, oracle_mod, cfg, cfd):
 
 
 # ---- S7-S10: rollouts and reverse sweep, identical step sequences -----------------------------------------------------
+@pytest.mark.parametrize("stages", [1, 0])
 @pytest.mark.parametrize("cfg", ["C1", "C2", "C3", "C4", "C5"])
-def test_rollout_and_gradient_replay_parity_fp64(B, oracle_mod, cfg):
+def test_rollout_and_gradient_replay_parity_fp64(B, oracle_mod, cfg, stages):
+    """stages=1: tape holds the stage rates (default); stages=0: checkpoints only, stages recomputed with F."""
     import torch
     w = W.make(cfg, **SMALL[cfg])
     nenv = w["nenv"]
     orc = oracle_mod.Oracle(w["model"]); m = B.Model(w["model"])
+    m.set_tape_stages(stages)
     of, g, og, nmax = _oracle_run(orc, w, cfd=False)
     x0, ctrl = m.dev(w["x0"]), m.dev(w["ctrl"])
     stats = m.alloc_stats(nenv)
