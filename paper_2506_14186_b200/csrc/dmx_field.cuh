@@ -247,7 +247,7 @@ template <class S, int ST, int G> DMX_DN bool cholesky(const Arr<S, ST>& A, int 
 #pragma unroll 1
     for (int i = j + gr.lane; i < n; i += G) {
       S t = A[i * n + j];
-#pragma unroll 1
+#pragma unroll 4
       for (int k = 0; k < j; ++k) t = t - A[i * n + k] * A[j * n + k];
       A[i * n + j] = t;
     }
@@ -431,7 +431,7 @@ DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
   for (int i = gr.lane; i < nr; i += G) {
     int c = ws.rowcand()[i] >> 2;
     S Jv(0.0);
-#pragma unroll 1
+#pragma unroll 4
     for (int j = 0; j < nv; ++j) Jv = Jv + ws.J()[i * nv + j] * in.v(j);
     ws.aref()[i] = ws.cpost()[c] - ws.cbd()[c] * Jv;
     ws.D()[i] = ws.cD()[c];
@@ -457,7 +457,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
 #pragma unroll 1
     for (int i = gr.lane; i < nr; i += G) {
       S t(0.0);
-#pragma unroll 1
+#pragma unroll 4
       for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.x()[j];
       ws.s()[i] = t - ws.aref()[i];
     }
@@ -467,9 +467,9 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
 #pragma unroll 1
     for (int a = gr.lane; a < nv; a += G) {
       S t(0.0);
-#pragma unroll 1
+#pragma unroll 4
       for (int b = 0; b < nv; ++b) t = t + ws.M()[a * nv + b] * ws.xa()[b];
-#pragma unroll 1
+#pragma unroll 4
       for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.J()[i * nv + a] * ws.D()[i] * ws.s()[i];
       ws.g()[a] = t; ws.dl()[a] = -t;
     }
@@ -477,7 +477,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
     for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
       int a, b; tri_index(e, a, b);
       S t = ws.M()[a * nv + b];
-#pragma unroll 1
+#pragma unroll 4
       for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.D()[i] * ws.J()[i * nv + a] * ws.J()[i * nv + b];
       ws.Hc()[a * nv + b] = t;
     }
@@ -488,7 +488,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
 #pragma unroll 1
     for (int i = gr.lane; i < nr; i += G) {
       S t(0.0);
-#pragma unroll 1
+#pragma unroll 4
       for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.dl()[j];
       ws.pr()[i] = t;
       if ((val(ws.s()[i]) < 0) != (val(ws.s()[i] + t) < 0)) same = false;
@@ -502,7 +502,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
 #pragma unroll 1
       for (int a = gr.lane; a < nv; a += G) {
         S t(0.0);
-#pragma unroll 1
+#pragma unroll 4
         for (int b = 0; b < nv; ++b) t = t + ws.M()[a * nv + b] * ws.dl()[b];
         ws.Md()[a] = t;
       }
@@ -541,10 +541,13 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
   return conv;
 }
 
-// ---- F (cfd=false) or F~ (cfd=true) at one state: result in ws.x(), rows and M left in ws ----------
-// returns nr >= 0, or -1 when M is not positive definite / the result is not finite
+// ---- F (cfd=false) or F~ (cfd=true) at one state: result in ws.x, rows and M left in ws ----------
+// returns nr >= 0, or -1 when M is not positive definite / the result is not finite.
+// xk != nullptr: the solution x* is already known (stage rate read from the tape; element j at xk[j*xst]); the
+// unconstrained solve and the Newton iterations are skipped and only M, the rows and x* are set up for the VJP.
 template <class WS, class R, int G, class IN>
-DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, bool& conv, const Grp<G>& gr) {
+DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, bool& conv, const Grp<G>& gr,
+                        const double* xk = nullptr, int xst = 1) {
   const int nv = m.nv;
   phase_sync();
   DMX_T0;
@@ -553,24 +556,28 @@ DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool c
   phase_sync();
   dynamics<WS, R, G, IN>(m, in, ws, gr);
   DMX_TICK(gr, 1);
-  phase_sync();
-#pragma unroll 1
-  for (int e = gr.lane; e < nv * nv; e += G) ws.Hc()[e] = ws.M()[e];
-#pragma unroll 1
-  for (int j = gr.lane; j < nv; j += G) ws.a0()[j] = ws.tau()[j] - ws.c()[j];
-  gr.sync();
   conv = true;
-  if (!cholesky(ws.Hc(), nv, gr)) return -1;
-  chol_solve(ws.Hc(), nv, ws.a0(), gr);
-  DMX_TICK(gr, 2);
+  if (!xk) {
+    phase_sync();
+    for (int e = gr.lane; e < nv * nv; e += G) ws.Hc()[e] = ws.M()[e];
+    for (int j = gr.lane; j < nv; j += G) ws.a0()[j] = ws.tau()[j] - ws.c()[j];
+    gr.sync();
+    if (!cholesky(ws.Hc(), nv, gr)) return -1;
+    chol_solve(ws.Hc(), nv, ws.a0(), gr);
+    DMX_TICK(gr, 2);
+  }
   phase_sync();
   int nr = build_rows<WS, R, G, IN>(m, in, ws, cfd, gr);
   DMX_TICK(gr, 3);
+  if (xk) {
+    for (int j = gr.lane; j < nv; j += G) ws.x()[j] = (R)xk[j * xst];
+    gr.sync();
+    return nr;
+  }
   phase_sync();
   conv = newton<WS, G>(nv, nr, m.newton_iters, m.ls_iters, ws, gr);
   DMX_TICK(gr, 4);
   bool fin = true;
-#pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) if (!isfinite(val(ws.x()[j]))) fin = false;
   if (!gr.all(fin)) return -1;
   return nr;
@@ -584,7 +591,7 @@ DMX_DN bool vjp_prepare(int nv, int nr, const WS& ws, const Grp<G>& gr) {
 #pragma unroll 1
   for (int i = gr.lane; i < nr; i += G) {
     S t(0.0);
-#pragma unroll 1
+#pragma unroll 4
     for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.x()[j];
     t = t - ws.aref()[i];
     ws.s()[i] = t;
@@ -595,7 +602,7 @@ DMX_DN bool vjp_prepare(int nv, int nr, const WS& ws, const Grp<G>& gr) {
   for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
     int a, b; tri_index(e, a, b);
     S t = ws.M()[a * nv + b];
-#pragma unroll 1
+#pragma unroll 4
     for (int i = 0; i < nr; ++i) if (ws.active()[i]) t = t + ws.D()[i] * ws.J()[i * nv + a] * ws.J()[i * nv + b];
     ws.Hc()[a * nv + b] = t;
   }

@@ -11,14 +11,14 @@ namespace dmx {
 template <class R, int G>
 DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yqr, const Arr<R, StrideOf<G>::value>& Vr, const R* u, const R* p,
                       const Arr<double, StrideOf<G>::value>& kappa, bool cfd, bool want_p, const Ws<R, StrideOf<G>::value>& ws,
-                      const Ws<Dual<R>, 32>& dws, const Rk<StrideOf<G>::value>& rk, const Grp<G>& gr, int dbg = 0) {
+                      const Ws<Dual<R>, 32>& dws, const Rk<StrideOf<G>::value>& rk, const Grp<G>& gr, int dbg = 0, const double* xk = nullptr) {
   const int ST = StrideOf<G>::value;
   const int nv = m.nv;
   if (dbg & 4) return true;
   DMX_T0;
   InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
   int conv;
-  int nr = field_eval<R, G>(u, p, cfd ? 1 : 0, &conv);
+  int nr = field_eval<R, G>(u, p, cfd ? 1 : 0, &conv, xk);
   if (nr < 0) return false;
   DMX_TICK(gr, 8);
   phase_sync();
@@ -165,7 +165,8 @@ __global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ M
         for (int j = gr.lane; j < nv; j += G) Vr[j] = (R)rk.sV()[i * nv + j];
         gr.sync();
         // A_i = F(Y_i), or F~ for the straight-through estimator (Eq. 4)
-        if (!vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.Ab().at(i * nv), a.cfd != 0, a.want_p != 0, ws, dws, rk, gr, a.dbg)) { good = false; break; }
+        if (!vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.Ab().at(i * nv), a.cfd != 0, a.want_p != 0, ws, dws, rk, gr, a.dbg,
+                              (a.tape_stages && !a.cfd) ? rk.A().at(i * nv).p : nullptr)) { good = false; break; }   // F: x* = taped A_i
 #pragma unroll 1
         for (int j = gr.lane; j < nv; j += G) rk.Vb()[j] += rk.vbar()[j];
         if (a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nu; c += G) a.dLdctrl[((size_t)e * nknot + knot) * nu + c] += (R)rk.ubar()[c];

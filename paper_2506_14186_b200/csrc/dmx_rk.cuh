@@ -124,7 +124,7 @@ template <int ST_> struct Rk {
 // stride of the cooperative workspaces: contiguous per group, warp-interleaved for one-lane groups
 template <int G> struct StrideOf { static const int value = (G == 1) ? 32 : 1; };
 
-template <class R, int G> __device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* conv_out);
+template <class R, int G> __device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* conv_out, const double* xk = nullptr);
 
 // ---- S7: one attempted step: stages 1..7 (stage 1 reused when have_k1), proposal, error vector -----
 // KEEP: also store every stage's (Yq, V, Dl) for the reverse sweep.
@@ -259,7 +259,7 @@ DMX_DI void bind_shared(unsigned char* smem, int nd, int nr_, int ni, Rk<StrideO
 // F or F~ at the stage state held in this group's (Yqr, Vr); one copy per kernel, shared by the stage recomputation
 // and the VJP.  All pointers are re-derived from the CTA's shared memory, so the accesses stay shared-space loads.
 template <class R, int G>
-__device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* conv_out) {
+__device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* conv_out, const double* xk) {
   const int ST = StrideOf<G>::value;
   CtaConst<R>& cc = cta_const<R>();
   const Grp<G> gr = make_group<G>();
@@ -267,7 +267,7 @@ __device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* con
   bind_shared<R, G>(dyn_smem, cc.nd, cc.wl.size + cc.rl.rsize, cc.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
   InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
   bool conv;
-  int nr = vector_field<Ws<R, ST>, R, G, InPlain<R, ST> >(cc.m, in, ws, cfd != 0, conv, gr);
+  int nr = vector_field<Ws<R, ST>, R, G, InPlain<R, ST> >(cc.m, in, ws, cfd != 0, conv, gr, xk, ST);
   *conv_out = conv ? 1 : 0;
   return nr;
 }
