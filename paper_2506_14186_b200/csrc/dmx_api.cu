@@ -324,16 +324,20 @@ int create_typed(dmx_model* m) {
   if (h.npair) CUDA_OK(cudaMemcpy(const_cast<R*>(dev.pair_invweight), pw.data(), sizeof(R) * h.npair, cudaMemcpyHostToDevice));
   if (sizeof(R) == 8) std::memcpy(&m->md, &dev, sizeof(dev)); else std::memcpy(&m->mf, &dev, sizeof(dev));
   // block size per kernel: the one that keeps the most lane groups resident on an SM
-  const int blocks[3] = {128, 64, 32};
-  for (int bi = 0; bi < 3; ++bi) {
+  const int blocks[4] = {256, 128, 64, 32};
+  const char* eb = std::getenv("DMX_BWD_BLOCK");
+  for (int bi = 0; bi < 4; ++bi) {
     int blk = blocks[bi], g = groups_per_block(m, blk);
     size_t sf = g * group_bytes(m, 0), sb = g * group_bytes(m, 1), sx = g * group_bytes(m, 2);
     int of = 0, ob = 0, ox = 0;
     size_t lim = (size_t)m->max_smem - 2048;     // room for the static shared constants
-    CUDA_OK(L.occupancy(blk, std::min(sf, lim), std::min(sb, lim), std::min(sx, lim), &of, &ob, &ox));
-    if (sf <= lim && of * g > m->cf.occ * groups_per_block(m, std::max(m->cf.block, 1))) { m->cf.block = blk; m->cf.occ = of; m->cf.smem = sf; }
-    if (sb <= lim && ob * g > m->cb.occ * groups_per_block(m, std::max(m->cb.block, 1))) { m->cb.block = blk; m->cb.occ = ob; m->cb.smem = sb; }
-    if (sx <= lim && ox * g > m->cx.occ * groups_per_block(m, std::max(m->cx.block, 1))) { m->cx.block = blk; m->cx.occ = ox; m->cx.smem = sx; }
+    if (blk > 128) { int b2 = 128, g2 = groups_per_block(m, b2); int t0, t2;   // only the backward kernel is compiled for 256 threads
+      CUDA_OK(L.occupancy(b2, std::min(g2 * group_bytes(m, 0), lim), std::min(sb, lim), std::min(g2 * group_bytes(m, 2), lim), &t0, &ob, &t2));
+      (void)t0; (void)t2; ob = sb <= lim ? 1 : 0; }
+    else CUDA_OK(L.occupancy(blk, std::min(sf, lim), std::min(sb, lim), std::min(sx, lim), &of, &ob, &ox));
+    if (blk <= 128 && sf <= lim && of * g > m->cf.occ * groups_per_block(m, std::max(m->cf.block, 1))) { m->cf.block = blk; m->cf.occ = of; m->cf.smem = sf; }
+    if (eb ? (std::atoi(eb) == blk && sb <= lim && ob > 0) : (blk <= 128 && sb <= lim && ob * g > m->cb.occ * groups_per_block(m, std::max(m->cb.block, 1)))) { m->cb.block = blk; m->cb.occ = ob; m->cb.smem = sb; }
+    if (blk <= 128 && sx <= lim && ox * g > m->cx.occ * groups_per_block(m, std::max(m->cx.block, 1))) { m->cx.block = blk; m->cx.occ = ox; m->cx.smem = sx; }
   }
   if (m->cf.occ < 1 || m->cb.occ < 1 || m->cx.occ < 1) return fail("model too large for the per-environment shared-memory workspace (try DMX_LANES=32)");
   if (std::getenv("DMX_VERBOSE"))

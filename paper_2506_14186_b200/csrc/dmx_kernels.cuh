@@ -76,7 +76,7 @@ DMX_DI Ws<Dual<R>, 32> bind_scratch(Dual<R>* scratch, int res_size, const WsLayo
 
 // ---- S10: reverse sweep over the tape, frozen step sizes ---------------------------
 template <class R, int G>
-__global__ void __launch_bounds__(128) backward_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ BackwardArgs<R> a) {
+__global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ BackwardArgs<R> a) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
   if (threadIdx.x == 0) g_lockstep = a.lockstep;
