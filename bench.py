@@ -34,6 +34,11 @@ FLOPS_PER_ATTEMPT = dict(C1=7e2, C2=5e4, C3=1.2e5, C4=4.7e5, C5=3.9e5)
 FLOPS_PER_FEVAL = dict(C1=1e2, C2=8e3, C3=2e4, C4=8e4, C5=6e4)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures of the default workload
+# (profiles/r1_rollout_kernel.md, profiles/r1_backward_kernel.md); other workloads were not captured.
+NCU_TRAFFIC_C2_F64_4096 = {"rollout_kernel": 0.571e9, "backward_kernel": 155.7e9}
+
+
 def grad_flops_per_accepted(cfg, cfd):
     """gradient per accepted step = 6 F (recompute) + 6 VJP (2.5 F each) + 6 F~ solves when CFD is on."""
     return (6 + 15 + (6 if cfd else 0)) * FLOPS_PER_FEVAL[cfg]
@@ -257,7 +262,7 @@ def main():
         "ms_per_step": 1e3 * t_step_max, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if args.precision == 64 else "f32", "data": "synthetic",
         "config": {"workload": w["name"], "nenv_per_gpu": nenv, "horizon_s": w["horizon"], "rtol": w["opts"]["rtol"], "cfd_backward": bool(cfd),
-                   "lanes_per_env": m.lanes, "l2": "flushed between timed iterations (256 MiB write)", "tape_steps": cap,
+                   "lanes_per_env": m.lanes, "l2": "flushed between timed iterations (256 MiB write)", "tape_steps": cap, "tape_record": "checkpoint + 6 stage rates",
                    "param_grads": bool(want_p)},
         "forward_env_steps_per_s": acc / t_f, "forward_attempted_steps_per_s": (acc + rej) / t_f, "backward_env_steps_per_s": acc / t_b,
         "ms_forward": 1e3 * t_f, "ms_backward": 1e3 * t_b, "accepted_steps": acc, "rejected_steps": rej, "f_evals": fev, "failed_envs": bad,
@@ -266,10 +271,10 @@ def main():
         "gpu_launches": 2 * args.steps,
         "clocks": clk,
         "roofline": {"bound": "alu", "kernel": dom, "achieved": fl_d / t_d / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s", "frac": fl_d / t_d / peak,
-                     "traffic": None, "peak_source": "measured FMA-chain (dmx_fma_peak) in this run; nominal 37.2 (fp64) / 74.4 (fp32)",
+                     "traffic": NCU_TRAFFIC_C2_F64_4096[dom] if (cfg == "C2" and nenv == 4096 and args.precision == 64 and cfd) else None, "peak_source": "measured FMA-chain (dmx_fma_peak) in this run; nominal 37.2 (fp64) / 74.4 (fp32)",
                      "forward": {"achieved": fl_f / t_f / 1e12, "frac": fl_f / t_f / peak},
                      "backward": {"achieved": fl_b / t_b / 1e12, "frac": fl_b / t_b / peak},
-                     "tape_gbs_write": acc * (m.nq + m.nv + 2) * (8 if args.precision == 64 else 4) / t_f / 1e9},
+                     "tape_gbs_write": acc * (m.nq + m.nv + 2 + 6 * m.nv) * (8 if args.precision == 64 else 4) / t_f / 1e9},
     }
     if not args.no_cpu_baseline:
         cores = os.cpu_count() or 1

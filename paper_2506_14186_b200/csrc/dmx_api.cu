@@ -376,7 +376,7 @@ int rollout_typed(const dmx_model* m, int nenv, const void* x0, const void* ctrl
   if (st) { a.n_accept = st->n_accept; a.n_reject = st->n_reject; a.n_feval = st->n_feval; a.n_unconv = st->n_newton_unconverged; a.status = st->status;
             a.h_min = st->h_min; a.h_max = st->h_max; a.t_end = st->t_end; }
   a.queue = m->queue; a.wl = m->wl; a.rl = m->rl;
-  { const char* e = std::getenv("DMX_LOCKSTEP"); a.lockstep = e ? (std::atoi(e) & 1) : 0; }                 // forward: 2 % fetch stalls, the barriers only cost
+  { const char* e = std::getenv("DMX_LOCKSTEP"); a.lockstep = e ? std::atoi(e) : 0; }                 // forward: 2 % fetch stalls, the barriers only cost
   CUDA_OK(cudaMemsetAsync(m->queue, 0, sizeof(int), s));
   LaunchCfg c; c.block = m->cf.block; c.smem = m->cf.smem;
   int gpb = groups_per_block(m, c.block);
@@ -399,7 +399,7 @@ int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const vo
   a.tape_hdr = (const int*)tape; a.tape = (const R*)((const unsigned char*)tape + hdr);
   a.ctrl = (const R*)ctrl; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u; a.xT = (const R*)xT; a.dLdxT = (const R*)dLdxT;
   a.status = status; a.so = opts_of(opts); a.dLdx0 = (R*)dLdx0; a.dLdctrl = (R*)dLdctrl; a.dLdparams = (R*)dLdparams;
-  { const char* e = std::getenv("DMX_LOCKSTEP"); a.lockstep = e ? ((std::atoi(e) >> 1) & 1) : 1; }          // backward: fetch-bound, phases in lockstep (measured 1.6-2.2x)
+  { const char* e = std::getenv("DMX_LOCKSTEP_BWD"); a.lockstep = e ? std::atoi(e) : 0x1ff; }          // backward: fetch-bound, phases in lockstep (measured 1.6-2.2x)
   a.queue = m->queue + 1; a.wl = m->wl; a.rwl = m->rwl; a.rl = m->rl; a.res_size = m->rwl.size;
   LaunchCfg c; c.block = m->cb.block; c.smem = m->cb.smem;
   int gpb = groups_per_block(m, c.block);

@@ -549,16 +549,16 @@ template <class WS, class R, int G, class IN>
 DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, bool& conv, const Grp<G>& gr,
                         const double* xk = nullptr, int xst = 1) {
   const int nv = m.nv;
-  phase_sync();
+  phase_sync(0);
   DMX_T0;
   kinematics<WS, R, G, IN, false>(m, in, ws, gr);
   DMX_TICK(gr, 0);
-  phase_sync();
+  phase_sync(1);
   dynamics<WS, R, G, IN>(m, in, ws, gr);
   DMX_TICK(gr, 1);
   conv = true;
   if (!xk) {
-    phase_sync();
+    phase_sync(2);
     for (int e = gr.lane; e < nv * nv; e += G) ws.Hc()[e] = ws.M()[e];
     for (int j = gr.lane; j < nv; j += G) ws.a0()[j] = ws.tau()[j] - ws.c()[j];
     gr.sync();
@@ -566,7 +566,7 @@ DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool c
     chol_solve(ws.Hc(), nv, ws.a0(), gr);
     DMX_TICK(gr, 2);
   }
-  phase_sync();
+  phase_sync(3);
   int nr = build_rows<WS, R, G, IN>(m, in, ws, cfd, gr);
   DMX_TICK(gr, 3);
   if (xk) {
@@ -574,7 +574,7 @@ DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool c
     gr.sync();
     return nr;
   }
-  phase_sync();
+  phase_sync(4);
   conv = newton<WS, G>(nv, nr, m.newton_iters, m.ls_iters, ws, gr);
   DMX_TICK(gr, 4);
   bool fin = true;

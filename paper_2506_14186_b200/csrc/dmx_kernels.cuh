@@ -21,24 +21,24 @@ DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yq
   int nr = field_eval<R, G>(u, p, cfd ? 1 : 0, &conv, xk);
   if (nr < 0) return false;
   DMX_TICK(gr, 8);
-  phase_sync();
+  phase_sync(5);
 #pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) ws.kap()[j] = (R)kappa[j];
   gr.sync();
   if (!vjp_prepare<Ws<R, ST>, G>(nv, nr, ws, gr)) return false;
   DMX_TICK(gr, 9);
-  phase_sync();
+  phase_sync(6);
   // u: closed form; v: reverse sweep over the tree; then the frames at acceleration x* for the tangent passes
 #pragma unroll 1
   for (int i = gr.lane; i < m.nu; i += G)
     rk.ubar()[i] = (double)(ws.kap()[m.jnt_vadr[m.act_jnt[i]]] * (m.act_type[i] == ACT_MOTOR ? m.act_gear[i] : m.act_kp[i]));
   if (!(dbg & 2)) vjp_velocity<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, nr, rk.vbar(), gr);
   DMX_TICK(gr, 10);
-  phase_sync();
+  phase_sync(7);
   in.aa = ws.x();
   kinematics<Ws<R, ST>, R, G, InPlain<R, ST>, true>(m, in, ws, gr);
   DMX_TICK(gr, 11);
-  phase_sync();
+  phase_sync(8);
   const int ndir = (dbg & 1) ? 0 : nv + (want_p ? m.np : 0);
 #pragma unroll 1
   for (int d = gr.lane; d < ndir; d += G) {

@@ -43,7 +43,7 @@ DMX_DI int cta_barrier_and(int p) {
   asm volatile("{\n\t.reg .pred q, o;\n\tsetp.ne.b32 q, %1, 0;\n\tbarrier.cta.red.and.pred o, 1, q;\n\tselp.b32 %0, 1, 0, o;\n\t}" : "=r"(r) : "r"(p) : "memory");
   return r;
 }
-DMX_DI void phase_sync() { if (g_lockstep) cta_barrier_and(0); }
+DMX_DI void phase_sync(int id) { if (g_lockstep & (1 << id)) cta_barrier_and(0); }   // g_lockstep: mask of synchronised phases
 DMX_DI void phase_drain() { if (g_lockstep) while (!cta_barrier_and(1)) {} }
 
 // ---- tangent scalar: value and one directional derivative -------------------------------

@@ -158,7 +158,7 @@ DMX_DN void rk_attempt(const ModelDev<R>& m, int tab, const Rk<StrideOf<G>::valu
     }
     gr.sync();
     if (restore) continue;       // stage rates A_i come from the tape: stage states only
-    if (i == 0 && have_k1) { for (int k = 0; k < 5; ++k) phase_sync(); continue; }   // keep the CTA's phases aligned
+    if (i == 0 && have_k1) { for (int k = 0; k < 5; ++k) phase_sync(k); continue; }   // keep the CTA's phases aligned
     int conv;
     int nr = field_eval<R, G>(u, p, 0, &conv);
     if (nr < 0) { ok = false; for (int j = gr.lane; j < nv; j += G) rk.A()[i * nv + j] = nan(""); }
