@@ -214,6 +214,20 @@ def test_batch_independence_bitwise(B, cfg):
     assert torch.equal(one[0], full[5])
 
 
+def test_many_waves_ragged_batch(B):
+    """50 001 one-lane environments (several waves through the work queue, ragged last warp): bitwise equal to a small batch."""
+    import torch
+    w = W.make("C1", nenv=50001, horizon=0.3)
+    m = B.Model(w["model"])
+    x0 = m.dev(w["x0"])
+    st = m.alloc_stats(50001)
+    full = m.rollout(x0, None, 0, 0.0, None, w["horizon"], w["opts"], stats=st)
+    assert (st["status"] == 0).all() and (st["t_end"] == w["horizon"]).all()
+    idx = torch.tensor([0, 31, 32, 12345, 49999, 50000], device=x0.device)
+    part = m.rollout(x0[idx].contiguous(), None, 0, 0.0, None, w["horizon"], w["opts"])
+    assert torch.equal(part, full[idx])
+
+
 def test_full_size_launch_sampled_against_oracle(B, oracle_mod):
     """BASELINE config 2 at full size (4096 envs) in the launch configuration bench.py times: sampled envs are compared
     with the oracle one by one; the rest through batch independence (bitwise equal to the same env run alone)."""
@@ -314,3 +328,42 @@ def test_custom_models_box_arm_spheres(B, oracle_mod):
         for k in ("dLdx0", "dLdctrl", "dLdparams"):
             if og[k] is not None:
                 assert _rel_grad_err(out[k].cpu().numpy(), og[k]).max() <= TOL_G64, k
+
+
+# ---- the CUDA path against what the mathematics fixes (independent of the oracle) ----------------------------------
+def test_gpu_closed_form_single_contact_and_free_flight(B):
+    """P1 on the CUDA path itself: one penalty contact without gravity is a damped oscillator with a closed-form release
+    time and rebound velocity; and a torque-free box keeps its world angular momentum and kinetic energy."""
+    import torch
+    from test_oracle_contact import _closed_form_bounce
+    dbar, tc, rho, T = 0.9, 0.004, 0.1, 0.5
+    w = W.ball_drop(nenv=4, gravity=0.0, solref=(tc, 1.0), solimp=(dbar, dbar, 0.001, 0.5, 2.0))
+    m = B.Model(w["model"])
+    opts = W.default_opts(W.DOPRI5, 1e-11, 1e-11, h0=1e-3)
+    x0 = np.array([[0.35, -1.7], [0.5, -2.2], [0.2, -0.9], [0.6, -3.0]])
+    xT = m.rollout(m.dev(x0), None, 0, 0.0, None, T, opts).cpu().numpy()
+    for i in range(4):
+        zT, trel, vrel = _closed_form_bounce(x0[i, 0], x0[i, 1], T, rho, dbar, tc)
+        assert abs(xT[i, 0] - zT) < 5e-9 and abs(xT[i, 1] - vrel) < 5e-8
+    # free flight of an asymmetric box: L_world = R I_body w_body and T = 1/2 m v^2 + 1/2 w.I w are invariants
+    model = H.free_box(gravity=(0, 0, 0))
+    mb = B.Model(model)
+    rng = np.random.default_rng(2)
+    n = 6
+    x0 = np.zeros((n, 13)); x0[:, 2] = 0.5
+    for i in range(n):
+        x0[i, 3:7] = H.rand_quat(rng)
+    x0[:, 7:10] = rng.normal(size=(n, 3)); x0[:, 10:13] = 3 * rng.normal(size=(n, 3))
+    xT = mb.rollout(mb.dev(x0), None, 0, 0.0, None, 1.0, W.default_opts(W.TSIT5, 1e-10, 1e-10)).cpu().numpy()
+    mass = float(model["body_mass"][1]); Ib = mass * np.asarray(model["body_inertia_unit"])[3:6]
+
+    def rot(q):
+        w_, x, y, z = q
+        return np.array([[1 - 2 * (y * y + z * z), 2 * (x * y - w_ * z), 2 * (x * z + w_ * y)],
+                         [2 * (x * y + w_ * z), 1 - 2 * (x * x + z * z), 2 * (y * z - w_ * x)],
+                         [2 * (x * z - w_ * y), 2 * (y * z + w_ * x), 1 - 2 * (x * x + y * y)]])
+    for a, b in zip(x0, xT):
+        La, Lb = rot(a[3:7]) @ (Ib * a[10:13]), rot(b[3:7]) @ (Ib * b[10:13])
+        assert np.abs(La - Lb).max() < 1e-8 * max(1.0, np.abs(La).max())
+        assert abs((Ib * a[10:13] ** 2).sum() - (Ib * b[10:13] ** 2).sum()) < 1e-8
+        assert abs(np.linalg.norm(b[3:7]) - 1.0) < 1e-12
