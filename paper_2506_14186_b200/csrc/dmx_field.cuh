@@ -787,46 +787,150 @@ DMX_DI Dual<R> contact_term(const ModelDev<R>& m, const IN& in, const DWS& dws, 
   return acc;
 }
 
-// one lane, one direction: dS/d(direction) for a configuration dof (in.kind 0, dof d) or a parameter (in.kind 3).
-// ws: cooperative workspace holding the frames at acceleration x*; dws: this lane's tangent workspace.
-// Configuration dof: tangent kinematics over the subtree below the dof, wrenches of those bodies, rows touching
-// them.  Body mass: that body's wrench only.  Pair parameter: that pair's rows only.  (One code path, so that
-// the body / row terms are emitted once.)
+// ---- configuration part, bodies: closed-form variation, cooperative over the (body, ancestor-dof) table -----------
+// For dof j with axis ax through o carried by the parent frame P of body(j) (free-joint rotation: P = world and the
+// anchor moves with the root origin), every material point x and vector of the subtree varies as
+//   dx = ax x (x-o),  dR = [ax]x R,  dOm = ax x (Om-Om_P),  dal = adot x (Om-Om_P) + ax x (al-al_P),
+//   dV(x) = adot x r + ax x (V(x)-odot),  da(x) = addot x r + 2 adot x (V(x)-odot) + ax x (a(x)-oddot),
+// adot = Om_P x ax, addot = al_P x ax + Om_P x adot (the variation commutes with d/dt along theta_j(t)+eps); the
+// virtual fields under w follow the first-order rules with the w-twists.  Slide and free-translation dofs shift the
+// subtree.  Then dS_b = dvw.F + m vw.da_c + dow.N + ow.dN with dN from the rotated inertia.
+// Needs: frames at x* (ACC kinematics), ws.Fb = velw(com), ws.Nb = omegaw (vjp_velocity), ws.Iw.  Uses ws.Isub for
+// (F, N, a_com) per body and ws.tw for the per-entry contributions.  Writes qbar[j] = -(dS/dq_j) of the body part and
+// the PD term; the rows' part is added by the tangent lanes.
+template <class WS, class R, int G, class IN, class AOUT>
+DMX_D void vjp_config_bodies(const ModelDev<R>& m, const IN& in, const WS& ws, const AOUT& qbar, const Grp<G>& gr) {
+  typedef typename WS::S S;
+  const int nv = m.nv, nb = m.nbody;
+#pragma unroll 1
+  for (int b = 1 + gr.lane; b < nb; b += G) {
+    V3<S> Fb, Nb; M3<S> Iw;
+    body_wrench<WS, R, IN>(m, in, ws, b, Fb, Nb, Iw);
+    FrameT<S> f; f.p = ld3(ws.fp(), b); f.w = ld3(ws.fw(), b); f.al = ld3(ws.fal(), b); f.ap = ld3(ws.fap(), b);
+    st3(ws.Isub(), 3 * b, Fb); st3(ws.Isub(), 3 * b + 1, Nb); st3(ws.Isub(), 3 * b + 2, point_acc(f, ld3(ws.com(), b)));
+  }
+  gr.sync();
+#pragma unroll 1
+  for (int e = gr.lane; e < m.ntw; e += G) {
+    const int b = m.tw_body[e], j = m.tw_dof[e], jn = m.dof_jnt[j], jt = m.jnt_type[jn], bj = m.dof_body[j], par = m.body_parent[bj];
+    S z(0.0), contrib(0.0);
+    V3<S> z3 = mk3<S>(z, z, z);
+    if (!(jt == JNT_FREE && !m.dof_rot[j])) {
+      V3<S> ax = ld3(ws.dax(), j);
+      V3<S> OmP = z3, alP = z3, OmPw = z3, od = z3, odd = z3, odw = z3, o = ld3(ws.dan(), j);
+      if (jt == JNT_FREE) {
+        int va = m.jnt_vadr[jn];
+        od = ld3(ws.fvp(), bj); odd = ld3(ws.fap(), bj);
+        odw = mk3<S>(ws.kap()[va], ws.kap()[va + 1], ws.kap()[va + 2]);
+      } else {
+        FrameT<S> P; P.p = ld3(ws.fp(), par); P.w = ld3(ws.fw(), par); P.al = ld3(ws.fal(), par); P.vp = ld3(ws.fvp(), par); P.ap = ld3(ws.fap(), par);
+        OmP = P.w; alP = P.al;
+        od = point_vel(P, o); odd = point_acc(P, o);
+        if (par > 0) { OmPw = ld3(ws.Nb(), par); odw = ld3(ws.Fb(), par) + cross(OmPw, o - ld3(ws.com(), par)); }
+      }
+      V3<S> adot = cross(OmP, ax), adotw = cross(OmPw, ax);
+      V3<S> addot = cross(alP, ax) + cross(OmP, adot);
+      V3<S> F = ld3(ws.Isub(), 3 * b), N = ld3(ws.Isub(), 3 * b + 1), vw = ld3(ws.Fb(), b), ow = ld3(ws.Nb(), b);
+      S mass = in.p(b);
+      if (jt == JNT_SLIDE) contrib = dot(adotw, F) + mass * dot(vw, addot);
+      else {
+        V3<S> c = ld3(ws.com(), b), Om = ld3(ws.fw(), b), al = ld3(ws.fal(), b), ac = ld3(ws.Isub(), 3 * b + 2);
+        V3<S> rc = c - o, Vc = ld3(ws.fvp(), b) + cross(Om, c - ld3(ws.fp(), b));
+        M3<S> I = ld9(ws.Iw(), b);
+        V3<S> d_ow = cross(ax, ow - OmPw);
+        V3<S> d_vw = cross(adotw, rc) + cross(ax, vw - odw);
+        V3<S> d_ac = cross(addot, rc) + cross(adot, Vc - od) * S(2.0) + cross(ax, ac - odd);
+        V3<S> d_Om = cross(ax, Om - OmP);
+        V3<S> d_al = cross(adot, Om - OmP) + cross(ax, al - alP);
+        V3<S> IOm = I * Om;
+        V3<S> dI_al = cross(ax, I * al) - I * cross(ax, al), dI_Om = cross(ax, IOm) - I * cross(ax, Om);
+        V3<S> d_N = dI_al + I * d_al + cross(d_Om, IOm) + cross(Om, dI_Om + I * d_Om);
+        contrib = dot(d_vw, F) + mass * dot(vw, d_ac) + dot(d_ow, N) + dot(ow, d_N);
+      }
+    }
+    ws.tw()[3 * e] = contrib;
+  }
+  gr.sync();
+#pragma unroll 1
+  for (int j = gr.lane; j < nv; j += G) {
+    int bj = m.dof_body[j], jn = m.dof_jnt[j];
+    S acc(0.0);
+#pragma unroll 1
+    for (int t = m.sub_ptr[bj]; t < m.sub_ptr[bj + 1]; ++t) acc = acc + ws.tw()[3 * m.tw_idx[m.sub_body[t] * nv + j]];
+    if (m.jnt_type[jn] != JNT_FREE)
+      for (int i = 0; i < m.nu; ++i) if (m.act_type[i] == ACT_PD && m.act_jnt[i] == jn) acc = acc + ws.kap()[j] * S(m.act_kp[i]);
+    qbar[j] = -(double)acc;
+  }
+  gr.sync();
+}
+
+// body b's pose and the axes / anchors of its ancestor dofs in a lane's tangent workspace, with the closed-form
+// tangent along configuration dof d (zero when b is not below d; d < 0: no tangent)
+template <class R, class WS, class DWS>
+DMX_DI void lift_pose(const ModelDev<R>& m, const WS& ws, const DWS& dws, int b, int d) {
+  typedef Dual<R> S;
+  const int nv = m.nv;
+  const bool moves = d >= 0 && m.tw_idx[b * nv + d] >= 0;
+  int jt = -1, rot = 0;
+  V3<R> ax = mk3<R>(R(0), R(0), R(0)), o = ax;
+  if (moves) { jt = m.jnt_type[m.dof_jnt[d]]; rot = m.dof_rot[d]; ax = ld3(ws.dax(), d); o = ld3(ws.dan(), d); }
+  const bool turn = moves && rot;                 // hinge / free rotation: rigid rotation about (ax, o); else: shift by ax
+  V3<R> p = ld3(ws.fp(), b);
+  V3<R> dp = !moves ? mk3<R>(R(0), R(0), R(0)) : (turn ? cross(ax, p - o) : ax);
+  dws.fp()[3 * b] = S(p.x, dp.x); dws.fp()[3 * b + 1] = S(p.y, dp.y); dws.fp()[3 * b + 2] = S(p.z, dp.z);
+  M3<R> Rm = ld9(ws.fR(), b);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    V3<R> col = colv(Rm, k);
+    V3<R> dc = turn ? cross(ax, col) : mk3<R>(R(0), R(0), R(0));
+    dws.fR()[9 * b + k] = S(col.x, dc.x); dws.fR()[9 * b + 3 + k] = S(col.y, dc.y); dws.fR()[9 * b + 6 + k] = S(col.z, dc.z);
+  }
+#pragma unroll 1
+  for (int e = m.tw_ptr[b]; e < m.tw_ptr[b + 1]; ++e) {
+    int k = m.tw_dof[e];
+    V3<R> a = ld3(ws.dax(), k), an = ld3(ws.dan(), k);
+    V3<R> da = mk3<R>(R(0), R(0), R(0)), dan = da;
+    // dof k is carried along iff its body is below d; world-fixed free-translation axes never turn
+    if (moves && m.tw_idx[m.dof_body[k] * nv + d] >= 0) {
+      bool ktrans_free = m.jnt_type[m.dof_jnt[k]] == JNT_FREE && !m.dof_rot[k];
+      if (turn) { if (!ktrans_free) da = cross(ax, a); dan = cross(ax, an - o); }
+      else dan = ax;
+    }
+    dws.dax()[3 * k] = S(a.x, da.x); dws.dax()[3 * k + 1] = S(a.y, da.y); dws.dax()[3 * k + 2] = S(a.z, da.z);
+    dws.dan()[3 * k] = S(an.x, dan.x); dws.dan()[3 * k + 1] = S(an.y, dan.y); dws.dan()[3 * k + 2] = S(an.z, dan.z);
+  }
+  (void)jt;
+}
+
+// one lane, one direction.  Configuration dof d (in.kind 0): the rows' part of dS/dq_d, with the poses of the touched
+// bodies lifted with their closed-form tangents.  Parameter (in.kind 3): a body mass (that body's wrench) or a pair
+// parameter (that pair's rows), frames lifted without tangent.
 template <class R, class IN, class WS, class DWS>
 DMX_D R residual_tangent(const ModelDev<R>& m, const IN& in, const WS& ws, const DWS& dws, int d, bool cfd) {
   typedef Dual<R> S;
   const int nv = m.nv;
   S acc(R(0));
-  int b0 = -1, bm = -1, pr = -1, t0 = 0, t1 = 0;
-  if (in.kind == 0) { b0 = m.dof_body[d]; bm = m.body_parent[b0]; t0 = m.sub_ptr[b0]; t1 = m.sub_ptr[b0 + 1]; }
-  else if (in.idx < m.nbody) { bm = in.idx; t1 = bm > 0 ? 1 : 0; }
-  else pr = in.idx < m.p_solref ? in.idx - m.p_fric : (in.idx < m.p_solimp ? (in.idx - m.p_solref) / 2 : (in.idx - m.p_solimp) / 5);
-  if (bm >= 0) lift_body<R>(m, ws, dws, bm);
-#pragma unroll 1
-  for (int t = t0; t < t1; ++t) {
-    int b = b0 >= 0 ? m.sub_body[t] : bm;
-    if (b0 >= 0) body_kin<DWS, R, IN, true>(m, in, dws, b);
-    acc = acc + body_term<R>(m, in, dws, ws.kap(), b);
+  const bool isq = in.kind == 0;
+  int pr = -1;
+  if (!isq) {
+    if (in.idx < m.nbody) {
+      if (in.idx > 0) { lift_body<R>(m, ws, dws, in.idx); acc = body_term<R>(m, in, dws, ws.kap(), in.idx); }
+      return acc.d;
+    }
+    pr = in.idx < m.p_solref ? in.idx - m.p_fric : (in.idx < m.p_solimp ? (in.idx - m.p_solref) / 2 : (in.idx - m.p_solimp) / 5);
   }
-  if (b0 >= 0) {
-    int jn = m.dof_jnt[d];
-    if (m.jnt_type[jn] != JNT_FREE)
-      for (int i = 0; i < m.nu; ++i) if (m.act_type[i] == ACT_PD && m.act_jnt[i] == jn) acc = acc - S(ws.kap()[d]) * (S(m.act_kp[i]) * (in.u(i) - in.q(m.jnt_qadr[jn])));
-  }
-  if (bm > 0 && b0 < 0) return acc.d;
 #pragma unroll 1
   for (int c = 0; c < m.nc; ++c) {
     int n = ws.incl()[c];
     if (n == 0) continue;
     int b1 = m.ct_b1[c], b2 = m.ct_b2[c];
-    bool in1 = b0 >= 0 && m.tw_idx[b1 * nv + d] >= 0, in2 = b0 >= 0 && m.tw_idx[b2 * nv + d] >= 0;
-    if (b0 >= 0 ? !(in1 || in2) : m.ct_pair[c] != pr) continue;
+    if (isq ? !(m.tw_idx[b1 * nv + d] >= 0 || m.tw_idx[b2 * nv + d] >= 0) : m.ct_pair[c] != pr) continue;
     int r0 = ws.rowstart()[c];
     bool any = false;
     for (int e = 0; e < n; ++e) any = any || ws.active()[r0 + e];
     if (!any) continue;
 #pragma unroll 1
-    for (int k = 0; k < 2; ++k) if (!(k ? in2 : in1)) lift_body<R>(m, ws, dws, k ? b2 : b1);
+    for (int k = 0; k < 2; ++k) lift_pose<R>(m, ws, dws, k ? b2 : b1, isq ? d : -1);
     acc = acc + contact_term<R>(m, in, dws, ws.kap(), c, n, r0, ws.active(), cfd);
   }
   return acc.d;

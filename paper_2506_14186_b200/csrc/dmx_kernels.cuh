@@ -39,6 +39,8 @@ DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yq
   kinematics<Ws<R, ST>, R, G, InPlain<R, ST>, true>(m, in, ws, gr);
   DMX_TICK(gr, 11);
   phase_sync(8);
+  // q: bodies in closed form (cooperative), then the rows' part and the parameters by one tangent lane per direction
+  vjp_config_bodies<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, rk.qbar(), gr);
   const int ndir = (dbg & 1) ? 0 : nv + (want_p ? m.np : 0);
 #pragma unroll 1
   for (int d = gr.lane; d < ndir; d += G) {
@@ -46,7 +48,7 @@ DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yq
     if (d < nv) seed_direction<R, ST>(m, din, d);
     else { din.kind = 3; din.idx = d - nv; din.dq0 = din.dq1 = din.dq2 = din.dq3 = R(0); }
     double s = -(double)residual_tangent<R, InDual<R, ST>, Ws<R, ST>, Ws<Dual<R>, 32> >(m, din, ws, dws, d, cfd);
-    if (d < nv) rk.qbar()[d] = s; else rk.pbar()[d - nv] = s;
+    if (d < nv) rk.qbar()[d] += s; else rk.pbar()[d - nv] = s;
   }
   gr.sync();
   DMX_TICK(gr, 12);
