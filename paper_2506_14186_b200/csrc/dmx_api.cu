@@ -187,7 +187,8 @@ void make_layouts(const HostModel& h, WsLayout& wl, WsLayout& rwl, RkLayout& rl)
   take(wl.M, nv * nv); take(wl.Hc, nv * nv); take(wl.tau, nv); take(wl.c, nv); take(wl.a0, nv); take(wl.x, nv); take(wl.g, nv);
   take(wl.dl, nv); take(wl.Md, nv); take(wl.xa, nv); take(wl.kap, nv);
   take(wl.cr, nc); take(wl.cn, 3 * nc); take(wl.cpos, 3 * nc); take(wl.ct1, 3 * nc); take(wl.ct2, 3 * nc);
-  take(wl.cD, nc); take(wl.cpost, nc); take(wl.cbd, nc); take(wl.cmu, nc);
+  take(wl.cD, nc); take(wl.cpost, nc); take(wl.cbd, nc); take(wl.cmu, nc); take(wl.cdD, nc); take(wl.cdpost, nc);
+  take(wl.fox, 3 * nb); take(wl.fvx, 3 * nb);
   take(wl.J, nr * nv); take(wl.aref, nr); take(wl.D, nr); take(wl.s, nr); take(wl.pr, nr);
   wl.size = o;
   rl.Yqr = o; rl.Vr = o + nq; rl.rsize = nq + nv;
@@ -225,7 +226,8 @@ template <class R> void build_dev(const HostModel& h, Arena& ar, ModelDev<R>& m,
     return;
   }
   m.nbody = h.nbody; m.njnt = h.njnt; m.nq = h.nq; m.nv = h.nv; m.nu = h.nu; m.npair = h.npair; m.nc = h.nc; m.np = h.np;
-  m.nlevel = h.nlevel; m.ntw = h.ntw; m.nmp = h.nmp; m.nrmax = h.nrmax; m.newton_iters = h.newton_iters; m.ls_iters = h.ls_iters;
+  m.nlevel = h.nlevel; m.ntw = h.ntw; m.nmp = h.nmp; m.nrmax = h.nrmax;
+  m.npp = 0; for (int c = 0; c < h.nc; ++c) m.npp += h.ct_kind[c] == CK_POINT_POINT; m.newton_iters = h.newton_iters; m.ls_iters = h.ls_iters;
   m.p_fric = h.nbody; m.p_solref = h.nbody + h.npair; m.p_solimp = h.nbody + 3 * h.npair;
   for (int k = 0; k < 3; ++k) m.gravity[k] = (R)h.gravity[k];
   size_t k = 0;

@@ -808,6 +808,16 @@ DMX_D void vjp_config_bodies(const ModelDev<R>& m, const IN& in, const WS& ws, c
     body_wrench<WS, R, IN>(m, in, ws, b, Fb, Nb, Iw);
     FrameT<S> f; f.p = ld3(ws.fp(), b); f.w = ld3(ws.fw(), b); f.al = ld3(ws.fal(), b); f.ap = ld3(ws.fap(), b);
     st3(ws.Isub(), 3 * b, Fb); st3(ws.Isub(), 3 * b + 1, Nb); st3(ws.Isub(), 3 * b + 2, point_acc(f, ld3(ws.com(), b)));
+    S z(0.0);
+    V3<S> vx = mk3<S>(z, z, z), ox = vx;                // twist of the body under the joint rates x* (for J_i x*)
+#pragma unroll 1
+    for (int e = m.tw_ptr[b]; e < m.tw_ptr[b + 1]; ++e) {
+      int j = m.tw_dof[e];
+      S xj = ws.x()[j];
+      vx = vx + ld3(ws.tw(), e) * xj;
+      if (m.dof_rot[j]) ox = ox + ld3(ws.dax(), j) * xj;
+    }
+    st3(ws.fvx(), b, vx); st3(ws.fox(), b, ox);
   }
   gr.sync();
 #pragma unroll 1
@@ -860,6 +870,159 @@ DMX_D void vjp_config_bodies(const ModelDev<R>& m, const IN& in, const WS& ws, c
     if (m.jnt_type[jn] != JNT_FREE)
       for (int i = 0; i < m.nu; ++i) if (m.act_type[i] == ACT_PD && m.act_jnt[i] == jn) acc = acc + ws.kap()[j] * S(m.act_kp[i]);
     qbar[j] = -(double)acc;
+  }
+  gr.sync();
+}
+
+// ---- configuration part, point-plane rows: closed-form variation, cooperative over (candidate, ancestor-dof) ---
+// The plane is fixed; the point c2 is a material point of body2, pos = c2 - n (rho + r/2).  For y in {x*, v, w}:
+// J_e y = dir_e . V^y(pos), V^y(pos) = V^y(c2) + Om^y x (pos - c2), and the variations follow the rules above.
+// S_c = sum_{e in A} (J_e w) D(r) (J_e x* - post(r) + b J_e v).  Uses ws.J as the (candidate, dof) contribution
+// buffer.  Needs ws.fox / ws.fvx (x*-twists), ws.Fb / ws.Nb (w-twists), ws.active, frames at x*.
+template <class WS, class R, int G, class IN, class AOUT>
+DMX_D void vjp_config_planes(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, const AOUT& qbar, const Grp<G>& gr) {
+  typedef typename WS::S S;
+  const int nv = m.nv, nc = m.nc;
+#pragma unroll 1
+  for (int c = gr.lane; c < nc; c += G) {
+    if (ws.incl()[c] == 0 || m.ct_kind[c] != CK_POINT_PLANE) continue;
+    InDual<S, WS::ST> din; din.pa = in.pa; din.kind = -1; din.idx = -1;      // parameters without tangent; r carries the seed
+    Dual<S> Dw, post, bd, mu;
+    candidate_terms<Dual<S>, R, InDual<S, WS::ST> >(m, din, c, Dual<S>(ws.cr()[c], S(1.0)), cfd, Dw, post, bd, mu);
+    ws.cdD()[c] = Dw.d; ws.cdpost()[c] = post.d;
+  }
+  gr.sync();
+#pragma unroll 1
+  for (int it = gr.lane; it < nc * nv; it += G) {
+    const int c = it / nv, j = it - c * nv;
+    S contrib(0.0);
+    const int n = ws.incl()[c], b2 = m.ct_b2[c];
+    bool go = n > 0 && m.ct_kind[c] == CK_POINT_PLANE && m.tw_idx[b2 * nv + j] >= 0;
+    int r0 = 0;
+    if (go) { r0 = ws.rowstart()[c]; bool any = false; for (int e = 0; e < n; ++e) any = any || ws.active()[r0 + e]; go = any; }
+    if (go) {
+      const int jn = m.dof_jnt[j], jt = m.jnt_type[jn], bj = m.dof_body[j], par = m.body_parent[bj];
+      const bool turn = m.dof_rot[j] != 0;
+      S z(0.0);
+      V3<S> z3 = mk3<S>(z, z, z), ax = ld3(ws.dax(), j), o = ld3(ws.dan(), j);
+      // parent-side data of the dof for the three rate fields (x*, v, w)
+      V3<S> OmP[3] = {z3, z3, z3}, od[3] = {z3, z3, z3};
+      if (jt == JNT_FREE) {
+        int va = m.jnt_vadr[jn];
+        od[0] = mk3<S>(ws.x()[va], ws.x()[va + 1], ws.x()[va + 2]);
+        od[1] = ld3(ws.fvp(), bj);
+        od[2] = mk3<S>(ws.kap()[va], ws.kap()[va + 1], ws.kap()[va + 2]);
+      } else if (par > 0) {
+        V3<S> cp = ld3(ws.com(), par), ro = o - cp;
+        OmP[0] = ld3(ws.fox(), par); od[0] = ld3(ws.fvx(), par) + cross(OmP[0], ro);
+        OmP[1] = ld3(ws.fw(), par);  od[1] = ld3(ws.fvp(), par) + cross(OmP[1], o - ld3(ws.fp(), par));
+        OmP[2] = ld3(ws.Nb(), par);  od[2] = ld3(ws.Fb(), par) + cross(OmP[2], ro);
+      }
+      // geometry
+      V3<S> nrm = c3<S>(m.ct_n, c), t1 = c3<S>(m.ct_t1, c), t2 = c3<S>(m.ct_t2, c);
+      V3<S> pb = ld3(ws.fp(), b2), cb = ld3(ws.com(), b2);
+      V3<S> c2 = pb + ld9(ws.fR(), b2) * c3<S>(m.ct_p2, c);
+      S r = ws.cr()[c], rho2(m.ct_rho2[c]);
+      V3<S> pc = nrm * (-(rho2 + S(0.5) * r));                 // pos - c2
+      V3<S> dc2 = turn ? cross(ax, c2 - o) : ax;
+      if (jt == JNT_FREE && !turn) { }                          // free translation: pure shift (OmP = 0)
+      S dr = dot(nrm, dc2);
+      V3<S> dpc = nrm * (S(-0.5) * dr);
+      // body2 twists for the three fields, at c2
+      V3<S> Om[3] = {ld3(ws.fox(), b2), ld3(ws.fw(), b2), ld3(ws.Nb(), b2)};
+      V3<S> Vc[3] = {ld3(ws.fvx(), b2) + cross(Om[0], c2 - cb), ld3(ws.fvp(), b2) + cross(Om[1], c2 - pb), ld3(ws.Fb(), b2) + cross(Om[2], c2 - cb)};
+      V3<S> Vp[3], dVp[3];
+#pragma unroll
+      for (int y = 0; y < 3; ++y) {
+        V3<S> dV, dO;
+        if (turn) { dV = cross(cross(OmP[y], ax), c2 - o) + cross(ax, Vc[y] - od[y]); dO = cross(ax, Om[y] - OmP[y]); }
+        else { dV = cross(OmP[y], ax); dO = z3; }
+        Vp[y] = Vc[y] + cross(Om[y], pc);
+        dVp[y] = dV + cross(dO, pc) + cross(Om[y], dpc);
+      }
+      S D = ws.cD()[c], post = ws.cpost()[c], bd = ws.cbd()[c], mu = ws.cmu()[c], dD = ws.cdD()[c] * dr, dpost = ws.cdpost()[c] * dr;
+#pragma unroll 1
+      for (int e = 0; e < n; ++e) {
+        if (!ws.active()[r0 + e]) continue;
+        V3<S> dir = nrm;
+        if (n == 4) { S sg = (e & 1) ? -mu : mu; dir = nrm + (e < 2 ? t1 : t2) * sg; }
+        S JX = dot(dir, Vp[0]), JV = dot(dir, Vp[1]), JW = dot(dir, Vp[2]);
+        S dJX = dot(dir, dVp[0]), dJV = dot(dir, dVp[1]), dJW = dot(dir, dVp[2]);
+        S s = JX - post + bd * JV;
+        contrib = contrib + dJW * D * s + JW * dD * s + JW * D * (dJX - dpost + bd * dJV);
+      }
+    }
+    ws.J()[it] = contrib;
+  }
+  gr.sync();
+#pragma unroll 1
+  for (int j = gr.lane; j < nv; j += G) {
+    S acc(0.0);
+#pragma unroll 1
+    for (int c = 0; c < nc; ++c) acc = acc + ws.J()[c * nv + j];
+    qbar[j] = qbar[j] - (double)acc;
+  }
+  gr.sync();
+}
+
+// ---- parameter part, closed form: S is linear in each body mass (dS/dm_b = S_b / m_b) and depends on a pair's
+// friction / solref / solimp only through the scalars (D, position term, b, mu) of that pair's candidates; the row
+// velocities J_e y come from the bodies' twists at the stored contact points.  One lane per body, then per
+// (pair, parameter slot).  Needs what vjp_config_bodies left in ws (F, N in ws.Isub; twists).
+template <class WS, class R, int G, class IN, class AOUT>
+DMX_D void vjp_params(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, const AOUT& pbar, const Grp<G>& gr) {
+  typedef typename WS::S S;
+  const int nc = m.nc;
+#pragma unroll 1
+  for (int b = gr.lane; b < m.nbody; b += G) {
+    S g(0.0);
+    if (b > 0) g = (dot(ld3(ws.Fb(), b), ld3(ws.Isub(), 3 * b)) + dot(ld3(ws.Nb(), b), ld3(ws.Isub(), 3 * b + 1))) / in.p(b);
+    pbar[b] = -(double)g;
+  }
+#pragma unroll 1
+  for (int it = gr.lane; it < 8 * m.npair; it += G) {
+    const int pr = it >> 3, k = it & 7;
+    const int ip = k == 0 ? m.p_fric + pr : (k < 3 ? m.p_solref + 2 * pr + (k - 1) : m.p_solimp + 5 * pr + (k - 3));
+    S acc(0.0);
+#pragma unroll 1
+    for (int c = 0; c < nc; ++c) {
+      const int n = ws.incl()[c];
+      if (n == 0 || m.ct_pair[c] != pr) continue;
+      const int r0 = ws.rowstart()[c];
+      bool any = false;
+      for (int e = 0; e < n; ++e) any = any || ws.active()[r0 + e];
+      if (!any) continue;
+      S z(0.0);
+      V3<S> pos = ld3(ws.cpos(), c), dX = mk3<S>(z, z, z), dV = dX, dW = dX;
+#pragma unroll 1
+      for (int side = 0; side < 2; ++side) {
+        const int b = side ? m.ct_b2[c] : m.ct_b1[c];
+        if (b == 0) continue;
+        S sg = side ? S(1.0) : S(-1.0);
+        V3<S> rc = pos - ld3(ws.com(), b);
+        dX = dX + (ld3(ws.fvx(), b) + cross(ld3(ws.fox(), b), rc)) * sg;
+        dV = dV + (ld3(ws.fvp(), b) + cross(ld3(ws.fw(), b), pos - ld3(ws.fp(), b))) * sg;
+        dW = dW + (ld3(ws.Fb(), b) + cross(ld3(ws.Nb(), b), rc)) * sg;
+      }
+      V3<S> nrm = ld3(ws.cn(), c), t1 = ld3(ws.ct1(), c), t2 = ld3(ws.ct2(), c);
+      InDual<S, WS::ST> din; din.pa = in.pa; din.kind = 3; din.idx = ip;
+      Dual<S> Dw, post, bd, mu;
+      candidate_terms<Dual<S>, R, InDual<S, WS::ST> >(m, din, c, Dual<S>(ws.cr()[c]), cfd, Dw, post, bd, mu);
+      S nX = dot(nrm, dX), nV = dot(nrm, dV), nW = dot(nrm, dW);
+      S tX[2] = {dot(t1, dX), dot(t2, dX)}, tV[2] = {dot(t1, dV), dot(t2, dV)}, tW[2] = {dot(t1, dW), dot(t2, dW)};
+#pragma unroll 1
+      for (int e = 0; e < n; ++e) {
+        if (!ws.active()[r0 + e]) continue;
+        Dual<S> JX(nX), JV(nV), JW(nW);
+        if (n == 4) {
+          Dual<S> sg = (e & 1) ? -mu : mu;
+          int a = e >> 1;
+          JX = JX + sg * Dual<S>(tX[a]); JV = JV + sg * Dual<S>(tV[a]); JW = JW + sg * Dual<S>(tW[a]);
+        }
+        acc = acc + (JW * (Dw * (JX - (post - bd * JV)))).d;
+      }
+    }
+    pbar[ip] = -(double)acc;
   }
   gr.sync();
 }
@@ -924,7 +1087,7 @@ DMX_D R residual_tangent(const ModelDev<R>& m, const IN& in, const WS& ws, const
     int n = ws.incl()[c];
     if (n == 0) continue;
     int b1 = m.ct_b1[c], b2 = m.ct_b2[c];
-    if (isq ? !(m.tw_idx[b1 * nv + d] >= 0 || m.tw_idx[b2 * nv + d] >= 0) : m.ct_pair[c] != pr) continue;
+    if (isq ? (m.ct_kind[c] == CK_POINT_PLANE || !(m.tw_idx[b1 * nv + d] >= 0 || m.tw_idx[b2 * nv + d] >= 0)) : m.ct_pair[c] != pr) continue;   // q: point-plane rows are done in closed form
     int r0 = ws.rowstart()[c];
     bool any = false;
     for (int e = 0; e < n; ++e) any = any || ws.active()[r0 + e];

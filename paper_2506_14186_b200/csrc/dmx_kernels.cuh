@@ -41,14 +41,15 @@ DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yq
   phase_sync(8);
   // q: bodies in closed form (cooperative), then the rows' part and the parameters by one tangent lane per direction
   vjp_config_bodies<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, rk.qbar(), gr);
-  const int ndir = (dbg & 1) ? 0 : nv + (want_p ? m.np : 0);
+  vjp_config_planes<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.qbar(), gr);
+  if (want_p) vjp_params<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.pbar(), gr);
+  // sphere-sphere rows: one tangent lane per configuration dof (closed-form pose tangents, Dual row terms)
+  const int ndir = ((dbg & 1) || m.npp == 0) ? 0 : nv;
 #pragma unroll 1
   for (int d = gr.lane; d < ndir; d += G) {
     InDual<R, ST> din; din.qa = Yqr; din.va = Vr; din.aa = ws.x(); din.ua = u; din.pa = p;
-    if (d < nv) seed_direction<R, ST>(m, din, d);
-    else { din.kind = 3; din.idx = d - nv; din.dq0 = din.dq1 = din.dq2 = din.dq3 = R(0); }
-    double s = -(double)residual_tangent<R, InDual<R, ST>, Ws<R, ST>, Ws<Dual<R>, 32> >(m, din, ws, dws, d, cfd);
-    if (d < nv) rk.qbar()[d] += s; else rk.pbar()[d - nv] = s;
+    seed_direction<R, ST>(m, din, d);
+    rk.qbar()[d] -= (double)residual_tangent<R, InDual<R, ST>, Ws<R, ST>, Ws<Dual<R>, 32> >(m, din, ws, dws, d, cfd);
   }
   gr.sync();
   DMX_TICK(gr, 12);

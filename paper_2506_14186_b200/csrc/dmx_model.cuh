@@ -11,7 +11,7 @@ enum { CK_POINT_PLANE = 0, CK_POINT_POINT = 1 };
 
 // Constants in the model's real type R (double or float); all pointers are device pointers.
 template <class R> struct ModelDev {
-  int nbody, njnt, nq, nv, nu, npair, nc, np, nlevel, ntw, nmp, nrmax;
+  int nbody, njnt, nq, nv, nu, npair, nc, np, nlevel, ntw, nmp, nrmax, npp /* point-point candidates */;
   int newton_iters, ls_iters;
   int p_fric, p_solref, p_solimp;          // offsets in the parameter vector (mass at 0)
   // tree
@@ -43,6 +43,8 @@ struct WsLayout {
   int Fb, Nb, Iw, Isub, tw;                           // body wrenches, world inertias, twist table
   int M, Hc, tau, c, a0, x, g, dl, Md, xa, kap;       // dynamics and Newton vectors
   int cr, cn, cpos, ct1, ct2, cD, cpost, cbd, cmu;    // per candidate
+  int cdD, cdpost;                                    // per candidate: dD/dr, d(position term)/dr (VJP)
+  int fox, fvx;                                       // per body: twist under the joint rates x* (angular, velocity of the COM)
   int J, aref, D, s, pr;                              // per row
   int size;                                           // scalars
   // int workspace (separate array)
@@ -59,7 +61,7 @@ template <class S_, int ST_> struct Ws {
   DMX_WS_ARR(fp) DMX_WS_ARR(fR) DMX_WS_ARR(fw) DMX_WS_ARR(fal) DMX_WS_ARR(fvp) DMX_WS_ARR(fap) DMX_WS_ARR(com) DMX_WS_ARR(dax) DMX_WS_ARR(dan)
   DMX_WS_ARR(Fb) DMX_WS_ARR(Nb) DMX_WS_ARR(Iw) DMX_WS_ARR(Isub) DMX_WS_ARR(tw)
   DMX_WS_ARR(M) DMX_WS_ARR(Hc) DMX_WS_ARR(tau) DMX_WS_ARR(c) DMX_WS_ARR(a0) DMX_WS_ARR(x) DMX_WS_ARR(g) DMX_WS_ARR(dl) DMX_WS_ARR(Md) DMX_WS_ARR(xa) DMX_WS_ARR(kap)
-  DMX_WS_ARR(cr) DMX_WS_ARR(cn) DMX_WS_ARR(cpos) DMX_WS_ARR(ct1) DMX_WS_ARR(ct2) DMX_WS_ARR(cD) DMX_WS_ARR(cpost) DMX_WS_ARR(cbd) DMX_WS_ARR(cmu)
+  DMX_WS_ARR(cr) DMX_WS_ARR(cn) DMX_WS_ARR(cpos) DMX_WS_ARR(ct1) DMX_WS_ARR(ct2) DMX_WS_ARR(cD) DMX_WS_ARR(cpost) DMX_WS_ARR(cbd) DMX_WS_ARR(cmu) DMX_WS_ARR(cdD) DMX_WS_ARR(cdpost) DMX_WS_ARR(fox) DMX_WS_ARR(fvx)
   DMX_WS_ARR(J) DMX_WS_ARR(aref) DMX_WS_ARR(D) DMX_WS_ARR(s) DMX_WS_ARR(pr)
   DMX_WS_INT(incl) DMX_WS_INT(rowstart) DMX_WS_INT(rowcand) DMX_WS_INT(active)
 };
