@@ -370,6 +370,13 @@ DMX_DI void candidate_terms(const ModelDev<R>& m, const IN& in, int c, const S& 
   Dw = d / (Ahat * (S(1.0) - d));
 }
 
+// one shared copy of the tangent-scalar evaluation of the candidate terms (impedance spline, softplus: large code)
+template <class R, class IN>
+__device__ __noinline__ void candidate_terms_dual(const ModelDev<R>& m, const IN& in, int c, Dual<R> r, bool cfd, Dual<R>& Dw, Dual<R>& post,
+                                                  Dual<R>& bd, Dual<R>& mu) {
+  candidate_terms<Dual<R>, R, IN>(m, in, c, r, cfd, Dw, post, bd, mu);
+}
+
 // relative velocity of the contact point per unit rate of dof j, body2 minus body1
 template <class WS, class R>
 DMX_DI V3<typename WS::S> rel_twist(const ModelDev<R>& m, const WS& ws, int j, int b1, int b2, const V3<typename WS::S>& pos) {
@@ -711,43 +718,6 @@ DMX_D void vjp_velocity(const ModelDev<R>& m, const IN& in, const WS& ws, int nr
   gr.sync();
 }
 
-// copy body b's frame and the axes / anchors of its ancestor dofs from the cooperative workspace (values at
-// acceleration x*) into a lane's tangent workspace, with zero tangent
-template <class R, class WS, class DWS>
-DMX_DI void lift_body(const ModelDev<R>& m, const WS& ws, const DWS& dws, int b) {
-  typedef Dual<R> S;
-#pragma unroll 1
-  for (int k = 0; k < 3; ++k) {
-    dws.fp()[3 * b + k] = S(ws.fp()[3 * b + k]); dws.fw()[3 * b + k] = S(ws.fw()[3 * b + k]); dws.fal()[3 * b + k] = S(ws.fal()[3 * b + k]);
-    dws.fvp()[3 * b + k] = S(ws.fvp()[3 * b + k]); dws.fap()[3 * b + k] = S(ws.fap()[3 * b + k]); dws.com()[3 * b + k] = S(ws.com()[3 * b + k]);
-  }
-#pragma unroll 1
-  for (int k = 0; k < 9; ++k) dws.fR()[9 * b + k] = S(ws.fR()[9 * b + k]);
-#pragma unroll 1
-  for (int e = m.tw_ptr[b]; e < m.tw_ptr[b + 1]; ++e) {
-    int j = m.tw_dof[e];
-#pragma unroll 1
-    for (int k = 0; k < 3; ++k) { dws.dax()[3 * j + k] = S(ws.dax()[3 * j + k]); dws.dan()[3 * j + k] = S(ws.dan()[3 * j + k]); }
-  }
-}
-// velw(com_b).F_b + omegaw(b).N_b in the tangent workspace
-template <class R, class IN, class DWS, class AW>
-DMX_DI Dual<R> body_term(const ModelDev<R>& m, const IN& in, const DWS& dws, const AW& w, int b) {
-  typedef Dual<R> S;
-  V3<S> Fb, Nb; M3<S> Iw;
-  body_wrench<DWS, R, IN>(m, in, dws, b, Fb, Nb, Iw);
-  V3<S> comb = ld3(dws.com(), b);
-  S z(R(0));
-  V3<S> vw = mk3<S>(z, z, z), ow = vw;
-#pragma unroll 1
-  for (int e = m.tw_ptr[b]; e < m.tw_ptr[b + 1]; ++e) {
-    int j = m.tw_dof[e], rot = m.dof_rot[j];
-    S wj(w[j]);
-    vw = vw + twist_lin(dws, j, rot, comb) * wj;
-    if (rot) ow = ow + ld3(dws.dax(), j) * wj;
-  }
-  return dot(vw, Fb) + dot(ow, Nb);
-}
 // sum over the active rows of candidate c of (J_i w) D_i (J_i x* - aref_i) in the tangent workspace
 template <class R, class IN, class DWS, class AW, class AI>
 DMX_DI Dual<R> contact_term(const ModelDev<R>& m, const IN& in, const DWS& dws, const AW& w, int c, int n, int r0, const AI& active, bool cfd) {
@@ -755,7 +725,7 @@ DMX_DI Dual<R> contact_term(const ModelDev<R>& m, const IN& in, const DWS& dws, 
   const int nv = m.nv;
   GeoT<S> g = collide<DWS, R>(m, dws, c);
   S Dw, post, bd, mu;
-  candidate_terms<S, R, IN>(m, in, c, g.r, cfd, Dw, post, bd, mu);
+  candidate_terms_dual<R, IN>(m, in, c, g.r, cfd, Dw, post, bd, mu);
   S z(R(0));
   S nX = z, t1X = z, t2X = z, nV = z, t1V = z, t2V = z, nW = z, t1W = z, t2W = z;
   int b1 = m.ct_b1[c], b2 = m.ct_b2[c];
@@ -888,7 +858,7 @@ DMX_D void vjp_config_planes(const ModelDev<R>& m, const IN& in, const WS& ws, b
     if (ws.incl()[c] == 0 || m.ct_kind[c] != CK_POINT_PLANE) continue;
     InDual<S, WS::ST> din; din.pa = in.pa; din.kind = -1; din.idx = -1;      // parameters without tangent; r carries the seed
     Dual<S> Dw, post, bd, mu;
-    candidate_terms<Dual<S>, R, InDual<S, WS::ST> >(m, din, c, Dual<S>(ws.cr()[c], S(1.0)), cfd, Dw, post, bd, mu);
+    candidate_terms_dual<R, InDual<S, WS::ST> >(m, din, c, Dual<S>(ws.cr()[c], S(1.0)), cfd, Dw, post, bd, mu);
     ws.cdD()[c] = Dw.d; ws.cdpost()[c] = post.d;
   }
   gr.sync();
@@ -1007,7 +977,7 @@ DMX_D void vjp_params(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
       V3<S> nrm = ld3(ws.cn(), c), t1 = ld3(ws.ct1(), c), t2 = ld3(ws.ct2(), c);
       InDual<S, WS::ST> din; din.pa = in.pa; din.kind = 3; din.idx = ip;
       Dual<S> Dw, post, bd, mu;
-      candidate_terms<Dual<S>, R, InDual<S, WS::ST> >(m, din, c, Dual<S>(ws.cr()[c]), cfd, Dw, post, bd, mu);
+      candidate_terms_dual<R, InDual<S, WS::ST> >(m, din, c, Dual<S>(ws.cr()[c]), cfd, Dw, post, bd, mu);
       S nX = dot(nrm, dX), nV = dot(nrm, dV), nW = dot(nrm, dW);
       S tX[2] = {dot(t1, dX), dot(t2, dX)}, tV[2] = {dot(t1, dV), dot(t2, dV)}, tW[2] = {dot(t1, dW), dot(t2, dW)};
 #pragma unroll 1
@@ -1065,35 +1035,25 @@ DMX_DI void lift_pose(const ModelDev<R>& m, const WS& ws, const DWS& dws, int b,
   (void)jt;
 }
 
-// one lane, one direction.  Configuration dof d (in.kind 0): the rows' part of dS/dq_d, with the poses of the touched
-// bodies lifted with their closed-form tangents.  Parameter (in.kind 3): a body mass (that body's wrench) or a pair
-// parameter (that pair's rows), frames lifted without tangent.
+// one lane, one configuration dof d: the sphere-sphere rows' part of dS/dq_d, with the poses of the two bodies lifted
+// with their closed-form tangents (point-plane rows, bodies and parameters are handled in closed form above).
 template <class R, class IN, class WS, class DWS>
 DMX_D R residual_tangent(const ModelDev<R>& m, const IN& in, const WS& ws, const DWS& dws, int d, bool cfd) {
   typedef Dual<R> S;
   const int nv = m.nv;
   S acc(R(0));
-  const bool isq = in.kind == 0;
-  int pr = -1;
-  if (!isq) {
-    if (in.idx < m.nbody) {
-      if (in.idx > 0) { lift_body<R>(m, ws, dws, in.idx); acc = body_term<R>(m, in, dws, ws.kap(), in.idx); }
-      return acc.d;
-    }
-    pr = in.idx < m.p_solref ? in.idx - m.p_fric : (in.idx < m.p_solimp ? (in.idx - m.p_solref) / 2 : (in.idx - m.p_solimp) / 5);
-  }
 #pragma unroll 1
   for (int c = 0; c < m.nc; ++c) {
     int n = ws.incl()[c];
-    if (n == 0) continue;
+    if (n == 0 || m.ct_kind[c] == CK_POINT_PLANE) continue;
     int b1 = m.ct_b1[c], b2 = m.ct_b2[c];
-    if (isq ? (m.ct_kind[c] == CK_POINT_PLANE || !(m.tw_idx[b1 * nv + d] >= 0 || m.tw_idx[b2 * nv + d] >= 0)) : m.ct_pair[c] != pr) continue;   // q: point-plane rows are done in closed form
+    if (!(m.tw_idx[b1 * nv + d] >= 0 || m.tw_idx[b2 * nv + d] >= 0)) continue;
     int r0 = ws.rowstart()[c];
     bool any = false;
     for (int e = 0; e < n; ++e) any = any || ws.active()[r0 + e];
     if (!any) continue;
 #pragma unroll 1
-    for (int k = 0; k < 2; ++k) lift_pose<R>(m, ws, dws, k ? b2 : b1, isq ? d : -1);
+    for (int k = 0; k < 2; ++k) lift_pose<R>(m, ws, dws, k ? b2 : b1, d);
     acc = acc + contact_term<R>(m, in, dws, ws.kap(), c, n, r0, ws.active(), cfd);
   }
   return acc.d;
