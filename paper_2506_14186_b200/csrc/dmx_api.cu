@@ -182,7 +182,7 @@ void make_layouts(const HostModel& h, WsLayout& wl, WsLayout& rwl, RkLayout& rl)
   auto take = [&](int& f, int n) { f = o; o += n; };
   take(wl.fp, 3 * nb); take(wl.fR, 9 * nb); take(wl.fw, 3 * nb); take(wl.fal, 3 * nb); take(wl.fvp, 3 * nb); take(wl.fap, 3 * nb);
   take(wl.com, 3 * nb); take(wl.dax, 3 * nv); take(wl.dan, 3 * nv);
-  rwl = wl; rwl.size = o;                                  // the tangent pass needs the frames only
+  rwl = wl; rwl.size = 0;                                  // no per-lane tangent workspace any more (closed-form VJP)
   take(wl.Fb, 3 * nb); take(wl.Nb, 3 * nb); take(wl.Iw, 9 * nb); take(wl.Isub, 9 * nb); take(wl.tw, 3 * std::max(h.ntw, 1));
   take(wl.M, nv * nv); take(wl.Hc, nv * nv); take(wl.tau, nv); take(wl.c, nv); take(wl.a0, nv); take(wl.x, nv); take(wl.g, nv);
   take(wl.dl, nv); take(wl.Md, nv); take(wl.xa, nv); take(wl.kap, nv);

@@ -718,45 +718,6 @@ DMX_D void vjp_velocity(const ModelDev<R>& m, const IN& in, const WS& ws, int nr
   gr.sync();
 }
 
-// sum over the active rows of candidate c of (J_i w) D_i (J_i x* - aref_i) in the tangent workspace
-template <class R, class IN, class DWS, class AW, class AI>
-DMX_DI Dual<R> contact_term(const ModelDev<R>& m, const IN& in, const DWS& dws, const AW& w, int c, int n, int r0, const AI& active, bool cfd) {
-  typedef Dual<R> S;
-  const int nv = m.nv;
-  GeoT<S> g = collide<DWS, R>(m, dws, c);
-  S Dw, post, bd, mu;
-  candidate_terms_dual<R, IN>(m, in, c, g.r, cfd, Dw, post, bd, mu);
-  S z(R(0));
-  S nX = z, t1X = z, t2X = z, nV = z, t1V = z, t2V = z, nW = z, t1W = z, t2W = z;
-  int b1 = m.ct_b1[c], b2 = m.ct_b2[c];
-#pragma unroll 1
-  for (int j = 0; j < nv; ++j) {
-    if (m.tw_idx[b2 * nv + j] < 0 && m.tw_idx[b1 * nv + j] < 0) continue;
-    V3<S> d = rel_twist<DWS, R>(m, dws, j, b1, b2, g.pos);
-    S nd = dot(g.n, d);
-    S xj = in.a(j), vj = in.v(j), wj(w[j]);
-    nX = nX + nd * xj; nV = nV + nd * vj; nW = nW + nd * wj;
-    if (n == 4) {
-      S t1d = dot(g.t1, d), t2d = dot(g.t2, d);
-      t1X = t1X + t1d * xj; t1V = t1V + t1d * vj; t1W = t1W + t1d * wj;
-      t2X = t2X + t2d * xj; t2V = t2V + t2d * vj; t2W = t2W + t2d * wj;
-    }
-  }
-  S acc = z;
-#pragma unroll 1
-  for (int e = 0; e < n; ++e) {
-    if (!active[r0 + e]) continue;
-    S JX = nX, JV = nV, JW = nW;
-    if (n == 4) {
-      S sg = (e & 1) ? -mu : mu;
-      if (e < 2) { JX = JX + sg * t1X; JV = JV + sg * t1V; JW = JW + sg * t1W; }
-      else { JX = JX + sg * t2X; JV = JV + sg * t2V; JW = JW + sg * t2W; }
-    }
-    acc = acc + JW * (Dw * (JX - (post - bd * JV)));
-  }
-  return acc;
-}
-
 // ---- configuration part, bodies: closed-form variation, cooperative over the (body, ancestor-dof) table -----------
 // For dof j with axis ax through o carried by the parent frame P of body(j) (free-joint rotation: P = world and the
 // anchor moves with the root origin), every material point x and vector of the subtree varies as
@@ -844,18 +805,20 @@ DMX_D void vjp_config_bodies(const ModelDev<R>& m, const IN& in, const WS& ws, c
   gr.sync();
 }
 
-// ---- configuration part, point-plane rows: closed-form variation, cooperative over (candidate, ancestor-dof) ---
-// The plane is fixed; the point c2 is a material point of body2, pos = c2 - n (rho + r/2).  For y in {x*, v, w}:
-// J_e y = dir_e . V^y(pos), V^y(pos) = V^y(c2) + Om^y x (pos - c2), and the variations follow the rules above.
-// S_c = sum_{e in A} (J_e w) D(r) (J_e x* - post(r) + b J_e v).  Uses ws.J as the (candidate, dof) contribution
-// buffer.  Needs ws.fox / ws.fvx (x*-twists), ws.Fb / ws.Nb (w-twists), ws.active, frames at x*.
-template <class WS, class R, int G, class IN, class AOUT>
-DMX_D void vjp_config_planes(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, const AOUT& qbar, const Grp<G>& gr) {
+// ---- configuration part, rows: closed-form variation, cooperative over (candidate, ancestor-dof) --------------
+// A candidate is a pair of material points c1 (body1; absent for a plane) and c2 (body2), pos on the mid-surface.
+// For y in {x*, v, w}: J_e y = dir_e . (V^y_2(pos) - V^y_1(pos)), V^y_b(pos) = V^y_b(c_b) + Om^y_b x (pos - c_b);
+// S_c = sum_{e in A} (J_e w) D(r) (J_e x* - post(r) + b J_e v).  Material points and twists of a body below dof j vary
+// by the rules above; r, n, the tangent frame and pos follow (sphere-sphere: n = (c2-c1)/|c2-c1|, Gram-Schmidt frame).
+// Uses ws.J as the (candidate, dof) contribution buffer.  Needs ws.fox / ws.fvx (x*-twists), ws.Fb / ws.Nb
+// (w-twists), ws.active, the frames at x*, and the candidate geometry stored by build_rows.
+template <bool PP, class WS, class R, int G, class IN, class AOUT>
+DMX_D void vjp_config_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, const AOUT& qbar, const Grp<G>& gr) {
   typedef typename WS::S S;
   const int nv = m.nv, nc = m.nc;
 #pragma unroll 1
   for (int c = gr.lane; c < nc; c += G) {
-    if (ws.incl()[c] == 0 || m.ct_kind[c] != CK_POINT_PLANE) continue;
+    if (ws.incl()[c] == 0 || (m.ct_kind[c] == CK_POINT_POINT) != PP) continue;
     InDual<S, WS::ST> din; din.pa = in.pa; din.kind = -1; din.idx = -1;      // parameters without tangent; r carries the seed
     Dual<S> Dw, post, bd, mu;
     candidate_terms_dual<R, InDual<S, WS::ST> >(m, din, c, Dual<S>(ws.cr()[c], S(1.0)), cfd, Dw, post, bd, mu);
@@ -866,58 +829,85 @@ DMX_D void vjp_config_planes(const ModelDev<R>& m, const IN& in, const WS& ws, b
   for (int it = gr.lane; it < nc * nv; it += G) {
     const int c = it / nv, j = it - c * nv;
     S contrib(0.0);
-    const int n = ws.incl()[c], b2 = m.ct_b2[c];
-    bool go = n > 0 && m.ct_kind[c] == CK_POINT_PLANE && m.tw_idx[b2 * nv + j] >= 0;
+    const int n = ws.incl()[c], b1 = m.ct_b1[c], b2 = m.ct_b2[c];
+    const bool in1 = b1 > 0 && m.tw_idx[b1 * nv + j] >= 0, in2 = b2 > 0 && m.tw_idx[b2 * nv + j] >= 0;
+    bool go = n > 0 && (in1 || in2) && (m.ct_kind[c] == CK_POINT_POINT) == PP;
     int r0 = 0;
     if (go) { r0 = ws.rowstart()[c]; bool any = false; for (int e = 0; e < n; ++e) any = any || ws.active()[r0 + e]; go = any; }
     if (go) {
       const int jn = m.dof_jnt[j], jt = m.jnt_type[jn], bj = m.dof_body[j], par = m.body_parent[bj];
-      const bool turn = m.dof_rot[j] != 0;
+      const bool turn = m.dof_rot[j] != 0, pp = PP;
       S z(0.0);
       V3<S> z3 = mk3<S>(z, z, z), ax = ld3(ws.dax(), j), o = ld3(ws.dan(), j);
-      // parent-side data of the dof for the three rate fields (x*, v, w)
-      V3<S> OmP[3] = {z3, z3, z3}, od[3] = {z3, z3, z3};
+      V3<S> OmP[3] = {z3, z3, z3}, od[3] = {z3, z3, z3};      // parent-side data of the dof for the rate fields x*, v, w
       if (jt == JNT_FREE) {
         int va = m.jnt_vadr[jn];
         od[0] = mk3<S>(ws.x()[va], ws.x()[va + 1], ws.x()[va + 2]);
         od[1] = ld3(ws.fvp(), bj);
         od[2] = mk3<S>(ws.kap()[va], ws.kap()[va + 1], ws.kap()[va + 2]);
       } else if (par > 0) {
-        V3<S> cp = ld3(ws.com(), par), ro = o - cp;
+        V3<S> ro = o - ld3(ws.com(), par);
         OmP[0] = ld3(ws.fox(), par); od[0] = ld3(ws.fvx(), par) + cross(OmP[0], ro);
         OmP[1] = ld3(ws.fw(), par);  od[1] = ld3(ws.fvp(), par) + cross(OmP[1], o - ld3(ws.fp(), par));
         OmP[2] = ld3(ws.Nb(), par);  od[2] = ld3(ws.Fb(), par) + cross(OmP[2], ro);
       }
-      // geometry
-      V3<S> nrm = c3<S>(m.ct_n, c), t1 = c3<S>(m.ct_t1, c), t2 = c3<S>(m.ct_t2, c);
-      V3<S> pb = ld3(ws.fp(), b2), cb = ld3(ws.com(), b2);
-      V3<S> c2 = pb + ld9(ws.fR(), b2) * c3<S>(m.ct_p2, c);
-      S r = ws.cr()[c], rho2(m.ct_rho2[c]);
-      V3<S> pc = nrm * (-(rho2 + S(0.5) * r));                 // pos - c2
-      V3<S> dc2 = turn ? cross(ax, c2 - o) : ax;
-      if (jt == JNT_FREE && !turn) { }                          // free translation: pure shift (OmP = 0)
-      S dr = dot(nrm, dc2);
-      V3<S> dpc = nrm * (S(-0.5) * dr);
-      // body2 twists for the three fields, at c2
-      V3<S> Om[3] = {ld3(ws.fox(), b2), ld3(ws.fw(), b2), ld3(ws.Nb(), b2)};
-      V3<S> Vc[3] = {ld3(ws.fvx(), b2) + cross(Om[0], c2 - cb), ld3(ws.fvp(), b2) + cross(Om[1], c2 - pb), ld3(ws.Fb(), b2) + cross(Om[2], c2 - cb)};
-      V3<S> Vp[3], dVp[3];
+      // material points and their variations
+      V3<S> nrm = ld3(ws.cn(), c), t1 = ld3(ws.ct1(), c), t2 = ld3(ws.ct2(), c), pos = ld3(ws.cpos(), c);
+      S r = ws.cr()[c], rho1(m.ct_rho1[c]);
+      V3<S> c1 = z3, c2 = ld3(ws.fp(), b2) + ld9(ws.fR(), b2) * c3<S>(m.ct_p2, c);
+      if (pp) c1 = ld3(ws.fp(), b1) + ld9(ws.fR(), b1) * c3<S>(m.ct_p1, c);
+      V3<S> dc1 = in1 ? (turn ? cross(ax, c1 - o) : ax) : z3, dc2 = in2 ? (turn ? cross(ax, c2 - o) : ax) : z3;
+      // geometry: r, n, tangent frame, pos
+      S dr; V3<S> dn = z3, dt1 = z3, dt2 = z3, dpos;
+      if (!pp) { dr = dot(nrm, dc2); dpos = dc2 - nrm * (S(0.5) * dr); }
+      else {
+        S dist = r + rho1 + S(m.ct_rho2[c]);
+        V3<S> ddl = dc2 - dc1;
+        dr = dot(nrm, ddl);
+        dn = (ddl - nrm * dr) * (S(1.0) / dist);
+        dpos = dc1 + dn * (rho1 + S(0.5) * r) + nrm * (S(0.5) * dr);
+        typename RealOf<S>::type axn = fabs(val(nrm.x)), ayn = fabs(val(nrm.y)), azn = fabs(val(nrm.z));
+        int ei = 0; if (ayn < axn) { ei = 1; axn = ayn; } if (azn < axn) ei = 2;
+        S o1(1.0);
+        V3<S> ev = mk3<S>(ei == 0 ? o1 : z, ei == 1 ? o1 : z, ei == 2 ? o1 : z);
+        S en = dot(ev, nrm);
+        V3<S> t = ev - nrm * en;
+        S tl = m_sqrt(dot(t, t));
+        V3<S> dt = z3 - dn * en - nrm * dot(ev, dn);
+        dt1 = (dt - t1 * dot(t1, dt)) * (S(1.0) / tl);
+        dt2 = cross(dn, t1) + cross(nrm, dt1);
+      }
+      // relative velocities at pos under the three rate fields and their variations
+      V3<S> rel[3] = {z3, z3, z3}, drel[3] = {z3, z3, z3};
+#pragma unroll 1
+      for (int side = PP ? 0 : 1; side < 2; ++side) {
+        const int b = side ? b2 : b1;
+        if (b == 0) continue;
+        const bool ins = side ? in2 : in1;
+        V3<S> cs = side ? c2 : c1, dcs = side ? dc2 : dc1;
+        V3<S> pb = ld3(ws.fp(), b), cb = ld3(ws.com(), b), pc = pos - cs, dpc = dpos - dcs;
+        S sg = side ? S(1.0) : S(-1.0);
 #pragma unroll
-      for (int y = 0; y < 3; ++y) {
-        V3<S> dV, dO;
-        if (turn) { dV = cross(cross(OmP[y], ax), c2 - o) + cross(ax, Vc[y] - od[y]); dO = cross(ax, Om[y] - OmP[y]); }
-        else { dV = cross(OmP[y], ax); dO = z3; }
-        Vp[y] = Vc[y] + cross(Om[y], pc);
-        dVp[y] = dV + cross(dO, pc) + cross(Om[y], dpc);
+        for (int y = 0; y < 3; ++y) {
+          V3<S> Om = y == 0 ? ld3(ws.fox(), b) : (y == 1 ? ld3(ws.fw(), b) : ld3(ws.Nb(), b));
+          V3<S> Vc = y == 0 ? ld3(ws.fvx(), b) + cross(Om, cs - cb) : (y == 1 ? ld3(ws.fvp(), b) + cross(Om, cs - pb) : ld3(ws.Fb(), b) + cross(Om, cs - cb));
+          V3<S> dV = z3, dO = z3;
+          if (ins) {
+            if (turn) { dV = cross(cross(OmP[y], ax), cs - o) + cross(ax, Vc - od[y]); dO = cross(ax, Om - OmP[y]); }
+            else dV = cross(OmP[y], ax);
+          }
+          rel[y] = rel[y] + (Vc + cross(Om, pc)) * sg;
+          drel[y] = drel[y] + (dV + cross(dO, pc) + cross(Om, dpc)) * sg;
+        }
       }
       S D = ws.cD()[c], post = ws.cpost()[c], bd = ws.cbd()[c], mu = ws.cmu()[c], dD = ws.cdD()[c] * dr, dpost = ws.cdpost()[c] * dr;
 #pragma unroll 1
       for (int e = 0; e < n; ++e) {
         if (!ws.active()[r0 + e]) continue;
-        V3<S> dir = nrm;
-        if (n == 4) { S sg = (e & 1) ? -mu : mu; dir = nrm + (e < 2 ? t1 : t2) * sg; }
-        S JX = dot(dir, Vp[0]), JV = dot(dir, Vp[1]), JW = dot(dir, Vp[2]);
-        S dJX = dot(dir, dVp[0]), dJV = dot(dir, dVp[1]), dJW = dot(dir, dVp[2]);
+        V3<S> dir = nrm, ddir = dn;
+        if (n == 4) { S sg = (e & 1) ? -mu : mu; dir = nrm + (e < 2 ? t1 : t2) * sg; ddir = dn + (e < 2 ? dt1 : dt2) * sg; }
+        S JX = dot(dir, rel[0]), JV = dot(dir, rel[1]), JW = dot(dir, rel[2]);
+        S dJX = dot(ddir, rel[0]) + dot(dir, drel[0]), dJV = dot(ddir, rel[1]) + dot(dir, drel[1]), dJW = dot(ddir, rel[2]) + dot(dir, drel[2]);
         S s = JX - post + bd * JV;
         contrib = contrib + dJW * D * s + JW * dD * s + JW * D * (dJX - dpost + bd * dJV);
       }
@@ -995,89 +985,6 @@ DMX_D void vjp_params(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
     pbar[ip] = -(double)acc;
   }
   gr.sync();
-}
-
-// body b's pose and the axes / anchors of its ancestor dofs in a lane's tangent workspace, with the closed-form
-// tangent along configuration dof d (zero when b is not below d; d < 0: no tangent)
-template <class R, class WS, class DWS>
-DMX_DI void lift_pose(const ModelDev<R>& m, const WS& ws, const DWS& dws, int b, int d) {
-  typedef Dual<R> S;
-  const int nv = m.nv;
-  const bool moves = d >= 0 && m.tw_idx[b * nv + d] >= 0;
-  int jt = -1, rot = 0;
-  V3<R> ax = mk3<R>(R(0), R(0), R(0)), o = ax;
-  if (moves) { jt = m.jnt_type[m.dof_jnt[d]]; rot = m.dof_rot[d]; ax = ld3(ws.dax(), d); o = ld3(ws.dan(), d); }
-  const bool turn = moves && rot;                 // hinge / free rotation: rigid rotation about (ax, o); else: shift by ax
-  V3<R> p = ld3(ws.fp(), b);
-  V3<R> dp = !moves ? mk3<R>(R(0), R(0), R(0)) : (turn ? cross(ax, p - o) : ax);
-  dws.fp()[3 * b] = S(p.x, dp.x); dws.fp()[3 * b + 1] = S(p.y, dp.y); dws.fp()[3 * b + 2] = S(p.z, dp.z);
-  M3<R> Rm = ld9(ws.fR(), b);
-#pragma unroll
-  for (int k = 0; k < 3; ++k) {
-    V3<R> col = colv(Rm, k);
-    V3<R> dc = turn ? cross(ax, col) : mk3<R>(R(0), R(0), R(0));
-    dws.fR()[9 * b + k] = S(col.x, dc.x); dws.fR()[9 * b + 3 + k] = S(col.y, dc.y); dws.fR()[9 * b + 6 + k] = S(col.z, dc.z);
-  }
-#pragma unroll 1
-  for (int e = m.tw_ptr[b]; e < m.tw_ptr[b + 1]; ++e) {
-    int k = m.tw_dof[e];
-    V3<R> a = ld3(ws.dax(), k), an = ld3(ws.dan(), k);
-    V3<R> da = mk3<R>(R(0), R(0), R(0)), dan = da;
-    // dof k is carried along iff its body is below d; world-fixed free-translation axes never turn
-    if (moves && m.tw_idx[m.dof_body[k] * nv + d] >= 0) {
-      bool ktrans_free = m.jnt_type[m.dof_jnt[k]] == JNT_FREE && !m.dof_rot[k];
-      if (turn) { if (!ktrans_free) da = cross(ax, a); dan = cross(ax, an - o); }
-      else dan = ax;
-    }
-    dws.dax()[3 * k] = S(a.x, da.x); dws.dax()[3 * k + 1] = S(a.y, da.y); dws.dax()[3 * k + 2] = S(a.z, da.z);
-    dws.dan()[3 * k] = S(an.x, dan.x); dws.dan()[3 * k + 1] = S(an.y, dan.y); dws.dan()[3 * k + 2] = S(an.z, dan.z);
-  }
-  (void)jt;
-}
-
-// one lane, one configuration dof d: the sphere-sphere rows' part of dS/dq_d, with the poses of the two bodies lifted
-// with their closed-form tangents (point-plane rows, bodies and parameters are handled in closed form above).
-template <class R, class IN, class WS, class DWS>
-DMX_D R residual_tangent(const ModelDev<R>& m, const IN& in, const WS& ws, const DWS& dws, int d, bool cfd) {
-  typedef Dual<R> S;
-  const int nv = m.nv;
-  S acc(R(0));
-#pragma unroll 1
-  for (int c = 0; c < m.nc; ++c) {
-    int n = ws.incl()[c];
-    if (n == 0 || m.ct_kind[c] == CK_POINT_PLANE) continue;
-    int b1 = m.ct_b1[c], b2 = m.ct_b2[c];
-    if (!(m.tw_idx[b1 * nv + d] >= 0 || m.tw_idx[b2 * nv + d] >= 0)) continue;
-    int r0 = ws.rowstart()[c];
-    bool any = false;
-    for (int e = 0; e < n; ++e) any = any || ws.active()[r0 + e];
-    if (!any) continue;
-#pragma unroll 1
-    for (int k = 0; k < 2; ++k) lift_pose<R>(m, ws, dws, k ? b2 : b1, d);
-    acc = acc + contact_term<R>(m, in, dws, ws.kap(), c, n, r0, ws.active(), cfd);
-  }
-  return acc.d;
-}
-
-// tangent of q (+) eps e_d at eps = 0: fills the seed of an InDual
-template <class R, int ST>
-DMX_DI void seed_direction(const ModelDev<R>& m, InDual<R, ST>& in, int d) {
-  const int nv = m.nv;
-  in.dq0 = R(1); in.dq1 = in.dq2 = in.dq3 = R(0);
-  if (d < nv) {
-    in.kind = 0;
-    int j = m.dof_jnt[d], c = d - m.jnt_vadr[j], qa = m.jnt_qadr[j];
-    if (m.jnt_type[j] != JNT_FREE || c < 3) { in.idx = qa + c; return; }
-    in.idx = qa + 3;
-    R w0 = in.qa[qa + 3], w1 = in.qa[qa + 4], w2 = in.qa[qa + 5], w3 = in.qa[qa + 6];
-    R e0 = c == 3 ? R(0.5) : R(0), e1 = c == 4 ? R(0.5) : R(0), e2 = c == 5 ? R(0.5) : R(0);
-    in.dq0 = -w1 * e0 - w2 * e1 - w3 * e2;
-    in.dq1 = w0 * e0 + w2 * e2 - w3 * e1;
-    in.dq2 = w0 * e1 - w1 * e2 + w3 * e0;
-    in.dq3 = w0 * e2 + w1 * e1 - w2 * e0;
-  } else if (d < 2 * nv) { in.kind = 1; in.idx = d - nv; }
-  else if (d < 2 * nv + m.nu) { in.kind = 2; in.idx = d - 2 * nv; }
-  else { in.kind = 3; in.idx = d - 2 * nv - m.nu; }
 }
 
 }  // namespace dmx

@@ -41,16 +41,9 @@ DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yq
   phase_sync(8);
   // q: bodies in closed form (cooperative), then the rows' part and the parameters by one tangent lane per direction
   vjp_config_bodies<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, rk.qbar(), gr);
-  vjp_config_planes<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.qbar(), gr);
+  vjp_config_rows<false, Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.qbar(), gr);                 // point-plane rows
+  if (m.npp > 0) vjp_config_rows<true, Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.qbar(), gr);   // sphere-sphere rows
   if (want_p) vjp_params<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.pbar(), gr);
-  // sphere-sphere rows: one tangent lane per configuration dof (closed-form pose tangents, Dual row terms)
-  const int ndir = ((dbg & 1) || m.npp == 0) ? 0 : nv;
-#pragma unroll 1
-  for (int d = gr.lane; d < ndir; d += G) {
-    InDual<R, ST> din; din.qa = Yqr; din.va = Vr; din.aa = ws.x(); din.ua = u; din.pa = p;
-    seed_direction<R, ST>(m, din, d);
-    rk.qbar()[d] -= (double)residual_tangent<R, InDual<R, ST>, Ws<R, ST>, Ws<Dual<R>, 32> >(m, din, ws, dws, d, cfd);
-  }
   gr.sync();
   DMX_TICK(gr, 12);
   return true;
