@@ -254,7 +254,6 @@ struct dmx_model {
   void* rk_scratch = nullptr; size_t rk_scratch_bytes = 0;              // backward integrator arrays (global memory)
   int* queue = nullptr;            // [4] work-queue counters
   void* zero_u = nullptr;          // zeros: controls when ctrl == NULL, velocities at create
-  void* scratch = nullptr; size_t scratch_bytes = 0;   // tangent workspaces of the VJP lanes
 };
 
 namespace {
@@ -279,13 +278,6 @@ int ensure_scratch(dmx_model* m, int grid, int block, bool rk) {
       m->rk_scratch_bytes = need2;
     }
   }
-  size_t dual = 2 * rsize(m);
-  size_t need = (size_t)grid * (block / 32) * 32 * (size_t)m->rwl.size * dual;
-  if (need <= m->scratch_bytes) return 0;
-  if (m->scratch) cudaFree(m->scratch);
-  m->scratch = nullptr; m->scratch_bytes = 0;
-  CUDA_OK(cudaMalloc(&m->scratch, need));
-  m->scratch_bytes = need;
   return 0;
 }
 
@@ -402,12 +394,12 @@ int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const vo
   a.ctrl = (const R*)ctrl; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u; a.xT = (const R*)xT; a.dLdxT = (const R*)dLdxT;
   a.status = status; a.so = opts_of(opts); a.dLdx0 = (R*)dLdx0; a.dLdctrl = (R*)dLdctrl; a.dLdparams = (R*)dLdparams;
   { const char* e = std::getenv("DMX_LOCKSTEP_BWD"); a.lockstep = e ? std::atoi(e) : 0x1ff; }          // backward: fetch-bound, phases in lockstep (measured 1.6-2.2x)
-  a.queue = m->queue + 1; a.wl = m->wl; a.rwl = m->rwl; a.rl = m->rl; a.res_size = m->rwl.size;
+  a.queue = m->queue + 1; a.wl = m->wl; a.rl = m->rl;
   LaunchCfg c; c.block = m->cb.block; c.smem = m->cb.smem;
   int gpb = groups_per_block(m, c.block);
   c.grid = std::max(1, std::min(m->cb.occ * m->sm_count, (nenv + gpb - 1) / gpb));
   if (ensure_scratch(m, c.grid, c.block, true)) return -1;
-  a.scratch = (Dual<R>*)m->scratch; a.rk_scratch = (double*)m->rk_scratch;
+  a.rk_scratch = (double*)m->rk_scratch;
   CUDA_OK(cudaMemsetAsync(m->queue + 1, 0, sizeof(int), s));
   if (dLdctrl && nknot > 0 && m->h.nu > 0) CUDA_OK(cudaMemsetAsync(dLdctrl, 0, (size_t)nenv * nknot * m->h.nu * sizeof(R), s));
   CUDA_OK(launchers_for<R>(m->G).backward(dev_of<R>(m), a, c, s));
@@ -420,11 +412,10 @@ int field_typed(dmx_model* m, int n, const void* x, const void* u, const void* p
   FieldArgs<R> a; std::memset(&a, 0, sizeof(a));
   a.n = n; a.cfd = cfd; a.want_p = pbar != nullptr; a.x = (const R*)x; a.u = (const R*)u; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u;
   a.kappa = (const R*)kappa; a.acc = (R*)acc; a.nrow = nrow; a.qbar = (R*)qbar; a.vbar = (R*)vbar; a.ubar = (R*)ubar; a.pbar = (R*)pbar;
-  a.wl = m->wl; a.rwl = m->rwl; a.rl = m->rl; a.res_size = m->rwl.size;
+  a.wl = m->wl; a.rl = m->rl;
   LaunchCfg c; c.block = m->cx.block; c.smem = m->cx.smem;
   int gpb = groups_per_block(m, c.block);
   c.grid = std::max(1, std::min(m->cx.occ * m->sm_count, (n + gpb - 1) / gpb));
-  if (kappa) { if (ensure_scratch(m, c.grid, c.block, false)) return -1; a.scratch = (Dual<R>*)m->scratch; }
   CUDA_OK(launchers_for<R>(m->G).field(dev_of<R>(m), a, c, s));
   return 0;
 }
@@ -490,7 +481,6 @@ void dmx_model_destroy(dmx_model* m) {
   if (m->arena.dev) cudaFree(m->arena.dev);
   if (m->queue) cudaFree(m->queue);
   if (m->zero_u) cudaFree(m->zero_u);
-  if (m->scratch) cudaFree(m->scratch);
   if (m->rk_scratch) cudaFree(m->rk_scratch);
   delete m;
 }

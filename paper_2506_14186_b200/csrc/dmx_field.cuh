@@ -20,21 +20,11 @@ template <class R, int ST> struct InPlain {
   DMX_DI R u(int i) const { return ua[i]; }
   DMX_DI R p(int i) const { return pa[i]; }
 };
-// the same inputs carrying one tangent direction (kind 0: configuration, 1: velocity, 2: control,
-// 3: parameter); the acceleration argument (x*) is held fixed
+// parameters carrying one tangent direction (index idx; idx < 0: none), for the candidate scalars of the VJP
 template <class R, int ST> struct InDual {
   typedef Dual<R> S;
-  Arr<R, ST> qa, va, aa; const R* ua; const R* pa;
-  int kind, idx; R dq0, dq1, dq2, dq3;
-  DMX_DI S q(int i) const {
-    R t = R(0);
-    if (kind == 0) { int k = i - idx; t = k == 0 ? dq0 : (k == 1 ? dq1 : (k == 2 ? dq2 : (k == 3 ? dq3 : R(0)))); }
-    return S(qa[i], t);
-  }
-  DMX_DI S v(int i) const { return S(va[i], (kind == 1 && i == idx) ? R(1) : R(0)); }
-  DMX_DI S a(int i) const { return S(aa[i], R(0)); }
-  DMX_DI S u(int i) const { return S(ua[i], (kind == 2 && i == idx) ? R(1) : R(0)); }
-  DMX_DI S p(int i) const { return S(pa[i], (kind == 3 && i == idx) ? R(1) : R(0)); }
+  const R* pa; int kind, idx;
+  DMX_DI S p(int i) const { return S(pa[i], (i == idx) ? R(1) : R(0)); }
 };
 
 template <class S> struct FrameT { V3<S> p; M3<S> R; V3<S> w, al, vp, ap; };

@@ -7,11 +7,11 @@
 namespace dmx {
 
 // ---- S11/S12: (qbar,vbar,ubar,pbar) = kappa^T dF/d(q,v,u,p), F~ when cfd (Eq. 4) ----------
-// Cooperative solve for x*, the active set and w = H^-1 kappa; then one tangent direction per lane.
+// Cooperative solve for x*, the active set and w = H^-1 kappa; then the closed-form gradient of S (dmx_field.cuh).
 template <class R, int G>
 DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yqr, const Arr<R, StrideOf<G>::value>& Vr, const R* u, const R* p,
                       const Arr<double, StrideOf<G>::value>& kappa, bool cfd, bool want_p, const Ws<R, StrideOf<G>::value>& ws,
-                      const Ws<Dual<R>, 32>& dws, const Rk<StrideOf<G>::value>& rk, const Grp<G>& gr, int dbg = 0, const double* xk = nullptr) {
+                      const Rk<StrideOf<G>::value>& rk, const Grp<G>& gr, int dbg = 0, const double* xk = nullptr) {
   const int ST = StrideOf<G>::value;
   const int nv = m.nv;
   if (dbg & 4) return true;
@@ -57,18 +57,9 @@ template <class R> struct BackwardArgs {
   R *dLdx0, *dLdctrl, *dLdparams;
   const int* tape_hdr; const R* tape;
   int* queue;
-  Dual<R>* scratch; int res_size;
   double* rk_scratch;       // integrator / adjoint arrays of every resident group (global memory: touched once per stage)
-  WsLayout wl, rwl; RkLayout rl;
+  WsLayout wl; RkLayout rl;
 };
-
-template <class R>
-DMX_DI Ws<Dual<R>, 32> bind_scratch(Dual<R>* scratch, int res_size, const WsLayout* rwl) {
-  Ws<Dual<R>, 32> dws;
-  size_t gwarp = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  dws.b = scratch + gwarp * (size_t)res_size * 32 + (threadIdx.x & 31); dws.ib = nullptr; dws.L = rwl;
-  return dws;
-}
 
 // ---- S10: reverse sweep over the tape, frozen step sizes ---------------------------
 template <class R, int G>
@@ -76,7 +67,7 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
   if (threadIdx.x == 0) g_lockstep = a.lockstep;
-  load_cta_const<R>(cc, m_, a.wl, a.rwl, a.rl, 0);
+  load_cta_const<R>(cc, m_, a.wl, a.wl, a.rl, 0);
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
@@ -84,7 +75,6 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
   bind_shared<R, G>(smem, 0, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
   if (G == 1) rk.b = a.rk_scratch + ((size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32 * (size_t)a.rl.size_bwd + (threadIdx.x & 31);
   else rk.b = a.rk_scratch + ((size_t)blockIdx.x * (blockDim.x / G) + threadIdx.x / G) * (size_t)a.rl.size_bwd;
-  Ws<Dual<R>, 32> dws = bind_scratch<R>(a.scratch, a.res_size, &cc.rwl);
   const int nq = m.nq, nv = m.nv, nu = m.nu, np = m.np, nx = nq + nv, tab = a.so.tableau, rec = nx + 2 + (a.tape_stages ? 6 * nv : 0);
   const bool has_ctrl = a.ctrl != nullptr && a.nknot > 0 && nu > 0;
   const int nknot = has_ctrl ? a.nknot : 0;
@@ -161,7 +151,7 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
         for (int j = gr.lane; j < nv; j += G) Vr[j] = (R)rk.sV()[i * nv + j];
         gr.sync();
         // A_i = F(Y_i), or F~ for the straight-through estimator (Eq. 4)
-        if (!vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.Ab().at(i * nv), a.cfd != 0, a.want_p != 0, ws, dws, rk, gr, a.dbg,
+        if (!vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.Ab().at(i * nv), a.cfd != 0, a.want_p != 0, ws, rk, gr, a.dbg,
                               (a.tape_stages && !a.cfd) ? rk.A().at(i * nv).p : nullptr)) { good = false; break; }   // F: x* = taped A_i
 #pragma unroll 1
         for (int j = gr.lane; j < nv; j += G) rk.Vb()[j] += rk.vbar()[j];
@@ -198,15 +188,14 @@ template <class R> struct FieldArgs {
   int n, cfd, want_p;
   const R *x, *u, *params, *zero_u, *kappa;
   R *acc, *qbar, *vbar, *ubar, *pbar; int* nrow;
-  Dual<R>* scratch; int res_size;
-  WsLayout wl, rwl; RkLayout rl;
+  WsLayout wl; RkLayout rl;
 };
 template <class R, int G>
 __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ FieldArgs<R> a) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
   if (threadIdx.x == 0) g_lockstep = 0;
-  load_cta_const<R>(cc, m_, a.wl, a.rwl, a.rl, a.rl.size_bwd);
+  load_cta_const<R>(cc, m_, a.wl, a.wl, a.rl, a.rl.size_bwd);
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
@@ -231,11 +220,10 @@ __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ Mode
       for (int j = gr.lane; j < nv; j += G) a.acc[(size_t)e * nv + j] = nr < 0 ? R(nan("")) : ws.x()[j];
       if (gr.lane == 0 && a.nrow) a.nrow[e] = nr;
     } else {
-      Ws<Dual<R>, 32> dws = bind_scratch<R>(a.scratch, a.res_size, &cc.rwl);
 #pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) rk.lam()[j] = (double)a.kappa[(size_t)e * nv + j];
       gr.sync();
-      bool ok = vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.lam(), a.cfd != 0, a.want_p != 0, ws, dws, rk, gr);
+      bool ok = vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.lam(), a.cfd != 0, a.want_p != 0, ws, rk, gr);
       R bad = R(nan(""));
 #pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) { a.qbar[(size_t)e * nv + j] = ok ? (R)rk.qbar()[j] : bad; a.vbar[(size_t)e * nv + j] = ok ? (R)rk.vbar()[j] : bad; }

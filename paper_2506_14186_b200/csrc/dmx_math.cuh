@@ -1,8 +1,8 @@
 // dmx_math.cuh — scalar, 3-D algebra and lane-group primitives of the CUDA path.
 //
 // The device code is written once, generic in
-//   S : the scalar (double, float, or the one-direction tangent scalar Dual<R> used by the
-//       vector-Jacobian product of the vector field, Eq. 4 / SURVEY O11), and
+//   S : the scalar (double or float; the one-direction tangent scalar Dual<R> serves the candidate
+//       scalars D(r), position term, b, mu inside the VJP, Eq. 4 / SURVEY O11), and
 //   G : the number of lanes that cooperate on one environment (1, 8, 16 or 32; a "lane group",
 //       BASELINE.json north_star subsystem 4).
 // Loops over independent items are strided over the group's lanes; the group re-converges
@@ -99,8 +99,7 @@ template <class T> DMX_DI Dual<T> m_pow(const Dual<T>& a, const Dual<T>& b) {
 
 // ---- strided array view: element i lives at p[i*ST] ----------------------------------------
 // ST == 1: contiguous per-group workspace in shared memory; ST == 32: per-lane workspaces of a
-// warp interleaved so that lanes touching the same index coalesce (G == 1 instantiations and the
-// per-lane tangent workspaces of the VJP).  The stride is a compile-time constant.
+// warp interleaved so that lanes touching the same index coalesce (G == 1 instantiations).  The stride is a compile-time constant.
 template <class S, int ST> struct Arr {
   S* p;
   DMX_DI Arr() {}
