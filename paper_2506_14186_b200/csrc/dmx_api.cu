@@ -175,7 +175,16 @@ void flatten(const dmx_model_desc* d, HostModel& h) {
   h.qpos0 = cpv(d->qpos0, h.nq);
 }
 
-void make_layouts(const HostModel& h, WsLayout& wl, WsLayout& rwl, RkLayout& rl) {
+// Optional shared-memory bank spread (DMX_PAD=1; off by default: measured on B200 it removes a third of the bank
+// conflicts but the shared-memory pipe runs at 0.25 wavefronts/cycle, so it buys <= 2 % and costs workspace bytes): with several lanes per environment a lane i reads row i of M, H
+// or J, so an even leading dimension puts the lanes of a group on 2-4 banks; an odd one spreads them over all of them.
+// With 8 lanes per environment the slices of neighbouring groups are offset by 8 scalars modulo 16 doubles / 32 floats,
+// so the groups that share a shared-memory wavefront use complementary banks.
+void make_layouts(const HostModel& h, int G, int real_bytes, WsLayout& wl, WsLayout& rwl, RkLayout& rl) {
+  const char* ep = std::getenv("DMX_PAD");
+  const bool pad = G > 1 && ep && std::atoi(ep) != 0;
+  const int ld = (pad && h.nv > 1 && h.nv % 2 == 0) ? h.nv + 1 : h.nv;
+  auto stagger = [&](int n, int scalar_bytes) { if (!pad || G != 8 || n == 0) return n; int mod = 64 / scalar_bytes * 2; while (n % mod != 8) ++n; return n; };
   const int nb = h.nbody, nv = h.nv, nq = h.nq, nc = std::max(h.nc, 1), nr = std::max(h.nrmax, 1);
   std::memset(&wl, 0, sizeof(wl)); std::memset(&rwl, 0, sizeof(rwl)); std::memset(&rl, 0, sizeof(rl));
   int o = 0;
@@ -184,24 +193,25 @@ void make_layouts(const HostModel& h, WsLayout& wl, WsLayout& rwl, RkLayout& rl)
   take(wl.com, 3 * nb); take(wl.dax, 3 * nv); take(wl.dan, 3 * nv);
   rwl = wl; rwl.size = 0;                                  // no per-lane tangent workspace any more (closed-form VJP)
   take(wl.Fb, 3 * nb); take(wl.Nb, 3 * nb); take(wl.Iw, 9 * nb); take(wl.Isub, 9 * nb); take(wl.tw, 3 * std::max(h.ntw, 1));
-  take(wl.M, nv * nv); take(wl.Hc, nv * nv); take(wl.tau, nv); take(wl.c, nv); take(wl.a0, nv); take(wl.x, nv); take(wl.g, nv);
+  wl.ld = ld;
+  take(wl.M, nv * ld); take(wl.Hc, nv * ld); take(wl.tau, nv); take(wl.c, nv); take(wl.a0, nv); take(wl.x, nv); take(wl.g, nv);
   take(wl.dl, nv); take(wl.Md, nv); take(wl.xa, nv); take(wl.kap, nv);
   take(wl.cr, nc); take(wl.cn, 3 * nc); take(wl.cpos, 3 * nc); take(wl.ct1, 3 * nc); take(wl.ct2, 3 * nc);
   take(wl.cD, nc); take(wl.cpost, nc); take(wl.cbd, nc); take(wl.cmu, nc); take(wl.cdD, nc); take(wl.cdpost, nc);
   take(wl.fox, 3 * nb); take(wl.fvx, 3 * nb);
-  take(wl.J, nr * nv); take(wl.aref, nr); take(wl.D, nr); take(wl.s, nr); take(wl.pr, nr);
-  wl.size = o;
+  take(wl.J, std::max(nr * ld, nc * nv) /* also the (candidate, dof) scratch of the VJP */); take(wl.aref, nr); take(wl.D, nr); take(wl.s, nr); take(wl.pr, nr);
+  wl.size = stagger(o + nq + nv, real_bytes) - (nq + nv);
   rl.Yqr = o; rl.Vr = o + nq; rl.rsize = nq + nv;
   o = 0;
   take(wl.i_incl, nc); take(wl.i_rowstart, nc); take(wl.i_rowcand, nr); take(wl.i_active, nr);
   wl.isize = o;
   o = 0;
   take(rl.q, nq); take(rl.v, nv); take(rl.Yq, nq); take(rl.V, nv); take(rl.Dl, nv); take(rl.K, 7 * nv); take(rl.A, 7 * nv); take(rl.err, 2 * nv);
-  rl.size_fwd = o;
+  rl.size_fwd = stagger(o, 8);
   take(rl.sYq, 6 * nq); take(rl.sV, 6 * nv); take(rl.sDl, 6 * nv); take(rl.Kb, 6 * nv); take(rl.Ab, 6 * nv);
   take(rl.qb, nv); take(rl.vb, nv); take(rl.dbar, nv); take(rl.Vb, nv); take(rl.lam, 2 * nv); take(rl.delta, nv);
   take(rl.qbar, nv); take(rl.vbar, nv); take(rl.ubar, std::max(h.nu, 1)); take(rl.pbar, h.np); take(rl.gp, h.np);
-  rl.size_bwd = o;
+  rl.size_bwd = stagger(o, 8);
 }
 
 template <class R> size_t add_real(Arena& a, const std::vector<double>& v) {
@@ -225,6 +235,7 @@ template <class R> void build_dev(const HostModel& h, Arena& ar, ModelDev<R>& m,
     for (auto v : rv) offs.push_back(add_real<R>(ar, *v));
     return;
   }
+  m.arena = ar.dev; m.arena_bytes = (int)((ar.host.size() + 15) & ~size_t(15)); m.arena_smem = 0;
   m.nbody = h.nbody; m.njnt = h.njnt; m.nq = h.nq; m.nv = h.nv; m.nu = h.nu; m.npair = h.npair; m.nc = h.nc; m.np = h.np;
   m.nlevel = h.nlevel; m.ntw = h.ntw; m.nmp = h.nmp; m.nrmax = h.nrmax;
   m.npp = 0; for (int c = 0; c < h.nc; ++c) m.npp += h.ct_kind[c] == CK_POINT_POINT; m.newton_iters = h.newton_iters; m.ls_iters = h.ls_iters;
@@ -297,6 +308,7 @@ int create_typed(dmx_model* m) {
   HostModel& h = m->h;
   ModelDev<R> dev;
   build_dev<R>(h, m->arena, dev, false);
+  m->arena.host.resize((m->arena.host.size() + 15) & ~size_t(15));
   CUDA_OK(cudaMalloc(&m->arena.dev, m->arena.host.size()));
   CUDA_OK(cudaMemcpy(m->arena.dev, m->arena.host.data(), m->arena.host.size(), cudaMemcpyHostToDevice));
   build_dev<R>(h, m->arena, dev, true);
@@ -317,26 +329,48 @@ int create_typed(dmx_model* m) {
   for (int i = 0; i < h.npair; ++i) { h.pair_invweight[i] = (double)bw[h.pair_body1[i]] + (double)bw[h.pair_body2[i]]; pw[i] = (R)h.pair_invweight[i]; }
   if (h.npair) CUDA_OK(cudaMemcpy(const_cast<R*>(dev.pair_invweight), pw.data(), sizeof(R) * h.npair, cudaMemcpyHostToDevice));
   if (sizeof(R) == 8) std::memcpy(&m->md, &dev, sizeof(dev)); else std::memcpy(&m->mf, &dev, sizeof(dev));
-  // block size per kernel: the one that keeps the most lane groups resident on an SM
-  const int blocks[4] = {256, 128, 64, 32};
+  // block size per kernel: the one that keeps the most lane groups resident on an SM.  The selection runs twice: with
+  // the constant arena appended to each CTA's dynamic shared memory (ModelDev::arena_smem) and without; the arena goes
+  // to shared memory only if no kernel loses resident groups to it (DMX_ARENA_SMEM=0 keeps it in global memory).
   const char* eb = std::getenv("DMX_BWD_BLOCK");
-  for (int bi = 0; bi < 4; ++bi) {
-    int blk = blocks[bi], g = groups_per_block(m, blk);
-    size_t sf = g * group_bytes(m, 0), sb = g * group_bytes(m, 1), sx = g * group_bytes(m, 2);
-    int of = 0, ob = 0, ox = 0;
-    size_t lim = (size_t)m->max_smem - 2048;     // room for the static shared constants
-    if (blk > 128) { int b2 = 128, g2 = groups_per_block(m, b2); int t0, t2;   // only the backward kernel is compiled for 256 threads
-      CUDA_OK(L.occupancy(b2, std::min(g2 * group_bytes(m, 0), lim), std::min(sb, lim), std::min(g2 * group_bytes(m, 2), lim), &t0, &ob, &t2));
-      (void)t0; (void)t2; ob = sb <= lim ? 1 : 0; }
-    else CUDA_OK(L.occupancy(blk, std::min(sf, lim), std::min(sb, lim), std::min(sx, lim), &of, &ob, &ox));
-    if (blk <= 128 && sf <= lim && of * g > m->cf.occ * groups_per_block(m, std::max(m->cf.block, 1))) { m->cf.block = blk; m->cf.occ = of; m->cf.smem = sf; }
-    if (eb ? (std::atoi(eb) == blk && sb <= lim && ob > 0) : (blk <= 128 && sb <= lim && ob * g > m->cb.occ * groups_per_block(m, std::max(m->cb.block, 1)))) { m->cb.block = blk; m->cb.occ = ob; m->cb.smem = sb; }
-    if (blk <= 128 && sx <= lim && ox * g > m->cx.occ * groups_per_block(m, std::max(m->cx.block, 1))) { m->cx.block = blk; m->cx.occ = ox; m->cx.smem = sx; }
+  const char* ef = std::getenv("DMX_FWD_BLOCK");
+  typedef dmx_model::Cfg Cfg;
+  auto select = [&](size_t ab, Cfg& cf, Cfg& cb, Cfg& cx) -> int {
+    const int blocks[4] = {256, 128, 64, 32};
+    cf = Cfg(); cb = Cfg(); cx = Cfg();
+    for (int bi = 0; bi < 4; ++bi) {
+      int blk = blocks[bi], g = groups_per_block(m, blk);
+      auto pad = [&](size_t b) { return ((b + 15) & ~size_t(15)) + ab; };
+      size_t sf = pad(g * group_bytes(m, 0)), sb = pad(g * group_bytes(m, 1)), sx = pad(g * group_bytes(m, 2));
+      int of = 0, ob = 0, ox = 0;
+      size_t lim = (size_t)m->max_smem - 2048;     // room for the static shared constants
+      if (blk > 128) { int b2 = 128, g2 = groups_per_block(m, b2); int t0, t2;   // only the backward kernel is compiled for 256 threads
+        CUDA_OK(L.occupancy(b2, std::min(pad(g2 * group_bytes(m, 0)), lim), std::min(sb, lim), std::min(pad(g2 * group_bytes(m, 2)), lim), &t0, &ob, &t2));
+        (void)t0; (void)t2; ob = sb <= lim ? 1 : 0; }
+      else CUDA_OK(L.occupancy(blk, std::min(sf, lim), std::min(sb, lim), std::min(sx, lim), &of, &ob, &ox));
+      if (ef ? (std::atoi(ef) == blk && blk <= 128 && sf <= lim && of > 0) : (blk <= 128 && sf <= lim && of * g > cf.occ * groups_per_block(m, std::max(cf.block, 1)))) { cf.block = blk; cf.occ = of; cf.smem = sf; }
+      if (eb ? (std::atoi(eb) == blk && sb <= lim && ob > 0) : (blk <= 128 && sb <= lim && ob * g > cb.occ * groups_per_block(m, std::max(cb.block, 1)))) { cb.block = blk; cb.occ = ob; cb.smem = sb; }
+      if (blk <= 128 && sx <= lim && ox * g > cx.occ * groups_per_block(m, std::max(cx.block, 1))) { cx.block = blk; cx.occ = ox; cx.smem = sx; }
+    }
+    return 0;
+  };
+  if (int rc = select(0, m->cf, m->cb, m->cx)) return rc;
+  {
+    const char* ea = std::getenv("DMX_ARENA_SMEM");
+    Cfg af, abk, ax;
+    if (!(ea && std::atoi(ea) == 0)) {
+      if (int rc = select(m->arena.host.size(), af, abk, ax)) return rc;
+      auto res = [&](const Cfg& c) { return c.occ * groups_per_block(m, std::max(c.block, 1)); };
+      if (af.occ >= 1 && abk.occ >= 1 && ax.occ >= 1 && res(af) >= res(m->cf) && res(abk) >= res(m->cb)) {
+        m->cf = af; m->cb = abk; m->cx = ax;
+        if (sizeof(R) == 8) m->md.arena_smem = 1; else m->mf.arena_smem = 1;
+      }
+    }
   }
   if (m->cf.occ < 1 || m->cb.occ < 1 || m->cx.occ < 1) return fail("model too large for the per-environment shared-memory workspace (try DMX_LANES=32)");
   if (std::getenv("DMX_VERBOSE"))
-    std::fprintf(stderr, "dmx: lanes %d | fwd block %d x occ %d smem %zu | bwd block %d x occ %d smem %zu | field block %d x occ %d smem %zu | group bytes f/b %zu/%zu\n",
-                 m->G, m->cf.block, m->cf.occ, m->cf.smem, m->cb.block, m->cb.occ, m->cb.smem, m->cx.block, m->cx.occ, m->cx.smem, group_bytes(m, 0), group_bytes(m, 1));
+    std::fprintf(stderr, "dmx: arena %zu B in %s | lanes %d | fwd block %d x occ %d smem %zu | bwd block %d x occ %d smem %zu | field block %d x occ %d smem %zu | group bytes f/b %zu/%zu\n",
+                 m->arena.host.size(), (m->precision == 64 ? m->md.arena_smem : m->mf.arena_smem) ? "smem" : "global", m->G, m->cf.block, m->cf.occ, m->cf.smem, m->cb.block, m->cb.occ, m->cb.smem, m->cx.block, m->cx.occ, m->cx.smem, group_bytes(m, 0), group_bytes(m, 1));
   // the occupancy queries above left the largest attribute set; restore the chosen sizes
   int d0, d1, d2;
   CUDA_OK(L.occupancy(m->cf.block, m->cf.smem, m->cb.smem, m->cx.smem, &d0, &d1, &d2));
@@ -461,7 +495,7 @@ int dmx_model_create(const dmx_model_desc* desc, int precision, dmx_model** out)
   try { flatten(desc, m->h); } catch (std::exception& e) { fail("model: %s", e.what()); delete m; return -1; }
   m->precision = precision;
   m->G = pick_lanes(m->h);
-  make_layouts(m->h, m->wl, m->rwl, m->rl);
+  make_layouts(m->h, m->G, precision / 8, m->wl, m->rwl, m->rl);
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
     fail("no CUDA device: the dmx library has no CPU fallback"); delete m; return -1;

@@ -157,6 +157,7 @@ DMX_DI void body_wrench(const ModelDev<R>& m, const IN& in, const WS& ws, int b,
 // world inertias of that subtree.  c_j = sum_b lin_jb . F_b + ang_j . N_b (virtual work).
 template <class WS, class R, int G, class IN>
 DMX_DN void dynamics(const ModelDev<R>& m, const IN& in, const WS& ws, const Grp<G>& gr) {
+  const int ld = ws.L->ld;
   typedef typename WS::S S;
   const int nv = m.nv, nb = m.nbody;
 #pragma unroll 1
@@ -193,7 +194,7 @@ DMX_DN void dynamics(const ModelDev<R>& m, const IN& in, const WS& ws, const Grp
       if (m.dof_rot[i] && m.dof_rot[j]) acc = acc + dot(ld3(ws.dax(), i), ld9(ws.Isub(), deep) * ld3(ws.dax(), j));
       if (i == j) acc = acc + S(m.jnt_armature[m.dof_jnt[i]]);
     }
-    ws.M()[i * nv + j] = acc; ws.M()[j * nv + i] = acc;
+    ws.M()[i * ld + j] = acc; ws.M()[j * ld + i] = acc;
   }
 #pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) {
@@ -231,48 +232,48 @@ DMX_DI void tri_index(int e, int& a, int& b) {
 // ---- dense Cholesky on the lower triangle, one column at a time, lanes over rows ---------------
 // The factor is stored with the RECIPROCAL of its diagonal (l_jj^-1 = rsqrt of the pivot), so the column scaling
 // and both substitutions multiply instead of divide: the dependent chain per column is one rsqrt, not sqrt + div.
-template <class S, int ST, int G> DMX_DN bool cholesky(const Arr<S, ST>& A, int n, const Grp<G>& gr) {
+template <class S, int ST, int G> DMX_DN bool cholesky(const Arr<S, ST>& A, int n, int ld, const Grp<G>& gr) {
 #pragma unroll 1
   for (int j = 0; j < n; ++j) {
 #pragma unroll 1
     for (int i = j + gr.lane; i < n; i += G) {
-      S t = A[i * n + j];
+      S t = A[i * ld + j];
 #pragma unroll 4
-      for (int k = 0; k < j; ++k) t = t - A[i * n + k] * A[j * n + k];
-      A[i * n + j] = t;
+      for (int k = 0; k < j; ++k) t = t - A[i * ld + k] * A[j * ld + k];
+      A[i * ld + j] = t;
     }
     gr.sync();
-    S s = A[j * n + j];
+    S s = A[j * ld + j];
     if (!(val(s) > 0)) return false;       // uniform over the group
     S il = m_rsqrt(s);
     gr.sync();
 #pragma unroll 1
-    for (int i = j + gr.lane; i < n; i += G) A[i * n + j] = (i == j) ? il : A[i * n + j] * il;
+    for (int i = j + gr.lane; i < n; i += G) A[i * ld + j] = (i == j) ? il : A[i * ld + j] * il;
     gr.sync();
   }
   return true;
 }
 // b <- (L L^T)^-1 b; column-oriented substitutions (diagonal of L holds reciprocals)
-template <class S, int ST, int G> DMX_DN void chol_solve(const Arr<S, ST>& L, int n, const Arr<S, ST>& b, const Grp<G>& gr) {
+template <class S, int ST, int G> DMX_DN void chol_solve(const Arr<S, ST>& L, int n, int ld, const Arr<S, ST>& b, const Grp<G>& gr) {
 #pragma unroll 1
   for (int i = 0; i < n; ++i) {
-    S bi = b[i] * L[i * n + i];
+    S bi = b[i] * L[i * ld + i];
 #pragma unroll 1
-    for (int k = i + 1 + gr.lane; k < n; k += G) b[k] = b[k] - L[k * n + i] * bi;
+    for (int k = i + 1 + gr.lane; k < n; k += G) b[k] = b[k] - L[k * ld + i] * bi;
     gr.sync();
   }
 #pragma unroll 1
-  for (int i = gr.lane; i < n; i += G) b[i] = b[i] * L[i * n + i];
+  for (int i = gr.lane; i < n; i += G) b[i] = b[i] * L[i * ld + i];
   gr.sync();
 #pragma unroll 1
   for (int i = n - 1; i >= 0; --i) {
-    S bi = b[i] * L[i * n + i];
+    S bi = b[i] * L[i * ld + i];
 #pragma unroll 1
-    for (int k = gr.lane; k < i; k += G) b[k] = b[k] - L[i * n + k] * bi;
+    for (int k = gr.lane; k < i; k += G) b[k] = b[k] - L[i * ld + k] * bi;
     gr.sync();
   }
 #pragma unroll 1
-  for (int i = gr.lane; i < n; i += G) b[i] = b[i] * L[i * n + i];
+  for (int i = gr.lane; i < n; i += G) b[i] = b[i] * L[i * ld + i];
   gr.sync();
 }
 
@@ -382,6 +383,7 @@ DMX_DI V3<typename WS::S> rel_twist(const ModelDev<R>& m, const WS& ws, int j, i
 // ---- S4+S5: rows of every candidate with r<0 (cfd: r<w_c), compacted in candidate order ----------
 template <class WS, class R, int G, class IN>
 DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, const Grp<G>& gr) {
+  const int ld = ws.L->ld;
   typedef typename WS::S S;
   const int nv = m.nv, nc = m.nc;
 #pragma unroll 1
@@ -415,12 +417,12 @@ DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
     int r0 = ws.rowstart()[c];
     V3<S> d = rel_twist<WS, R>(m, ws, j, m.ct_b1[c], m.ct_b2[c], ld3(ws.cpos(), c));
     S nd = dot(ld3(ws.cn(), c), d);
-    if (n == 1) ws.J()[r0 * nv + j] = nd;
+    if (n == 1) ws.J()[r0 * ld + j] = nd;
     else {
       S mu = ws.cmu()[c];
       S t1d = mu * dot(ld3(ws.ct1(), c), d), t2d = mu * dot(ld3(ws.ct2(), c), d);
-      ws.J()[r0 * nv + j] = nd + t1d; ws.J()[(r0 + 1) * nv + j] = nd - t1d;
-      ws.J()[(r0 + 2) * nv + j] = nd + t2d; ws.J()[(r0 + 3) * nv + j] = nd - t2d;
+      ws.J()[r0 * ld + j] = nd + t1d; ws.J()[(r0 + 1) * ld + j] = nd - t1d;
+      ws.J()[(r0 + 2) * ld + j] = nd + t2d; ws.J()[(r0 + 3) * ld + j] = nd - t2d;
     }
   }
   gr.sync();
@@ -429,7 +431,7 @@ DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
     int c = ws.rowcand()[i] >> 2;
     S Jv(0.0);
 #pragma unroll 4
-    for (int j = 0; j < nv; ++j) Jv = Jv + ws.J()[i * nv + j] * in.v(j);
+    for (int j = 0; j < nv; ++j) Jv = Jv + ws.J()[i * ld + j] * in.v(j);
     ws.aref()[i] = ws.cpost()[c] - ws.cbd()[c] * Jv;
     ws.D()[i] = ws.cD()[c];
   }
@@ -443,6 +445,7 @@ DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
 // Returns true when the last step was a full step inside an unchanged active set.
 template <class WS, int G>
 DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G>& gr) {
+  const int ld = ws.L->ld;
   typedef typename WS::S S;
 #pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) ws.x()[j] = ws.a0()[j];
@@ -455,7 +458,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
     for (int i = gr.lane; i < nr; i += G) {
       S t(0.0);
 #pragma unroll 4
-      for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.x()[j];
+      for (int j = 0; j < nv; ++j) t = t + ws.J()[i * ld + j] * ws.x()[j];
       ws.s()[i] = t - ws.aref()[i];
     }
 #pragma unroll 1
@@ -465,28 +468,28 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
     for (int a = gr.lane; a < nv; a += G) {
       S t(0.0);
 #pragma unroll 4
-      for (int b = 0; b < nv; ++b) t = t + ws.M()[a * nv + b] * ws.xa()[b];
+      for (int b = 0; b < nv; ++b) t = t + ws.M()[a * ld + b] * ws.xa()[b];
 #pragma unroll 4
-      for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.J()[i * nv + a] * ws.D()[i] * ws.s()[i];
+      for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.J()[i * ld + a] * ws.D()[i] * ws.s()[i];
       ws.g()[a] = t; ws.dl()[a] = -t;
     }
 #pragma unroll 1
     for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
       int a, b; tri_index(e, a, b);
-      S t = ws.M()[a * nv + b];
+      S t = ws.M()[a * ld + b];
 #pragma unroll 4
-      for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.D()[i] * ws.J()[i * nv + a] * ws.J()[i * nv + b];
-      ws.Hc()[a * nv + b] = t;
+      for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.D()[i] * ws.J()[i * ld + a] * ws.J()[i * ld + b];
+      ws.Hc()[a * ld + b] = t;
     }
     gr.sync();
-    if (!cholesky(ws.Hc(), nv, gr)) break;
-    chol_solve(ws.Hc(), nv, ws.dl(), gr);
+    if (!cholesky(ws.Hc(), nv, ld, gr)) break;
+    chol_solve(ws.Hc(), nv, ld, ws.dl(), gr);
     bool same = true;
 #pragma unroll 1
     for (int i = gr.lane; i < nr; i += G) {
       S t(0.0);
 #pragma unroll 4
-      for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.dl()[j];
+      for (int j = 0; j < nv; ++j) t = t + ws.J()[i * ld + j] * ws.dl()[j];
       ws.pr()[i] = t;
       if ((val(ws.s()[i]) < 0) != (val(ws.s()[i] + t) < 0)) same = false;
     }
@@ -500,7 +503,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
       for (int a = gr.lane; a < nv; a += G) {
         S t(0.0);
 #pragma unroll 4
-        for (int b = 0; b < nv; ++b) t = t + ws.M()[a * nv + b] * ws.dl()[b];
+        for (int b = 0; b < nv; ++b) t = t + ws.M()[a * ld + b] * ws.dl()[b];
         ws.Md()[a] = t;
       }
       gr.sync();
@@ -545,6 +548,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
 template <class WS, class R, int G, class IN>
 DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, bool& conv, const Grp<G>& gr,
                         const double* xk = nullptr, int xst = 1) {
+  const int ld = ws.L->ld;
   const int nv = m.nv;
   phase_sync(0);
   DMX_T0;
@@ -556,11 +560,11 @@ DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool c
   conv = true;
   if (!xk) {
     phase_sync(2);
-    for (int e = gr.lane; e < nv * nv; e += G) ws.Hc()[e] = ws.M()[e];
+    for (int e = gr.lane; e < nv * ld; e += G) ws.Hc()[e] = ws.M()[e];
     for (int j = gr.lane; j < nv; j += G) ws.a0()[j] = ws.tau()[j] - ws.c()[j];
     gr.sync();
-    if (!cholesky(ws.Hc(), nv, gr)) return -1;
-    chol_solve(ws.Hc(), nv, ws.a0(), gr);
+    if (!cholesky(ws.Hc(), nv, ld, gr)) return -1;
+    chol_solve(ws.Hc(), nv, ld, ws.a0(), gr);
     DMX_TICK(gr, 2);
   }
   phase_sync(3);
@@ -584,12 +588,13 @@ DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool c
 // ws.kap() holds kappa on entry and w on exit.  Returns false if H is not positive definite.
 template <class WS, int G>
 DMX_DN bool vjp_prepare(int nv, int nr, const WS& ws, const Grp<G>& gr) {
+  const int ld = ws.L->ld;
   typedef typename WS::S S;
 #pragma unroll 1
   for (int i = gr.lane; i < nr; i += G) {
     S t(0.0);
 #pragma unroll 4
-    for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.x()[j];
+    for (int j = 0; j < nv; ++j) t = t + ws.J()[i * ld + j] * ws.x()[j];
     t = t - ws.aref()[i];
     ws.s()[i] = t;
     ws.active()[i] = val(t) < 0 ? 1 : 0;
@@ -598,14 +603,14 @@ DMX_DN bool vjp_prepare(int nv, int nr, const WS& ws, const Grp<G>& gr) {
 #pragma unroll 1
   for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
     int a, b; tri_index(e, a, b);
-    S t = ws.M()[a * nv + b];
+    S t = ws.M()[a * ld + b];
 #pragma unroll 4
-    for (int i = 0; i < nr; ++i) if (ws.active()[i]) t = t + ws.D()[i] * ws.J()[i * nv + a] * ws.J()[i * nv + b];
-    ws.Hc()[a * nv + b] = t;
+    for (int i = 0; i < nr; ++i) if (ws.active()[i]) t = t + ws.D()[i] * ws.J()[i * ld + a] * ws.J()[i * ld + b];
+    ws.Hc()[a * ld + b] = t;
   }
   gr.sync();
-  if (!cholesky(ws.Hc(), nv, gr)) return false;
-  chol_solve(ws.Hc(), nv, ws.kap(), gr);
+  if (!cholesky(ws.Hc(), nv, ld, gr)) return false;
+  chol_solve(ws.Hc(), nv, ld, ws.kap(), gr);
   return true;
 }
 
@@ -621,6 +626,7 @@ DMX_DN bool vjp_prepare(int nv, int nr, const WS& ws, const Grp<G>& gr) {
 // w in ws.kap.  Uses ws.Fb/ws.Nb for velw/omegaw, ws.Isub for the body adjoints, ws.pr for J_i w.
 template <class WS, class R, int G, class IN, class AOUT>
 DMX_D void vjp_velocity(const ModelDev<R>& m, const IN& in, const WS& ws, int nr, const AOUT& vbar, const Grp<G>& gr) {
+  const int ld = ws.L->ld;
   typedef typename WS::S S;
   const int nv = m.nv, nb = m.nbody;
   // seeds: cotangents of (omega_b, alpha_b, ap_b) from F_b = m (ac_b - g), N_b = I alpha + omega x I omega
@@ -646,7 +652,7 @@ DMX_D void vjp_velocity(const ModelDev<R>& m, const IN& in, const WS& ws, int nr
 #pragma unroll 1
   for (int i = gr.lane; i < nr; i += G) {
     S t(0.0);
-    if (ws.active()[i]) for (int j = 0; j < nv; ++j) t = t + ws.J()[i * nv + j] * ws.kap()[j];
+    if (ws.active()[i]) for (int j = 0; j < nv; ++j) t = t + ws.J()[i * ld + j] * ws.kap()[j];
     ws.pr()[i] = t;
   }
   gr.sync();
@@ -702,7 +708,7 @@ DMX_D void vjp_velocity(const ModelDev<R>& m, const IN& in, const WS& ws, int nr
     for (int i = 0; i < m.nu; ++i) if (m.act_type[i] == ACT_PD && m.jnt_vadr[m.act_jnt[i]] == j) kd = kd + S(m.act_kd[i]);
     g = g + ws.kap()[j] * kd;
 #pragma unroll 1
-    for (int i = 0; i < nr; ++i) if (ws.active()[i]) g = g + ws.pr()[i] * ws.D()[i] * ws.cbd()[ws.rowcand()[i] >> 2] * ws.J()[i * nv + j];
+    for (int i = 0; i < nr; ++i) if (ws.active()[i]) g = g + ws.pr()[i] * ws.D()[i] * ws.cbd()[ws.rowcand()[i] >> 2] * ws.J()[i * ld + j];
     vbar[j] = -(double)g;
   }
   gr.sync();

@@ -258,10 +258,11 @@ __global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ 
   InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = zero_v; in.pa = m.p_default;
   kinematics<Ws<R, ST>, R, G, InPlain<R, ST>, false>(m, in, ws, gr);
   dynamics<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, gr);
+  const int ld = ws.L->ld;
 #pragma unroll 1
-  for (int e = gr.lane; e < nv * nv; e += G) ws.Hc()[e] = ws.M()[e];
+  for (int e = gr.lane; e < nv * ld; e += G) ws.Hc()[e] = ws.M()[e];
   gr.sync();
-  bool pd = cholesky(ws.Hc(), nv, gr);
+  bool pd = cholesky(ws.Hc(), nv, ld, gr);
 #pragma unroll 1
   for (int b = 0; b < m.nbody; ++b) {
     R tr = R(0);
@@ -275,7 +276,7 @@ __global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ 
         ws.g()[j] = val_; ws.dl()[j] = val_;
       }
       gr.sync();
-      chol_solve(ws.Hc(), nv, ws.dl(), gr);
+      chol_solve(ws.Hc(), nv, ld, ws.dl(), gr);
 #pragma unroll 1
       for (int j = 0; j < nv; ++j) tr += ws.g()[j] * ws.dl()[j];
       gr.sync();

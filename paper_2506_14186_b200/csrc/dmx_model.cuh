@@ -1,6 +1,7 @@
 // dmx_model.cuh — device-side model (flattened kinematic tree, candidate contacts, index tables)
 // and the per-environment workspace layouts.  Built on the host by dmx_api.cu.
 #pragma once
+#include <cstddef>
 #include "dmx_math.cuh"
 
 namespace dmx {
@@ -14,6 +15,13 @@ template <class R> struct ModelDev {
   int nbody, njnt, nq, nv, nu, npair, nc, np, nlevel, ntw, nmp, nrmax, npp /* point-point candidates */;
   int newton_iters, ls_iters;
   int p_fric, p_solref, p_solimp;          // offsets in the parameter vector (mass at 0)
+  // The constant arrays below live in one device allocation [arena, arena + arena_bytes).  arena_smem != 0: every CTA
+  // copies the arena to the end of its dynamic shared memory and rebases the pointers (load_cta_const), so the index
+  // tables are read with shared-memory latency instead of L1/L2 latency (the workspaces leave L1 only a few KB).
+  int arena_bytes, arena_smem;
+  R gravity[3];
+  const unsigned char* arena;
+  // ---- pointers into the arena: one contiguous block, body_parent first, p_default last (see N_ARENA_PTR) ----
   // tree
   const int *body_parent, *body_jnt, *level_ptr, *level_body;
   const R *body_pos, *body_rot, *body_ipos, *body_irot, *body_iunit;
@@ -31,9 +39,13 @@ template <class R> struct ModelDev {
   const R *pair_invweight, *pair_solimp_cfd, *pair_cfd_beta;
   const int *act_type, *act_jnt;
   const R *act_gear, *act_kp, *act_kd;
-  R gravity[3];
   const R *p_default;
 };
+enum { N_ARENA_PTR = 52 };
+static_assert(offsetof(ModelDev<double>, p_default) - offsetof(ModelDev<double>, body_parent) == (N_ARENA_PTR - 1) * sizeof(void*),
+              "ModelDev: the arena pointers must form one contiguous block");
+static_assert(offsetof(ModelDev<float>, p_default) - offsetof(ModelDev<float>, body_parent) == (N_ARENA_PTR - 1) * sizeof(void*),
+              "ModelDev: the arena pointers must form one contiguous block");
 
 // Offsets (in scalars) of the per-environment arrays inside a workspace of scalar type S.
 // `full` layouts serve the cooperative evaluation of F; `res` layouts serve the per-lane
@@ -47,6 +59,7 @@ struct WsLayout {
   int fox, fvx;                                       // per body: twist under the joint rates x* (angular, velocity of the COM)
   int J, aref, D, s, pr;                              // per row
   int size;                                           // scalars
+  int ld;                                             // leading dimension of M, Hc and J (odd when lanes share a warp: bank spread)
   // int workspace (separate array)
   int i_incl, i_rowstart, i_rowcand, i_active, isize;
 };

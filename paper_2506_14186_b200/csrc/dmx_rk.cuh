@@ -236,6 +236,20 @@ DMX_DI void load_cta_const(CtaConst<R>& c, const ModelDev<R>& m, const WsLayout&
   const int n[4] = {(int)(sizeof(ModelDev<R>) / 4), (int)(sizeof(WsLayout) / 4), (int)(sizeof(WsLayout) / 4), (int)(sizeof(RkLayout) / 4)};
 #pragma unroll 1
   for (int k = 0; k < 4; ++k) for (int i = threadIdx.x; i < n[k]; i += blockDim.x) dst[k][i] = src[k][i];
+  if (m.arena_smem) {
+    // the constant arena goes to the last arena_bytes (a multiple of 16) of the CTA's dynamic shared memory
+    unsigned dyn_bytes;
+    asm volatile("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn_bytes));
+    unsigned char* sa = dyn_smem + (dyn_bytes - (unsigned)m.arena_bytes);
+    const int4* g4 = reinterpret_cast<const int4*>(m.arena);
+    int4* s4 = reinterpret_cast<int4*>(sa);
+#pragma unroll 1
+    for (int i = threadIdx.x; i < m.arena_bytes / 16; i += blockDim.x) s4[i] = g4[i];
+    __syncthreads();
+    const unsigned char** ptr = reinterpret_cast<const unsigned char**>(&c.m.body_parent);
+#pragma unroll 1
+    for (int i = threadIdx.x; i < N_ARENA_PTR; i += blockDim.x) ptr[i] = sa + (ptr[i] - m.arena);
+  }
   __syncthreads();
 }
 
