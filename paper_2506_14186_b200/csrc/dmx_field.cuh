@@ -460,6 +460,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
 #pragma unroll 4
       for (int j = 0; j < nv; ++j) t = t + ws.J()[i * ld + j] * ws.x()[j];
       ws.s()[i] = t - ws.aref()[i];
+      ws.active()[i] = val(ws.s()[i]) < 0 ? 1 : 0;     // the set the factor left in Hc belongs to (reused by vjp_prepare)
     }
 #pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) ws.xa()[j] = ws.x()[j] - ws.a0()[j];
@@ -587,9 +588,13 @@ DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool c
 // ---- S11/S12, cooperative part: final active set A, H = M + J_A^T D_A J_A, w = H^-1 kappa ---------
 // ws.kap() holds kappa on entry and w on exit.  Returns false if H is not positive definite.
 template <class WS, int G>
-DMX_DN bool vjp_prepare(int nv, int nr, const WS& ws, const Grp<G>& gr) {
+DMX_DN bool vjp_prepare(int nv, int nr, bool hc_valid, const WS& ws, const Grp<G>& gr) {
   const int ld = ws.L->ld;
   typedef typename WS::S S;
+  // hc_valid: Hc still holds the Cholesky factor of the last Newton iteration (or of M when there are no rows) and
+  // ws.active the set it was built for.  A converged solve ends on an unchanged active set, so that factor IS the
+  // factor of H at x*; it is reused unless the recomputed residuals disagree with the set on a sign.
+  bool same = hc_valid;
 #pragma unroll 1
   for (int i = gr.lane; i < nr; i += G) {
     S t(0.0);
@@ -597,19 +602,24 @@ DMX_DN bool vjp_prepare(int nv, int nr, const WS& ws, const Grp<G>& gr) {
     for (int j = 0; j < nv; ++j) t = t + ws.J()[i * ld + j] * ws.x()[j];
     t = t - ws.aref()[i];
     ws.s()[i] = t;
-    ws.active()[i] = val(t) < 0 ? 1 : 0;
+    const int act = val(t) < 0 ? 1 : 0;
+    if (hc_valid && ws.active()[i] != act) same = false;
+    ws.active()[i] = act;
   }
+  const bool reuse = gr.all(same);
   gr.sync();
+  if (!reuse) {
 #pragma unroll 1
-  for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
-    int a, b; tri_index(e, a, b);
-    S t = ws.M()[a * ld + b];
+    for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
+      int a, b; tri_index(e, a, b);
+      S t = ws.M()[a * ld + b];
 #pragma unroll 4
-    for (int i = 0; i < nr; ++i) if (ws.active()[i]) t = t + ws.D()[i] * ws.J()[i * ld + a] * ws.J()[i * ld + b];
-    ws.Hc()[a * ld + b] = t;
+      for (int i = 0; i < nr; ++i) if (ws.active()[i]) t = t + ws.D()[i] * ws.J()[i * ld + a] * ws.J()[i * ld + b];
+      ws.Hc()[a * ld + b] = t;
+    }
+    gr.sync();
+    if (!cholesky(ws.Hc(), nv, ld, gr)) return false;
   }
-  gr.sync();
-  if (!cholesky(ws.Hc(), nv, ld, gr)) return false;
   chol_solve(ws.Hc(), nv, ld, ws.kap(), gr);
   return true;
 }

@@ -25,7 +25,7 @@ DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yq
 #pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) ws.kap()[j] = (R)kappa[j];
   gr.sync();
-  if (!vjp_prepare<Ws<R, ST>, G>(nv, nr, ws, gr)) return false;
+  if (!vjp_prepare<Ws<R, ST>, G>(nv, nr, xk == nullptr && conv != 0 && !(dbg & 8), ws, gr)) return false;
   DMX_TICK(gr, 9);
   phase_sync(6);
   // u: closed form; v: reverse sweep over the tree; then the frames at acceleration x* for the tangent passes
