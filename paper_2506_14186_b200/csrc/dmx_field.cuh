@@ -232,7 +232,28 @@ DMX_DI void tri_index(int e, int& a, int& b) {
 // ---- dense Cholesky on the lower triangle, one column at a time, lanes over rows ---------------
 // The factor is stored with the RECIPROCAL of its diagonal (l_jj^-1 = rsqrt of the pivot), so the column scaling
 // and both substitutions multiply instead of divide: the dependent chain per column is one rsqrt, not sqrt + div.
+// With n <= G lane i owns row i: the pivot travels by shuffle and every lane scales its own entry, so a column costs one
+// group barrier instead of three (same operations per entry: bitwise the result of the general version below).
 template <class S, int ST, int G> DMX_DN bool cholesky(const Arr<S, ST>& A, int n, int ld, const Grp<G>& gr) {
+  if (G > 1 && n <= G) {
+    const int i = gr.lane;
+#pragma unroll 1
+    for (int j = 0; j < n; ++j) {
+      const bool act = i >= j && i < n;
+      S t(0.0);
+      if (act) {
+        t = A[i * ld + j];
+#pragma unroll 4
+        for (int k = 0; k < j; ++k) t = t - A[i * ld + k] * A[j * ld + k];
+      }
+      S s = gr.from_lane(t, j);
+      if (!(val(s) > 0)) return false;       // uniform over the group
+      S il = m_rsqrt(s);
+      if (act) A[i * ld + j] = (i == j) ? il : t * il;
+      gr.sync();
+    }
+    return true;
+  }
 #pragma unroll 1
   for (int j = 0; j < n; ++j) {
 #pragma unroll 1
@@ -254,7 +275,30 @@ template <class S, int ST, int G> DMX_DN bool cholesky(const Arr<S, ST>& A, int 
   return true;
 }
 // b <- (L L^T)^-1 b; column-oriented substitutions (diagonal of L holds reciprocals)
+// With n <= G the right-hand side lives in registers, one entry per lane, and the pivot entry travels by shuffle: the
+// dependent chain per column is shuffle + multiply + fma instead of shared load + multiply + fma + store + group barrier
+// (same operations on every entry in the same order, so the result is bitwise that of the shared-memory version).
 template <class S, int ST, int G> DMX_DN void chol_solve(const Arr<S, ST>& L, int n, int ld, const Arr<S, ST>& b, const Grp<G>& gr) {
+  if (G > 1 && n <= G) {
+    const int k = gr.lane;
+    const bool in = k < n;
+    S bk = in ? b[k] : S(0.0);
+#pragma unroll 1
+    for (int i = 0; i < n; ++i) {
+      S bi = gr.from_lane(bk, i) * L[i * ld + i];
+      if (in && k > i) bk = bk - L[k * ld + i] * bi;
+      else if (k == i) bk = bi;
+    }
+#pragma unroll 1
+    for (int i = n - 1; i >= 0; --i) {
+      S bi = gr.from_lane(bk, i) * L[i * ld + i];
+      if (k < i) bk = bk - L[i * ld + k] * bi;
+      else if (k == i) bk = bi;
+    }
+    if (in) b[k] = bk;
+    gr.sync();
+    return;
+  }
 #pragma unroll 1
   for (int i = 0; i < n; ++i) {
     S bi = b[i] * L[i * ld + i];

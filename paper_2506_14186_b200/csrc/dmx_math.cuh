@@ -117,6 +117,10 @@ template <int G> struct Grp {
     unsigned b = __ballot_sync(mask, pred);
     return (b & mask) == mask;
   }
+  template <class T> DMX_DI T from_lane(T x, int src) const {   // value held by the group's lane `src` (uniform over the group)
+    if (G == 1) return x;
+    return __shfl_sync(mask, x, ((threadIdx.x & 31) & ~(G - 1)) + src);
+  }
   DMX_DI int bcast_int(int x) const {            // value of the group's lane 0
     if (G == 1) return x;
     return __shfl_sync(mask, x, (threadIdx.x & 31) & ~(G - 1));
