@@ -422,7 +422,7 @@ int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const vo
   size_t hdr = tape_header_bytes(nenv);
   if (!tape || tape_bytes < hdr + (size_t)nenv * rec * sizeof(R)) return fail("tape missing or too small");
   a.nenv = nenv; a.nknot = nknot; a.want_p = dLdparams != nullptr; a.cfd = cfd_on; a.tape_stages = m->tape_stages;
-  { const char* e = std::getenv("DMX_DBG"); a.dbg = e ? std::atoi(e) : 0; }   // timing experiments only (results invalid when set)
+  { const char* e = std::getenv("DMX_DBG"); a.dbg = e ? std::atoi(e) : 0; }   // timing experiments only (results invalid when set, except bit 8: VJP rebuilds H instead of reusing the Newton factor)
   a.tape_cap = (int)std::min<size_t>((tape_bytes - hdr) / ((size_t)nenv * rec * sizeof(R)), (size_t)1 << 30);
   a.tape_hdr = (const int*)tape; a.tape = (const R*)((const unsigned char*)tape + hdr);
   a.ctrl = (const R*)ctrl; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u; a.xT = (const R*)xT; a.dLdxT = (const R*)dLdxT;

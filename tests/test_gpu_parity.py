@@ -367,3 +367,47 @@ def test_gpu_closed_form_single_contact_and_free_flight(B):
         assert np.abs(La - Lb).max() < 1e-8 * max(1.0, np.abs(La).max())
         assert abs((Ib * a[10:13] ** 2).sum() - (Ib * b[10:13] ** 2).sum()) < 1e-8
         assert abs(np.linalg.norm(b[3:7]) - 1.0) < 1e-12
+
+
+@pytest.mark.parametrize("cfg", ["C2", "C3"])
+def test_layout_and_factor_reuse_invariance(B, cfg, monkeypatch):
+    """Implementation choices that must not change a bit of the forward pass, nor the gradients beyond rounding:
+    constant arena in shared vs global memory (DMX_ARENA_SMEM), padded leading dimensions / staggered group slices
+    (DMX_PAD), and the VJP reusing the Newton solve's Cholesky factor vs rebuilding H (DMX_DBG=8).  Every variant
+    performs the same floating-point operations per entry, so all outputs are compared bitwise, except the factor
+    reuse, which is compared to 1e-12 (the rebuilt H is summed by differently compiled code)."""
+    import torch
+    kw = dict(SMALL[cfg]); kw["nenv"] = 40
+    w = W.make(cfg, **kw)
+    nenv = w["nenv"]
+
+    def run(env):
+        for k in ("DMX_ARENA_SMEM", "DMX_PAD", "DMX_DBG"):
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        m = B.Model(w["model"])
+        x0, ctrl = m.dev(w["x0"]), m.dev(w["ctrl"])
+        stats = m.alloc_stats(nenv)
+        xT = m.rollout(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], stats=stats)
+        torch.cuda.synchronize()
+        nmax = int(stats["n_accept"].max().item())
+        tape = m.alloc_tape(nenv, nmax + 8); tape.zero_()
+        g = m.dev(np.random.default_rng(11).standard_normal((nenv, w["x0"].shape[1])))
+        out = m.rollout_grad(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], g, cfg == "C2", tape, stats=stats)
+        torch.cuda.synchronize()
+        return xT, out, tape
+
+    xT0, out0, tape0 = run({})
+    assert float(out0["dLdx0"].abs().max()) > 0
+    keys = [k for k in ("dLdx0", "dLdctrl", "dLdparams") if out0[k] is not None]   # C3 has no controls
+    for env in ({"DMX_ARENA_SMEM": "0"}, {"DMX_PAD": "1"}):
+        xT, out, tape = run(env)
+        assert torch.equal(xT, xT0) and torch.equal(tape, tape0), env
+        for k in keys:
+            assert torch.equal(out[k], out0[k]), (env, k)
+    xT, out, tape = run({"DMX_DBG": "8"})
+    assert torch.equal(xT, xT0) and torch.equal(tape, tape0)
+    for k in keys:
+        e = _rel_grad_err(out[k].cpu().numpy(), out0[k].cpu().numpy())
+        assert e.max() <= 1e-12, k
