@@ -261,7 +261,7 @@ struct dmx_model {
   Arena arena;
   ModelDev<double> md; ModelDev<float> mf;
   WsLayout wl, rwl; RkLayout rl;
-  struct Cfg { int block = 0, occ = 0; size_t smem = 0; } cf, cb, cx;   // forward, backward, field kernels
+  struct Cfg { int block = 0, occ = 0; size_t smem = 0; int arena = 0 /* constant arena in this kernel's shared memory */; } cf, cb, cx;   // forward, backward, field kernels
   void* rk_scratch = nullptr; size_t rk_scratch_bytes = 0;              // backward integrator arrays (global memory)
   int* queue = nullptr;            // [4] work-queue counters
   void* zero_u = nullptr;          // zeros: controls when ctrl == NULL, velocities at create
@@ -361,16 +361,16 @@ int create_typed(dmx_model* m) {
     if (!(ea && std::atoi(ea) == 0)) {
       if (int rc = select(m->arena.host.size(), af, abk, ax)) return rc;
       auto res = [&](const Cfg& c) { return c.occ * groups_per_block(m, std::max(c.block, 1)); };
-      if (af.occ >= 1 && abk.occ >= 1 && ax.occ >= 1 && res(af) >= res(m->cf) && res(abk) >= res(m->cb)) {
-        m->cf = af; m->cb = abk; m->cx = ax;
-        if (sizeof(R) == 8) m->md.arena_smem = 1; else m->mf.arena_smem = 1;
-      }
+      // per kernel: the arena goes to shared memory where it costs no resident lane group
+      if (af.occ >= 1 && res(af) >= res(m->cf)) { m->cf = af; m->cf.arena = 1; }
+      if (abk.occ >= 1 && res(abk) >= res(m->cb)) { m->cb = abk; m->cb.arena = 1; }
+      if (ax.occ >= 1 && res(ax) >= res(m->cx)) { m->cx = ax; m->cx.arena = 1; }
     }
   }
   if (m->cf.occ < 1 || m->cb.occ < 1 || m->cx.occ < 1) return fail("model too large for the per-environment shared-memory workspace (try DMX_LANES=32)");
   if (std::getenv("DMX_VERBOSE"))
-    std::fprintf(stderr, "dmx: arena %zu B in %s | lanes %d | fwd block %d x occ %d smem %zu | bwd block %d x occ %d smem %zu | field block %d x occ %d smem %zu | group bytes f/b %zu/%zu\n",
-                 m->arena.host.size(), (m->precision == 64 ? m->md.arena_smem : m->mf.arena_smem) ? "smem" : "global", m->G, m->cf.block, m->cf.occ, m->cf.smem, m->cb.block, m->cb.occ, m->cb.smem, m->cx.block, m->cx.occ, m->cx.smem, group_bytes(m, 0), group_bytes(m, 1));
+    std::fprintf(stderr, "dmx: arena %zu B, in smem fwd/bwd/field %d/%d/%d | lanes %d | fwd block %d x occ %d smem %zu | bwd block %d x occ %d smem %zu | field block %d x occ %d smem %zu | group bytes f/b %zu/%zu\n",
+                 m->arena.host.size(), m->cf.arena, m->cb.arena, m->cx.arena, m->G, m->cf.block, m->cf.occ, m->cf.smem, m->cb.block, m->cb.occ, m->cb.smem, m->cx.block, m->cx.occ, m->cx.smem, group_bytes(m, 0), group_bytes(m, 1));
   // the occupancy queries above left the largest attribute set; restore the chosen sizes
   int d0, d1, d2;
   CUDA_OK(L.occupancy(m->cf.block, m->cf.smem, m->cb.smem, m->cx.smem, &d0, &d1, &d2));
@@ -409,7 +409,8 @@ int rollout_typed(const dmx_model* m, int nenv, const void* x0, const void* ctrl
   LaunchCfg c; c.block = m->cf.block; c.smem = m->cf.smem;
   int gpb = groups_per_block(m, c.block);
   c.grid = std::max(1, std::min(m->cf.occ * m->sm_count, (nenv + gpb - 1) / gpb));
-  CUDA_OK(launchers_for<R>(m->G).rollout(dev_of<R>(m), a, c, s));
+  ModelDev<R> md = dev_of<R>(m); md.arena_smem = m->cf.arena;
+  CUDA_OK(launchers_for<R>(m->G).rollout(md, a, c, s));
   return 0;
 }
 
@@ -436,7 +437,8 @@ int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const vo
   a.rk_scratch = (double*)m->rk_scratch;
   CUDA_OK(cudaMemsetAsync(m->queue + 1, 0, sizeof(int), s));
   if (dLdctrl && nknot > 0 && m->h.nu > 0) CUDA_OK(cudaMemsetAsync(dLdctrl, 0, (size_t)nenv * nknot * m->h.nu * sizeof(R), s));
-  CUDA_OK(launchers_for<R>(m->G).backward(dev_of<R>(m), a, c, s));
+  ModelDev<R> md = dev_of<R>(m); md.arena_smem = m->cb.arena;
+  CUDA_OK(launchers_for<R>(m->G).backward(md, a, c, s));
   return 0;
 }
 
@@ -450,7 +452,8 @@ int field_typed(dmx_model* m, int n, const void* x, const void* u, const void* p
   LaunchCfg c; c.block = m->cx.block; c.smem = m->cx.smem;
   int gpb = groups_per_block(m, c.block);
   c.grid = std::max(1, std::min(m->cx.occ * m->sm_count, (n + gpb - 1) / gpb));
-  CUDA_OK(launchers_for<R>(m->G).field(dev_of<R>(m), a, c, s));
+  ModelDev<R> md = dev_of<R>(m); md.arena_smem = m->cx.arena;
+  CUDA_OK(launchers_for<R>(m->G).field(md, a, c, s));
   return 0;
 }
 
