@@ -505,6 +505,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
       for (int j = 0; j < nv; ++j) t = t + ws.J()[i * ld + j] * ws.x()[j];
       ws.s()[i] = t - ws.aref()[i];
       ws.active()[i] = val(ws.s()[i]) < 0 ? 1 : 0;     // the set the factor left in Hc belongs to (reused by vjp_prepare)
+      ws.pr()[i] = val(ws.s()[i]) < 0 ? ws.D()[i] : S(0.0);   // masked weight (pr is free until the step direction is known): branch-free sums below
     }
 #pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) ws.xa()[j] = ws.x()[j] - ws.a0()[j];
@@ -515,7 +516,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
 #pragma unroll 4
       for (int b = 0; b < nv; ++b) t = t + ws.M()[a * ld + b] * ws.xa()[b];
 #pragma unroll 4
-      for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.J()[i * ld + a] * ws.D()[i] * ws.s()[i];
+      for (int i = 0; i < nr; ++i) t = t + ws.J()[i * ld + a] * ws.pr()[i] * ws.s()[i];
       ws.g()[a] = t; ws.dl()[a] = -t;
     }
 #pragma unroll 1
@@ -523,7 +524,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
       int a, b; tri_index(e, a, b);
       S t = ws.M()[a * ld + b];
 #pragma unroll 4
-      for (int i = 0; i < nr; ++i) if (val(ws.s()[i]) < 0) t = t + ws.D()[i] * ws.J()[i * ld + a] * ws.J()[i * ld + b];
+      for (int i = 0; i < nr; ++i) t = t + ws.pr()[i] * ws.J()[i * ld + a] * ws.J()[i * ld + b];
       ws.Hc()[a * ld + b] = t;
     }
     gr.sync();
@@ -649,6 +650,7 @@ DMX_DN bool vjp_prepare(int nv, int nr, bool hc_valid, const WS& ws, const Grp<G
     const int act = val(t) < 0 ? 1 : 0;
     if (hc_valid && ws.active()[i] != act) same = false;
     ws.active()[i] = act;
+    ws.pr()[i] = act ? ws.D()[i] : S(0.0);               // masked weight for the branch-free H build (pr is rewritten by vjp_velocity)
   }
   const bool reuse = gr.all(same);
   gr.sync();
@@ -658,7 +660,7 @@ DMX_DN bool vjp_prepare(int nv, int nr, bool hc_valid, const WS& ws, const Grp<G
       int a, b; tri_index(e, a, b);
       S t = ws.M()[a * ld + b];
 #pragma unroll 4
-      for (int i = 0; i < nr; ++i) if (ws.active()[i]) t = t + ws.D()[i] * ws.J()[i * ld + a] * ws.J()[i * ld + b];
+      for (int i = 0; i < nr; ++i) t = t + ws.pr()[i] * ws.J()[i * ld + a] * ws.J()[i * ld + b];
       ws.Hc()[a * ld + b] = t;
     }
     gr.sync();
