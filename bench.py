@@ -36,7 +36,7 @@ FLOPS_PER_FEVAL = dict(C1=1e2, C2=8e3, C3=2e4, C4=8e4, C5=6e4)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full captures of the default workload
 # (profiles/r1_rollout_kernel.md, profiles/r1_backward_kernel.md); other workloads were not captured.
-NCU_TRAFFIC_C2_F64_4096 = {"rollout_kernel": 0.576e9, "backward_kernel": 0.724e9}
+NCU_TRAFFIC_C2_F64_4096 = {"rollout_kernel": 0.571e9, "backward_kernel": 0.716e9}
 
 
 def grad_flops_per_accepted(cfg, cfd):
