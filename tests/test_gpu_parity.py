@@ -411,3 +411,24 @@ def test_layout_and_factor_reuse_invariance(B, cfg, monkeypatch):
     for k in keys:
         e = _rel_grad_err(out[k].cpu().numpy(), out0[k].cpu().numpy())
         assert e.max() <= 1e-12, k
+
+
+@pytest.mark.parametrize("which", [W.DOPRI5, W.TSIT5])
+def test_gpu_chart_rate_keeps_order_five_on_a_tumbling_body(B, which):
+    """Reading G10 on the CUDA path itself (no oracle involved): fixed steps n = 20/40/80 of a torque-free asymmetric box
+    with |omega| = 6 rad/s against the path's own rtol = 1e-13 run; the slope must be 5 (a wrong 1/2 or 1/12 coefficient of
+    the chart rate gives 2 or 3, see tests/test_oracle_integrator.py::test_chart_rate_keeps_order_five_on_a_tumbling_body)."""
+    import torch
+    from test_oracle_integrator import _tumbling_box_case
+    m = B.Model(H.free_box())
+    x0 = m.dev(_tumbling_box_case()); T = 1.0
+    ref = m.rollout(x0, None, 0, 0.0, None, T, W.default_opts(W.TSIT5, 1e-13, 1e-13, h0=1e-3)).cpu().numpy()[0]
+    errs = []
+    for n in (20, 40, 80):
+        st = m.alloc_stats(1)
+        hs = torch.full((1, n), T / n, dtype=torch.float64, device=x0.device)
+        xT = m.rollout(x0, None, 0, 0.0, None, T, W.default_opts(which), h_replay=hs, stats=st).cpu().numpy()[0]
+        assert int(st["n_accept"][0]) == n
+        errs.append(np.abs(xT - ref).max())
+    slopes = np.log2(np.array(errs[:-1]) / np.array(errs[1:]))
+    assert np.all(slopes > 4.7) and np.all(slopes < 5.6), (errs, slopes)

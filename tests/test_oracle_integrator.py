@@ -166,3 +166,119 @@ def test_kinetic_energy_two_ways(oracle_mod):
         # armature is joint-space only
         arm_ = sum(model["jnt_armature"][j] * v[model["jnt_vadr"][j]] ** 2 * 0.5 for j in range(model["njnt"]) if model["jnt_type"][j] != W.JNT_FREE)
         assert abs(0.5 * v @ M @ v - T - arm_) < 1e-12 * max(1, T)
+
+
+def _tumbling_box_case():
+    """Torque-free ASYMMETRIC box (principal inertias all different, COM offset), |omega| = 6 rad/s, no contacts."""
+    rng = np.random.default_rng(5)
+    w = rng.normal(size=3); w *= 6.0 / np.linalg.norm(w)
+    return np.concatenate([[0, 0, 0.5], H.rand_quat(rng), rng.normal(size=3), w])[None]
+
+
+@pytest.mark.parametrize("which", [W.DOPRI5, W.TSIT5])
+def test_chart_rate_keeps_order_five_on_a_tumbling_body(oracle_mod, which):
+    """Pin of reading G10 ("exact integration of quaternions"; PAPER.md:456 order-p consistency): with
+    tangent-space stages Q_i = q_n (+) Theta_i the rotational chart rate must be dexp^-1 truncated after B_2,
+        Theta' = w + 1/2 Theta x w + 1/12 Theta x (Theta x w),
+    for the pair to keep order 5 on a body whose angular velocity changes direction.  Fixed steps n = 20/40/80 over
+    1 s against a free-running rtol = 1e-13 solution.  Measured slopes (log2 of successive error ratios), this test's
+    input, oracle as committed: Dopri5 4.99 / 5.00, Tsit5 5.25 / 4.93.  With the oracle's chart_rate mutated:
+        1/12 term removed        -> 3.02 / 3.00   (fails)
+        1/12 replaced by 1/6     -> 3.02 / 3.01   (fails)
+        1/2 term removed         -> 2.02 / 2.07   (fails)
+    P10 cannot see these terms (Theta || w there) and the adaptive invariants of P4 only take smaller steps."""
+    orc = oracle_mod.Oracle(H.free_box())
+    x0 = _tumbling_box_case(); T = 1.0
+    ref = orc.rollout(x0, None, 0, 0.0, None, T, W.default_opts(W.TSIT5, 1e-13, 1e-13, h0=1e-3))
+    assert ref["stats"]["status"][0] == 0
+    errs = []
+    for n in (20, 40, 80):
+        r = orc.rollout(x0, None, 0, 0.0, None, T, W.default_opts(which), h_replay=np.full((1, n), T / n))
+        assert r["stats"]["n_accept"][0] == n
+        errs.append(np.abs(r["xT"][0] - ref["xT"][0]).max())
+    slopes = np.log2(np.array(errs[:-1]) / np.array(errs[1:]))
+    assert np.all(slopes > 4.7) and np.all(slopes < 5.6), (errs, slopes)
+
+
+def _controller_replica(A, tab, y0, T, nknot, knot_dt, o, max_attempts=400):
+    """Adaptive integration of the LINEAR system y' = A y written out with NumPy from DESIGN.md G12 / G2 (not from the
+    oracle's code): stages by the tableau, e = h sum (b - bhat)_i k_i, scale = atol + rtol max(|y_n|, |y_n+1|),
+    E = sqrt(mean((e/scale)^2)), accept iff E <= 1, fac = clip(safety E^(-(P+I)/5) E_prev^(P/5), fac_min, fac_max),
+    fac = fac_min when the attempt is not finite, E floored at 1e-30, E_prev updated on accept only, h <- h fac after
+    accept and after reject EXCEPT after an accepted step that was clipped to a knot / the horizon (the proposal is
+    kept), steps clipped to knot boundaries when h (1 + 1e-7) >= remaining."""
+    c, a, b, e = tab
+    t, y, hprop, Eprev, knot = 0.0, np.array(y0, dtype=float), o["h0"], 1.0, 0
+    hs, nrej = [], 0
+    for _ in range(max_attempts):
+        if not t < T:
+            break
+        tb = min((knot + 1) * knot_dt, T) if nknot > 0 else T
+        if knot + 1 >= nknot:
+            tb = T
+        rem = tb - t
+        hits = hprop * (1 + 1e-7) >= rem
+        h = rem if hits else hprop
+        with np.errstate(all="ignore"):
+            k = []
+            for i in range(7):
+                Yi = y + h * sum((a[i, l] * k[l] for l in range(i)), np.zeros(2))
+                k.append(A @ Yi)
+            y1 = y + h * sum((a[6, l] * k[l] for l in range(6)), np.zeros(2))
+            err = h * sum((e[i] * k[i] for i in range(7)), np.zeros(2))
+            finite = bool(np.all(np.isfinite(err)) and np.all(np.isfinite(np.array(k))))
+            if finite:
+                E = np.sqrt(np.mean((err / (o["atol"] + o["rtol"] * np.maximum(np.abs(y), np.abs(y1)))) ** 2))
+                accept = E <= 1.0
+                Ec = max(E, 1e-30)
+                fac = o["safety"] * Ec ** (-(o["pcoeff"] + o["icoeff"]) / 5.0) * Eprev ** (o["pcoeff"] / 5.0)
+            else:
+                accept, Ec, fac = False, np.inf, o["fac_min"]
+        fac = min(o["fac_max"], max(o["fac_min"], fac))
+        if (not accept) or (not hits):
+            hprop = h * fac
+        if not accept:
+            nrej += 1
+            continue
+        Eprev = Ec
+        hs.append(h); y = y1
+        if hits:
+            t = tb
+            if tb < T:
+                knot += 1
+        else:
+            t += h
+    return np.array(hs), nrej, y
+
+
+@pytest.mark.parametrize("which", [W.DOPRI5, W.TSIT5])
+@pytest.mark.parametrize("case", ["knots_and_rejections", "non_finite_start"])
+def test_controller_step_sequence_matches_hand_computation(oracle_mod, which, case):
+    """Pin of reading G12 / G2 (PAPER.md:347 fixes only P = 0.2, I = 0.4, D = 0): the oracle's accepted step sizes and
+    reject count on m q'' = -kp q against the replica above.  Swapping the two exponents, dropping E_prev, updating
+    E_prev on rejects, or letting a clipped accepted step overwrite the proposal changes the h sequence."""
+    m, kp = 1.3, 7.0
+    orc = oracle_mod.Oracle(H.oscillator(m, kp))
+    A = np.array([[0.0, 1.0], [-kp / m, 0.0]])
+    tab = oracle_mod.tableau(which)
+    if case == "knots_and_rejections":     # h0 far too large: rejections first; 4 knots clip accepted steps
+        o = W.default_opts(which, 1e-7, 1e-7, h0=0.9); T, nknot, knot_dt = 2.0, 4, 0.5
+    else:                                  # h0 = 1e60 on an unreachable horizon: stages overflow -> non-finite -> fac_min until
+        o = W.default_opts(which, 1e-6, 1e-6, h0=1e60, max_steps=120); T, nknot, knot_dt = 1e70, 1, 1e80   # finite; stopped by the budget
+    x0 = np.array([[0.8, -0.3]])
+    r = orc.rollout(x0, np.zeros((1, nknot, 1)), nknot, knot_dt, None, T, o, n_hout=400)
+    hs, nrej, yT = _controller_replica(A, tab, x0[0], T, nknot, knot_dt, o, max_attempts=o["max_steps"])
+    na = int(r["stats"]["n_accept"][0])
+    assert r["stats"]["status"][0] == (0 if case == "knots_and_rejections" else 1)      # 1: step budget (PAPER.md:377)
+    assert na == len(hs) and int(r["stats"]["n_reject"][0]) == nrej
+    assert nrej >= (3 if case == "knots_and_rejections" else 80) and na >= 10
+    # The first dozen accepted steps agree to rounding.  Later ones only to ~1e-5: a step clipped to a knot can be tiny,
+    # its error estimate is then rounding noise, and that noise enters the next factors through E_prev^(P/5).
+    assert np.abs(r["h"][0, :12] - hs[:12]).max() <= 1e-9 * hs.max()
+    assert np.abs(r["h"][0, :na] - hs).max() <= 2e-4 * hs.max()
+    assert np.abs(r["xT"][0] - yT).max() < 1e-9
+    if case == "knots_and_rejections":
+        # at least one accepted step was clipped to a knot and the next step resumed with the unclipped proposal
+        ends = np.cumsum(hs)
+        clipped = [i for i in range(len(hs) - 1) if abs(ends[i] / knot_dt - round(ends[i] / knot_dt)) < 1e-12 and hs[i + 1] > hs[i] * 1.0000001]
+        assert clipped
