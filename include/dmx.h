@@ -13,8 +13,13 @@
  *     tape); h_replay and all statistics are always double / int.
  *   - State x = [q | v]: q[nq] (free joint: 3 position + unit quaternion
  *     w,x,y,z; hinge / slide: one scalar), v[nv] (free joint: world linear, body angular).
- *   - Calls only enqueue work on `cuda_stream`; they do not synchronise.  One call may be in
- *     flight per dmx_model at a time (the model owns the work-queue counters and scratch).
+ *   - Calls only enqueue work on `cuda_stream`; they do not synchronise and do not allocate (all
+ *     scratch is sized at dmx_model_create).  Calls on one model may be issued on different
+ *     streams: each call takes its own work-queue counter (up to 64 calls in flight), and a reverse
+ *     sweep waits (cudaStreamWaitEvent) for the previous reverse sweep of the same model, whose
+ *     adjoint scratch it reuses.  dmx_model_set_tape_stages must not change between the rollout
+ *     that writes a tape and the sweep that reads it; the tape records its layout and a sweep over
+ *     a tape of another layout, batch size or plan returns zero gradients.
  *   - Return value: 0 ok; <0 invalid argument / CUDA error (text via dmx_last_error()).
  *     Numerical trouble inside one environment never fails a call, it is reported in
  *     stats.status[e]: 0 ok, 1 step budget exceeded, 2 step-size
@@ -79,10 +84,18 @@ typedef struct {
   int max_steps;        /* budget of attempted steps per environment */
 } dmx_solver_opts;
 
-/* Per-environment step statistics; DEVICE pointers, each [nenv]; any may be NULL. */
+/* Per-environment step statistics; DEVICE pointers, each [nenv]; any may be NULL.
+ * n_newton_unconverged: F evaluations of the forward pass whose fixed-iteration Newton solve did not
+ * end on a full step inside an unchanged active set.  n_newton_unconverged_bwd: the same count over the contact solves
+ * of the reverse sweep (F~ with cfd_on, or F when the stages are recomputed); the vector-Jacobian product of such a stage
+ * is the implicit-function gradient at a point that is not stationary (reading G9). */
 typedef struct {
   int *n_accept, *n_reject, *n_feval, *n_newton_unconverged, *status;
   double *h_min, *h_max, *t_end;
+  int *n_newton_unconverged_bwd;
+  unsigned long long *work;   /* [nenv][6]: work actually done, for the roofline numerator: Newton iterations,
+                                 row-iterations (sum over iterations of the rows in the solve) and rows (sum over
+                                 evaluations of the rows built) of the forward pass [0..2] and of the reverse sweep [3..5] */
 } dmx_stats;
 
 /* Builds the device model.  precision: 64 (double) or 32 (float stage arithmetic; time, step
@@ -101,14 +114,29 @@ int dmx_model_default_params(const dmx_model *m, double *p_host);
 /* Lanes per environment the kernels use for this model (1, 8, 16 or 32). */
 int dmx_model_lanes(const dmx_model *m);
 
-/* Tape record per accepted step: the checkpoint (y_n, t_n, h_n), nq+nv+2 reals, and - by
+/* Tape record per accepted step (padded to 16 bytes, written with 16-byte stores): the checkpoint (y_n as nq+nv reals;
+ * t_n, h_n as two doubles in both precisions), and - by
  * default - the six stage rates A_1..A_6 (6*nv reals), so that the reverse sweep rebuilds the stage states without
  * re-evaluating F (memory for time, the checkpoint-count knob of PAPER.md:371).  on = 0 keeps the checkpoint only and
  * the reverse sweep recomputes the stages with six F evaluations per step.  Set before sizing / writing a tape. */
 int dmx_model_set_tape_stages(dmx_model *m, int on);
 
-/* Bytes of tape for nenv environments with room for tape_steps accepted steps each. */
+/* Bytes of tape for nenv environments with room for tape_steps accepted steps each (uniform slots; no plan). */
 size_t dmx_tape_bytes(const dmx_model *m, int nenv, int tape_steps);
+
+/* Launch plan (optional; "the batched loop waits for the slowest environment", PAPER.md:371 memory =
+ * checkpoints x state size).  From the accepted-step counts n_accept[nenv] (DEVICE, e.g. the stats of a previous or
+ * sizing pass) dmx_tape_plan writes into `plan` (DEVICE buffer of dmx_plan_bytes(nenv)):
+ *   - the hand-out order of the work queue: environments by descending n_accept, so the longest chains start first;
+ *   - per-environment tape slots of cap(e) = n_accept[e] + n_accept[e]*margin_pct/100 + pad records at the exclusive
+ *     prefix sum of the caps, so that the tape holds sum(cap) records instead of nenv * max(cap).
+ * The total is dmx_tape_bytes_records(m, nenv, sum_e cap(e)); the caller sizes the tape with the same integer formula.
+ * A slot that does not fit the tape buffer, or an environment that outgrows its slot, ends with status 4 (tape full).
+ * Pass the same plan to the rollout that writes a tape and to the sweep that reads it.  Enqueues one kernel. */
+size_t dmx_plan_bytes(int nenv);
+size_t dmx_tape_bytes_records(const dmx_model *m, int nenv, long long total_records);
+int dmx_tape_plan(const dmx_model *m, int nenv, const int *n_accept, int margin_pct, int pad, void *plan,
+                  size_t plan_bytes, void *cuda_stream);
 
 /* Forward rollout (PAPER.md:41 x_{k+1}=step(x_k,a_k,p); Eq. 5 at PAPER.md:422-425): integrates
  * every environment from t=0 to `horizon` with its own error-controlled step size
@@ -120,11 +148,12 @@ size_t dmx_tape_bytes(const dmx_model *m, int nenv, int tape_steps);
  *           (a non-positive entry ends the rollout), no error control
  *   xT      device [nenv, nq+nv] real (out)
  *   stats   device arrays (out), may be NULL
- *   tape    device buffer of tape_bytes, or NULL for no tape */
+ *   tape    device buffer of tape_bytes (16-byte aligned), or NULL for no tape
+ *   plan    device buffer written by dmx_tape_plan, or NULL (identity order, uniform tape slots) */
 int dmx_rollout(const dmx_model *m, int nenv, const void *x0, const void *ctrl, int nknot, double knot_dt,
                 const void *params, double horizon, const dmx_solver_opts *opts, const double *h_replay,
                 int n_replay, void *xT, const dmx_stats *stats, void *tape, size_t tape_bytes,
-                void *cuda_stream);
+                const void *plan, void *cuda_stream);
 
 /* Forward rollout with tape, then the reverse sweep through the accepted steps with frozen
  * step sizes (discretize-then-optimize).  With cfd_on the vector-Jacobian
@@ -140,13 +169,16 @@ int dmx_rollout(const dmx_model *m, int nenv, const void *x0, const void *ctrl, 
 int dmx_rollout_grad(const dmx_model *m, int nenv, const void *x0, const void *ctrl, int nknot, double knot_dt,
                      const void *params, double horizon, const dmx_solver_opts *opts, const double *h_replay,
                      int n_replay, const void *dLdxT, int cfd_on, void *xT, void *dLdx0, void *dLdctrl,
-                     void *dLdparams, const dmx_stats *stats, void *tape, size_t tape_bytes, void *cuda_stream);
+                     void *dLdparams, const dmx_stats *stats, void *tape, size_t tape_bytes, const void *plan,
+                     void *cuda_stream);
 
-/* Reverse sweep only, over a tape written by dmx_rollout with the same inputs. */
+/* Reverse sweep only, over a tape written by dmx_rollout with the same inputs (and the same plan).
+ *   stats   NULL, or: stats->status (in, [nenv] or NULL) marks environments to skip (non-zero: zero gradients);
+ *           stats->n_newton_unconverged_bwd (out, [nenv] or NULL).  Other fields are ignored. */
 int dmx_rollout_backward(const dmx_model *m, int nenv, const void *ctrl, int nknot, const void *params,
                          const dmx_solver_opts *opts, const void *xT, const void *dLdxT, int cfd_on,
-                         void *dLdx0, void *dLdctrl, void *dLdparams, const int *status /* device [nenv] or NULL */,
-                         const void *tape, size_t tape_bytes, void *cuda_stream);
+                         void *dLdx0, void *dLdctrl, void *dLdparams, const dmx_stats *stats,
+                         const void *tape, size_t tape_bytes, const void *plan, void *cuda_stream);
 
 /* Building blocks exposed for parity tests (one lane-group per state, same device code as the
  * rollouts).  All pointers DEVICE, real typed; n states.

@@ -13,7 +13,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("DMX_LIB", os.path.join(_HERE, "libdmx.so"))
 
 SYMBOLS = ["dmx_model_create", "dmx_model_destroy", "dmx_model_set_tape_stages", "dmx_model_np", "dmx_model_nc", "dmx_model_default_params",
-           "dmx_model_lanes", "dmx_tape_bytes", "dmx_rollout", "dmx_rollout_grad", "dmx_rollout_backward",
+           "dmx_model_lanes", "dmx_tape_bytes", "dmx_tape_bytes_records", "dmx_plan_bytes", "dmx_tape_plan",
+           "dmx_rollout", "dmx_rollout_grad", "dmx_rollout_backward",
            "dmx_vector_field", "dmx_vjp_field", "dmx_fma_peak", "dmx_debug_counters", "dmx_last_error"]
 
 _pd, _pi = C.POINTER(C.c_double), C.POINTER(C.c_int)
@@ -44,7 +45,7 @@ class SolverOpts(C.Structure):
 class Stats(C.Structure):
     _fields_ = [("n_accept", C.c_void_p), ("n_reject", C.c_void_p), ("n_feval", C.c_void_p),
                 ("n_newton_unconverged", C.c_void_p), ("status", C.c_void_p),
-                ("h_min", C.c_void_p), ("h_max", C.c_void_p), ("t_end", C.c_void_p)]
+                ("h_min", C.c_void_p), ("h_max", C.c_void_p), ("t_end", C.c_void_p), ("n_newton_unconverged_bwd", C.c_void_p), ("work", C.c_void_p)]
 
 
 _lib = None
@@ -60,6 +61,11 @@ def load():
         L.dmx_last_error.restype = C.c_char_p
         L.dmx_tape_bytes.restype = C.c_size_t
         L.dmx_tape_bytes.argtypes = [C.c_void_p, C.c_int, C.c_int]
+        L.dmx_tape_bytes_records.restype = C.c_size_t
+        L.dmx_tape_bytes_records.argtypes = [C.c_void_p, C.c_int, C.c_longlong]
+        L.dmx_plan_bytes.restype = C.c_size_t
+        L.dmx_plan_bytes.argtypes = [C.c_int]
+        L.dmx_tape_plan.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
         L.dmx_model_create.argtypes = [C.POINTER(ModelDesc), C.c_int, C.POINTER(C.c_void_p)]
         L.dmx_model_destroy.argtypes = [C.c_void_p]
         for f in ("dmx_model_np", "dmx_model_nc", "dmx_model_lanes"):
@@ -67,10 +73,10 @@ def load():
         L.dmx_model_default_params.argtypes = [C.c_void_p, C.c_void_p]
         L.dmx_model_set_tape_stages.argtypes = [C.c_void_p, C.c_int]
         vp, i, d, sz = C.c_void_p, C.c_int, C.c_double, C.c_size_t
-        L.dmx_rollout.argtypes = [vp, i, vp, vp, i, d, vp, d, C.POINTER(SolverOpts), vp, i, vp, C.POINTER(Stats), vp, sz, vp]
+        L.dmx_rollout.argtypes = [vp, i, vp, vp, i, d, vp, d, C.POINTER(SolverOpts), vp, i, vp, C.POINTER(Stats), vp, sz, vp, vp]
         L.dmx_rollout_grad.argtypes = [vp, i, vp, vp, i, d, vp, d, C.POINTER(SolverOpts), vp, i, vp, i, vp, vp, vp, vp,
-                                       C.POINTER(Stats), vp, sz, vp]
-        L.dmx_rollout_backward.argtypes = [vp, i, vp, i, vp, C.POINTER(SolverOpts), vp, vp, i, vp, vp, vp, vp, vp, sz, vp]
+                                       C.POINTER(Stats), vp, sz, vp, vp]
+        L.dmx_rollout_backward.argtypes = [vp, i, vp, i, vp, C.POINTER(SolverOpts), vp, vp, i, vp, vp, vp, C.POINTER(Stats), vp, sz, vp, vp]
         L.dmx_vector_field.argtypes = [vp, i, vp, vp, vp, i, vp, vp, vp]
         L.dmx_vjp_field.argtypes = [vp, i, vp, vp, vp, vp, i, vp, vp, vp, vp, vp]
         L.dmx_fma_peak.argtypes = [i, i, _pd, _pd]
@@ -179,25 +185,41 @@ class Model:
                  n_newton_unconverged=T.zeros(nenv, dtype=T.int32, device=self.device),
                  status=T.zeros(nenv, dtype=T.int32, device=self.device),
                  h_min=T.zeros(nenv, dtype=T.float64, device=self.device), h_max=T.zeros(nenv, dtype=T.float64, device=self.device),
-                 t_end=T.zeros(nenv, dtype=T.float64, device=self.device))
+                 t_end=T.zeros(nenv, dtype=T.float64, device=self.device),
+                 n_newton_unconverged_bwd=T.zeros(nenv, dtype=T.int32, device=self.device),
+                 work=T.zeros((nenv, 6), dtype=T.int64, device=self.device))
         return s
 
     @staticmethod
     def _stats_struct(s):
         if s is None:
             return None
-        return Stats(*[s[k].data_ptr() for k in ("n_accept", "n_reject", "n_feval", "n_newton_unconverged", "status",
-                                                 "h_min", "h_max", "t_end")])
+        return Stats(*[(s[k].data_ptr() if s.get(k) is not None else None) for k in
+                       ("n_accept", "n_reject", "n_feval", "n_newton_unconverged", "status", "h_min", "h_max", "t_end", "n_newton_unconverged_bwd", "work")])
 
     def alloc_tape(self, nenv, tape_steps):
         return self.torch.empty(self.tape_bytes(nenv, tape_steps), dtype=self.torch.uint8, device=self.device)
+
+    def plan(self, n_accept, margin_pct=25, pad=16, stream=None):
+        """dmx_tape_plan on the accepted-step counts of a previous pass (device int32 [nenv]).  Returns (plan, tape):
+        the plan buffer and a tape sized for it - sum_e (n + n*margin_pct//100 + pad) records, the formula of dmx.h."""
+        T = self.torch
+        nenv = n_accept.shape[0]
+        n_accept = n_accept.to(device=self.device, dtype=T.int32).contiguous()
+        plan = T.empty(int(load().dmx_plan_bytes(nenv)), dtype=T.uint8, device=self.device)
+        if load().dmx_tape_plan(self.h, nenv, _ptr(n_accept), int(margin_pct), int(pad), _ptr(plan), plan.numel(), self._stream(stream)) != 0:
+            raise RuntimeError("dmx_tape_plan: " + _err())
+        n64 = n_accept.to(T.int64)
+        total = int((n64 + n64 * int(margin_pct) // 100 + int(pad)).sum().item())
+        tape = T.empty(int(load().dmx_tape_bytes_records(self.h, nenv, total)), dtype=T.uint8, device=self.device)
+        return plan, tape
 
     def _stream(self, stream):
         s = stream if stream is not None else self.torch.cuda.current_stream(self.device)
         return C.c_void_p(s.cuda_stream)
 
     # ---- the C-ABI calls (device tensors in, device tensors out) ---------------------------------
-    def rollout(self, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay=None, xT=None, stats=None, tape=None, stream=None):
+    def rollout(self, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay=None, xT=None, stats=None, tape=None, stream=None, plan=None):
         nenv = x0.shape[0]
         xT = self.torch.empty_like(x0) if xT is None else xT
         st = self._stats_struct(stats)
@@ -205,13 +227,14 @@ class Model:
         nrep = 0 if h_replay is None else h_replay.shape[1]
         rc = load().dmx_rollout(self.h, nenv, _ptr(x0), _ptr(ctrl), int(nknot), float(knot_dt), _ptr(params), float(horizon), C.byref(o),
                                 _ptr(h_replay), nrep, _ptr(xT), C.byref(st) if st else None, _ptr(tape),
-                                0 if tape is None else tape.numel(), self._stream(stream))
+                                0 if tape is None else tape.numel(), _ptr(plan), self._stream(stream))
         if rc != 0:
             raise RuntimeError("dmx_rollout: " + _err())
         return xT
 
     def rollout_backward(self, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, tape, want_params=True, status=None, stream=None,
-                         out=None):
+                         out=None, plan=None, stats=None):
+        """status: device int32 [nenv] marking environments to skip; stats: dict whose n_newton_unconverged_bwd is written."""
         T = self.torch
         nenv = xT.shape[0]
         if out is None:
@@ -219,15 +242,22 @@ class Model:
                        dLdctrl=T.empty((nenv, nknot, self.nu), dtype=self.dtype, device=self.device) if (ctrl is not None and nknot > 0) else None,
                        dLdparams=T.empty((nenv, self.np_), dtype=self.dtype, device=self.device) if want_params else None)
         o = _opts(opts)
+        st = Stats()
+        if status is not None:
+            st.status = status.data_ptr()
+        if stats is not None and stats.get("n_newton_unconverged_bwd") is not None:
+            st.n_newton_unconverged_bwd = stats["n_newton_unconverged_bwd"].data_ptr()
+        if stats is not None and stats.get("work") is not None:
+            st.work = stats["work"].data_ptr()
         rc = load().dmx_rollout_backward(self.h, nenv, _ptr(ctrl), int(nknot), _ptr(params), C.byref(o), _ptr(xT), _ptr(dLdxT), int(cfd_on),
-                                         _ptr(out["dLdx0"]), _ptr(out["dLdctrl"]), _ptr(out["dLdparams"]), _ptr(status), _ptr(tape),
-                                         tape.numel(), self._stream(stream))
+                                         _ptr(out["dLdx0"]), _ptr(out["dLdctrl"]), _ptr(out["dLdparams"]), C.byref(st), _ptr(tape),
+                                         tape.numel(), _ptr(plan), self._stream(stream))
         if rc != 0:
             raise RuntimeError("dmx_rollout_backward: " + _err())
         return out
 
     def rollout_grad(self, x0, ctrl, nknot, knot_dt, params, horizon, opts, dLdxT, cfd_on, tape, h_replay=None, want_params=True,
-                     stats=None, stream=None, out=None):
+                     stats=None, stream=None, out=None, plan=None):
         T = self.torch
         nenv = x0.shape[0]
         if out is None:
@@ -239,7 +269,7 @@ class Model:
         nrep = 0 if h_replay is None else h_replay.shape[1]
         rc = load().dmx_rollout_grad(self.h, nenv, _ptr(x0), _ptr(ctrl), int(nknot), float(knot_dt), _ptr(params), float(horizon), C.byref(o),
                                      _ptr(h_replay), nrep, _ptr(dLdxT), int(cfd_on), _ptr(out["xT"]), _ptr(out["dLdx0"]), _ptr(out["dLdctrl"]),
-                                     _ptr(out["dLdparams"]), C.byref(st) if st else None, _ptr(tape), tape.numel(), self._stream(stream))
+                                     _ptr(out["dLdparams"]), C.byref(st) if st else None, _ptr(tape), tape.numel(), _ptr(plan), self._stream(stream))
         if rc != 0:
             raise RuntimeError("dmx_rollout_grad: " + _err())
         return out

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <string>
 #include <vector>
+#include <atomic>
 #include <stdexcept>
 #include "../../include/dmx.h"
 #include "dmx_kernels.cuh"
@@ -28,20 +29,49 @@ template <class R> struct Launchers {
   cudaError_t (*occupancy)(int, size_t, size_t, size_t, int*, int*, int*);
   cudaError_t (*prof_dump)(unsigned long long*, cudaStream_t);
 };
-template <class R, int G> Launchers<R> make_launchers() {
+template <class R, int G, class SH> Launchers<R> make_launchers() {
   Launchers<R> l;
-  l.rollout = &launch_rollout<R, G>; l.backward = &launch_backward<R, G>; l.field = &launch_field<R, G>;
-  l.invweight = &launch_invweight<R, G>; l.occupancy = &kernel_occupancy<R, G>; l.prof_dump = &launch_prof_dump<R, G>;
+  l.rollout = &launch_rollout<R, G, SH>; l.backward = &launch_backward<R, G, SH>; l.field = &launch_field<R, G, SH>;
+  l.invweight = &launch_invweight<R, G, SH>; l.occupancy = &kernel_occupancy<R, G, SH>; l.prof_dump = &launch_prof_dump<R, G, SH>;
   return l;
 }
-template <class R> Launchers<R> launchers_for(int G) {
+// shape: 0 = sizes taken at run time; 2..5 = the static instantiation of BASELINE config C2..C5 (dmx_model.cuh)
+template <class R> Launchers<R> launchers_for(int G, int shape);
+template <> Launchers<double> launchers_for<double>(int G, int shape) {
+  if (shape == 2 && G == 8) return make_launchers<double, 8, ShapeC2>();
+  if (shape == 3 && G == 16) return make_launchers<double, 16, ShapeC3>();
+  if (shape == 4 && G == 32) return make_launchers<double, 32, ShapeC4>();
+  if (shape == 5 && G == 32) return make_launchers<double, 32, ShapeC5>();
   switch (G) {
-    case 1: return make_launchers<R, 1>();
-    case 8: return make_launchers<R, 8>();
-    case 16: return make_launchers<R, 16>();
-    default: return make_launchers<R, 32>();
+    case 1: return make_launchers<double, 1, ShapeDyn>();
+    case 8: return make_launchers<double, 8, ShapeDyn>();
+    case 16: return make_launchers<double, 16, ShapeDyn>();
+    default: return make_launchers<double, 32, ShapeDyn>();
   }
 }
+template <> Launchers<float> launchers_for<float>(int G, int shape) {
+  if (shape == 3 && G == 16) return make_launchers<float, 16, ShapeC3>();
+  switch (G) {
+    case 1: return make_launchers<float, 1, ShapeDyn>();
+    case 8: return make_launchers<float, 8, ShapeDyn>();
+    case 16: return make_launchers<float, 16, ShapeDyn>();
+    default: return make_launchers<float, 32, ShapeDyn>();
+  }
+}
+template <class SH> bool shape_matches(int nv, int nc, int nr) { return SH::NV == nv && SH::NC == nc && SH::NR == nr; }
+// static instantiation whose sizes equal the model's (DMX_STATIC=0 forces the run-time sizes)
+int pick_shape(int precision, int G, int nv, int nc, int nr) {
+  const char* e = std::getenv("DMX_STATIC");
+  if (e && std::atoi(e) == 0) return 0;
+  if (precision == 64 && G == 8 && shape_matches<ShapeC2>(nv, nc, nr)) return 2;
+  if (G == 16 && shape_matches<ShapeC3>(nv, nc, nr)) return 3;
+  if (precision == 64 && G == 32 && shape_matches<ShapeC4>(nv, nc, nr)) return 4;
+  // C5 (nv = 18): measured slower than the run-time sizes (the unrolled code no longer fits the instruction cache:
+  // stall_no_inst 30 %); selected only on request
+  if (e && std::atoi(e) == 2 && precision == 64 && G == 32 && shape_matches<ShapeC5>(nv, nc, nr)) return 5;
+  return 0;
+}
+int shape_ld(int shape, int nv) { return shape == 2 ? ShapeC2::LD : shape == 3 ? ShapeC3::LD : shape == 4 ? ShapeC4::LD : shape == 5 ? ShapeC5::LD : nv; }
 
 // ---- device arena: one allocation holding every constant array ------------------------------------------
 struct Arena {
@@ -180,18 +210,22 @@ void flatten(const dmx_model_desc* d, HostModel& h) {
 // or J, so an even leading dimension puts the lanes of a group on 2-4 banks; an odd one spreads them over all of them.
 // With 8 lanes per environment the slices of neighbouring groups are offset by 8 scalars modulo 16 doubles / 32 floats,
 // so the groups that share a shared-memory wavefront use complementary banks.
-void make_layouts(const HostModel& h, int G, int real_bytes, WsLayout& wl, WsLayout& rwl, RkLayout& rl) {
+// wl / rl: the full workspace (reverse sweep, field kernels).  wlf / rlf: the forward kernel's workspace, in which arrays
+// with disjoint lifetimes inside one F evaluation share storage (DMX_FWD_ALIAS=0: same as wl): the body velocities /
+// accelerations and the temporaries of the dynamics phase (wrenches, world inertias, twist table) are dead once M, c and
+// tau are known, and the arrays of the contact solve (H, J, row vectors, Newton vectors) are first written after that;
+// the arrays only the VJP touches are dropped.  Fewer bytes per environment = more resident lane groups per SM.
+void make_layouts(const HostModel& h, int G, int real_bytes, int static_ld, WsLayout& wl, WsLayout& wlf, RkLayout& rl, RkLayout& rlf) {
   const char* ep = std::getenv("DMX_PAD");
-  const bool pad = G > 1 && ep && std::atoi(ep) != 0;
-  const int ld = (pad && h.nv > 1 && h.nv % 2 == 0) ? h.nv + 1 : h.nv;
+  const bool pad = G > 1 && ep && std::atoi(ep) != 0 && static_ld == 0;
+  const int ld = static_ld ? static_ld : ((pad && h.nv > 1 && h.nv % 2 == 0) ? h.nv + 1 : h.nv);
   auto stagger = [&](int n, int scalar_bytes) { if (!pad || G != 8 || n == 0) return n; int mod = 64 / scalar_bytes * 2; while (n % mod != 8) ++n; return n; };
   const int nb = h.nbody, nv = h.nv, nq = h.nq, nc = std::max(h.nc, 1), nr = std::max(h.nrmax, 1);
-  std::memset(&wl, 0, sizeof(wl)); std::memset(&rwl, 0, sizeof(rwl)); std::memset(&rl, 0, sizeof(rl));
+  std::memset(&wl, 0, sizeof(wl)); std::memset(&wlf, 0, sizeof(wlf)); std::memset(&rl, 0, sizeof(rl));
   int o = 0;
   auto take = [&](int& f, int n) { f = o; o += n; };
   take(wl.fp, 3 * nb); take(wl.fR, 9 * nb); take(wl.fw, 3 * nb); take(wl.fal, 3 * nb); take(wl.fvp, 3 * nb); take(wl.fap, 3 * nb);
   take(wl.com, 3 * nb); take(wl.dax, 3 * nv); take(wl.dan, 3 * nv);
-  rwl = wl; rwl.size = 0;                                  // no per-lane tangent workspace any more (closed-form VJP)
   take(wl.Fb, 3 * nb); take(wl.Nb, 3 * nb); take(wl.Iw, 9 * nb); take(wl.Isub, 9 * nb); take(wl.tw, 3 * std::max(h.ntw, 1));
   wl.ld = ld;
   take(wl.M, nv * ld); take(wl.Hc, nv * ld); take(wl.tau, nv); take(wl.c, nv); take(wl.a0, nv); take(wl.x, nv); take(wl.g, nv);
@@ -212,6 +246,28 @@ void make_layouts(const HostModel& h, int G, int real_bytes, WsLayout& wl, WsLay
   take(rl.qb, nv); take(rl.vb, nv); take(rl.dbar, nv); take(rl.Vb, nv); take(rl.lam, 2 * nv); take(rl.delta, nv);
   take(rl.qbar, nv); take(rl.vbar, nv); take(rl.ubar, std::max(h.nu, 1)); take(rl.pbar, h.np); take(rl.gp, h.np);
   rl.size_bwd = stagger(o, 8);
+  wlf = wl; rlf = rl;
+  const char* ea = std::getenv("DMX_FWD_ALIAS");
+  if (ea && std::atoi(ea) == 0) return;
+  {
+    WsLayout& f = wlf;
+    o = 0;
+    take(f.fp, 3 * nb); take(f.fR, 9 * nb); take(f.com, 3 * nb); take(f.dax, 3 * nv); take(f.dan, 3 * nv);
+    take(f.M, nv * ld); take(f.tau, nv); take(f.c, nv); take(f.a0, nv);
+    take(f.cr, nc); take(f.cn, 3 * nc); take(f.cpos, 3 * nc); take(f.ct1, 3 * nc); take(f.ct2, 3 * nc);
+    take(f.cD, nc); take(f.cpost, nc); take(f.cbd, nc); take(f.cmu, nc);
+    const int base = o;
+    take(f.fw, 3 * nb); take(f.fal, 3 * nb); take(f.fvp, 3 * nb); take(f.fap, 3 * nb);       // kinematics -> dynamics
+    take(f.Fb, 3 * nb); take(f.Nb, 3 * nb); take(f.Iw, 9 * nb); take(f.Isub, 9 * nb); take(f.tw, 3 * std::max(h.ntw, 1));
+    const int endA = o;
+    o = base;                                                                                    // factor of M onwards
+    take(f.Hc, nv * ld); take(f.J, nr * ld); take(f.aref, nr); take(f.D, nr); take(f.s, nr); take(f.pr, nr);
+    take(f.x, nv); take(f.g, nv); take(f.dl, nv); take(f.Md, nv); take(f.xa, nv);
+    o = std::max(o, endA);
+    f.kap = f.cdD = f.cdpost = f.fox = f.fvx = base;     // VJP only: never touched by the forward kernel
+    f.size = stagger(o + nq + nv, real_bytes) - (nq + nv);
+    rlf.Yqr = o; rlf.Vr = o + nq;
+  }
 }
 
 template <class R> size_t add_real(Arena& a, const std::vector<double>& v) {
@@ -256,14 +312,18 @@ template <class R> void build_dev(const HostModel& h, Arena& ar, ModelDev<R>& m,
 
 // ---- the model object -------------------------------------------------------------------------------------
 struct dmx_model {
-  int precision, G, sm_count, max_smem, tape_stages = 1;
+  int precision, G, shape = 0, sm_count, max_smem, tape_stages = 1;
+  int fwd_rk_global = 0;           // forward integrator arrays in global memory (like the reverse sweep's) instead of shared memory
+  void* rk_scratch_fwd = nullptr;
   HostModel h;
   Arena arena;
   ModelDev<double> md; ModelDev<float> mf;
-  WsLayout wl, rwl; RkLayout rl;
+  WsLayout wl, wlf; RkLayout rl, rlf;      // full / forward-kernel workspaces (make_layouts)
   struct Cfg { int block = 0, occ = 0; size_t smem = 0; int arena = 0 /* constant arena in this kernel's shared memory */; } cf, cb, cx;   // forward, backward, field kernels
-  void* rk_scratch = nullptr; size_t rk_scratch_bytes = 0;              // backward integrator arrays (global memory)
-  int* queue = nullptr;            // [4] work-queue counters
+  void* rk_scratch = nullptr; size_t rk_scratch_bytes = 0;              // backward integrator arrays (global memory), sized at create
+  cudaEvent_t bwd_done = nullptr;  // reverse sweeps of one model share rk_scratch: a sweep waits for the previous one
+  int* queue = nullptr;            // [N_QUEUE] work-queue counters, one per call in flight (round robin)
+  mutable std::atomic<unsigned> qnext{0};
   void* zero_u = nullptr;          // zeros: controls when ctrl == NULL, velocities at create
 };
 
@@ -274,21 +334,62 @@ size_t rsize(const dmx_model* m) { return m->precision == 64 ? sizeof(double) : 
 // shared memory of one lane group: kind 0 forward (integrator arrays + field workspace), 1 backward (field workspace
 // only; the integrator / adjoint arrays live in global memory), 2 field kernels (both)
 size_t group_bytes(const dmx_model* m, int kind) {
-  size_t rk = kind == 0 ? m->rl.size_fwd : (kind == 1 ? 0 : m->rl.size_bwd);
-  return rk * sizeof(double) + (size_t)(m->wl.size + m->rl.rsize) * rsize(m) + (size_t)m->wl.isize * sizeof(int);
+  size_t rk = kind == 0 ? (m->fwd_rk_global ? 0 : m->rl.size_fwd) : (kind == 1 ? 0 : m->rl.size_bwd);
+  const WsLayout& wl = kind == 0 ? m->wlf : m->wl;
+  return rk * sizeof(double) + (size_t)(wl.size + m->rl.rsize) * rsize(m) + (size_t)wl.isize * sizeof(int);
 }
 int groups_per_block(const dmx_model* m, int block) { return m->G == 1 ? block : block / m->G; }
 
-int ensure_scratch(dmx_model* m, int grid, int block, bool rk) {
-  if (rk) {
-    size_t need2 = (size_t)grid * block * (size_t)m->rl.size_bwd * sizeof(double);   // >= groups * size_bwd
-    if (need2 > m->rk_scratch_bytes) {
-      if (m->rk_scratch) cudaFree(m->rk_scratch);
-      m->rk_scratch = nullptr; m->rk_scratch_bytes = 0;
-      CUDA_OK(cudaMalloc(&m->rk_scratch, need2));
-      m->rk_scratch_bytes = need2;
-    }
+enum { N_QUEUE = 64, N_FWD_SCRATCH = 1 };
+int* next_queue(const dmx_model* m) { return m->queue + (m->qnext.fetch_add(1) % N_QUEUE); }
+
+// backward integrator arrays of every lane group the largest reverse-sweep grid can hold: allocated once at create, so
+// that dmx_rollout_backward only enqueues work
+int alloc_scratch(dmx_model* m) {
+  size_t groups = (size_t)m->cb.occ * m->sm_count * groups_per_block(m, m->cb.block);
+  if (m->G == 1) groups = (groups + 31) / 32 * 32;
+  m->rk_scratch_bytes = std::max<size_t>(groups * (size_t)m->rl.size_bwd * sizeof(double), 256);
+  CUDA_OK(cudaMalloc(&m->rk_scratch, m->rk_scratch_bytes));
+  CUDA_OK(cudaEventCreateWithFlags(&m->bwd_done, cudaEventDisableTiming));
+  if (m->fwd_rk_global) {
+    size_t gf = (size_t)m->cf.occ * m->sm_count * groups_per_block(m, m->cf.block);
+    if (m->G == 1) gf = (gf + 31) / 32 * 32;
+    CUDA_OK(cudaMalloc(&m->rk_scratch_fwd, std::max<size_t>(gf * (size_t)m->rl.size_fwd * sizeof(double), 256) * N_FWD_SCRATCH));
   }
+  return 0;
+}
+
+// ---- tape geometry ---------------------------------------------------------------------------------------------
+size_t align_up(size_t b, size_t a) { return (b + a - 1) / a * a; }
+size_t tape_header_bytes(int nenv) { return 256 + align_up((size_t)nenv * 2 * sizeof(int), 256); }
+template <class R> void tape_geometry(const dmx_model* m, TapeView<R>& tp) {
+  const int per16 = 16 / (int)sizeof(R), per8 = 8 / (int)sizeof(R), nx = m->h.nq + m->h.nv;
+  tp.o_th = (nx + per16 - 1) / per16 * per16;
+  int o = tp.o_th + 2 * per8;
+  tp.o_A = m->tape_stages ? o : -1;
+  if (m->tape_stages) o += 6 * m->h.nv;
+  tp.rec = (o + per16 - 1) / per16 * per16;
+}
+size_t record_bytes(const dmx_model* m) {
+  if (m->precision == 64) { TapeView<double> t; tape_geometry(m, t); return (size_t)t.rec * 8; }
+  TapeView<float> t; tape_geometry(m, t); return (size_t)t.rec * 4;
+}
+template <class R> int bind_tape(const dmx_model* m, int nenv, void* tape, size_t tape_bytes, const void* plan, TapeView<R>& tp, PlanView& pl) {
+  tape_geometry(m, tp);
+  std::memset(&pl, 0, sizeof(pl));
+  if (plan) {
+    const unsigned char* b = (const unsigned char*)plan;
+    size_t a4 = align_up((size_t)nenv * sizeof(int), 256);
+    pl.order = (const int*)(b + 256); pl.cap = (const int*)(b + 256 + a4); pl.offset = (const long long*)(b + 256 + 2 * a4);
+  }
+  tp.meta = nullptr; tp.hdr = nullptr; tp.data = nullptr; tp.capacity = 0; tp.uniform_cap = 0;
+  if (!tape) return 0;
+  size_t hdr = tape_header_bytes(nenv), rb = (size_t)tp.rec * sizeof(R);
+  if (tape_bytes < hdr + (plan ? rb : (size_t)nenv * rb)) return fail("tape too small");
+  if (((size_t)tape & 15) != 0) return fail("tape must be 16-byte aligned");
+  tp.meta = (int*)tape; tp.hdr = (int*)((unsigned char*)tape + 256); tp.data = (R*)((unsigned char*)tape + hdr);
+  tp.capacity = (long long)((tape_bytes - hdr) / rb);
+  tp.uniform_cap = (int)std::min<long long>(tp.capacity / nenv, (long long)1 << 30);
   return 0;
 }
 
@@ -301,7 +402,6 @@ SolverOpts opts_of(const dmx_solver_opts* o) {
   s.safety = o->safety; s.fac_min = o->fac_min; s.fac_max = o->fac_max; s.max_steps = o->max_steps;
   return s;
 }
-size_t tape_header_bytes(int nenv) { return (((size_t)nenv * 2 * sizeof(int)) + 255) & ~size_t(255); }
 
 template <class R>
 int create_typed(dmx_model* m) {
@@ -312,7 +412,7 @@ int create_typed(dmx_model* m) {
   CUDA_OK(cudaMalloc(&m->arena.dev, m->arena.host.size()));
   CUDA_OK(cudaMemcpy(m->arena.dev, m->arena.host.data(), m->arena.host.size(), cudaMemcpyHostToDevice));
   build_dev<R>(h, m->arena, dev, true);
-  Launchers<R> L = launchers_for<R>(m->G);
+  Launchers<R> L = launchers_for<R>(m->G, m->shape);
   // A^: body inverse weights at qpos0 on the device (same kinematics / mass-matrix / Cholesky code as the rollouts)
   std::vector<R> q0(h.nq); for (int i = 0; i < h.nq; ++i) q0[i] = (R)h.qpos0[i];
   R *dq0 = nullptr, *dw = nullptr;
@@ -329,7 +429,9 @@ int create_typed(dmx_model* m) {
   for (int i = 0; i < h.npair; ++i) { h.pair_invweight[i] = (double)bw[h.pair_body1[i]] + (double)bw[h.pair_body2[i]]; pw[i] = (R)h.pair_invweight[i]; }
   if (h.npair) CUDA_OK(cudaMemcpy(const_cast<R*>(dev.pair_invweight), pw.data(), sizeof(R) * h.npair, cudaMemcpyHostToDevice));
   if (sizeof(R) == 8) std::memcpy(&m->md, &dev, sizeof(dev)); else std::memcpy(&m->mf, &dev, sizeof(dev));
-  // block size per kernel: the one that keeps the most lane groups resident on an SM.  The selection runs twice: with
+  // block size per kernel: the largest CTA (its warps share the fetched instruction lines; the kernels are fetch-bound,
+  // measured 1.2x forward C2 and 1.4x reverse sweep C3 from 64/128 -> 128/256 threads at equal residency) unless a
+  // smaller one keeps >= 1.3x as many lane groups resident on an SM.  The selection runs twice: with
   // the constant arena appended to each CTA's dynamic shared memory (ModelDev::arena_smem) and without; the arena goes
   // to shared memory only if no kernel loses resident groups to it (DMX_ARENA_SMEM=0 keeps it in global memory).
   const char* eb = std::getenv("DMX_BWD_BLOCK");
@@ -348,9 +450,10 @@ int create_typed(dmx_model* m) {
         CUDA_OK(L.occupancy(b2, std::min(pad(g2 * group_bytes(m, 0)), lim), std::min(sb, lim), std::min(pad(g2 * group_bytes(m, 2)), lim), &t0, &ob, &t2));
         (void)t0; (void)t2; ob = sb <= lim ? 1 : 0; }
       else CUDA_OK(L.occupancy(blk, std::min(sf, lim), std::min(sb, lim), std::min(sx, lim), &of, &ob, &ox));
-      if (ef ? (std::atoi(ef) == blk && blk <= 128 && sf <= lim && of > 0) : (blk <= 128 && sf <= lim && of * g > cf.occ * groups_per_block(m, std::max(cf.block, 1)))) { cf.block = blk; cf.occ = of; cf.smem = sf; }
-      if (eb ? (std::atoi(eb) == blk && sb <= lim && ob > 0) : (blk <= 128 && sb <= lim && ob * g > cb.occ * groups_per_block(m, std::max(cb.block, 1)))) { cb.block = blk; cb.occ = ob; cb.smem = sb; }
-      if (blk <= 128 && sx <= lim && ox * g > cx.occ * groups_per_block(m, std::max(cx.block, 1))) { cx.block = blk; cx.occ = ox; cx.smem = sx; }
+      auto better = [&](int occ_new, const Cfg& cur) { return cur.occ == 0 ? occ_new > 0 : 10 * occ_new * g >= 13 * cur.occ * groups_per_block(m, cur.block); };
+      if (ef ? (std::atoi(ef) == blk && blk <= 128 && sf <= lim && of > 0) : (blk <= 128 && sf <= lim && better(of, cf))) { cf.block = blk; cf.occ = of; cf.smem = sf; }
+      if (eb ? (std::atoi(eb) == blk && sb <= lim && ob > 0) : (sb <= lim && better(ob, cb))) { cb.block = blk; cb.occ = ob; cb.smem = sb; }
+      if (blk <= 128 && sx <= lim && better(ox, cx)) { cx.block = blk; cx.occ = ox; cx.smem = sx; }
     }
     return 0;
   };
@@ -389,56 +492,49 @@ int pick_lanes(const HostModel& h) {
 template <class R>
 int rollout_typed(const dmx_model* m, int nenv, const void* x0, const void* ctrl, int nknot, double knot_dt, const void* params, double horizon,
                   const dmx_solver_opts* opts, const double* h_replay, int n_replay, void* xT, const dmx_stats* st, void* tape, size_t tape_bytes,
-                  cudaStream_t s) {
+                  const void* plan, cudaStream_t s) {
   RolloutArgs<R> a; std::memset(&a, 0, sizeof(a));
-  const int rec = m->h.nq + m->h.nv + 2 + (m->tape_stages ? 6 * m->h.nv : 0);
-  a.nenv = nenv; a.nknot = nknot; a.n_replay = h_replay ? n_replay : 0; a.want_tape = tape != nullptr; a.tape_stages = m->tape_stages;
-  if (tape) {
-    size_t hdr = tape_header_bytes(nenv);
-    if (tape_bytes < hdr + (size_t)nenv * rec * sizeof(R)) return fail("tape too small");
-    a.tape_cap = (int)std::min<size_t>((tape_bytes - hdr) / ((size_t)nenv * rec * sizeof(R)), (size_t)1 << 30);
-    a.tape_hdr = (int*)tape; a.tape = (R*)((unsigned char*)tape + hdr);
-  }
+  a.nenv = nenv; a.nknot = nknot; a.n_replay = h_replay ? n_replay : 0; a.want_tape = tape != nullptr;
+  if (bind_tape<R>(m, nenv, tape, tape_bytes, plan, a.tp, a.pl)) return -1;
   a.x0 = (const R*)x0; a.ctrl = (const R*)ctrl; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u; a.h_replay = h_replay;
   a.knot_dt = knot_dt; a.horizon = horizon; a.so = opts_of(opts); a.xT = (R*)xT;
   if (st) { a.n_accept = st->n_accept; a.n_reject = st->n_reject; a.n_feval = st->n_feval; a.n_unconv = st->n_newton_unconverged; a.status = st->status;
-            a.h_min = st->h_min; a.h_max = st->h_max; a.t_end = st->t_end; }
-  a.queue = m->queue; a.wl = m->wl; a.rl = m->rl;
-  { const char* e = std::getenv("DMX_LOCKSTEP"); a.lockstep = e ? std::atoi(e) : 0; }                 // forward: 2 % fetch stalls, the barriers only cost
-  CUDA_OK(cudaMemsetAsync(m->queue, 0, sizeof(int), s));
+            a.h_min = st->h_min; a.h_max = st->h_max; a.t_end = st->t_end; a.work = st->work; }
+  a.queue = next_queue(m); a.wl = m->wlf; a.rl = m->rlf; a.rk_scratch = (double*)m->rk_scratch_fwd;
+  { const char* e = std::getenv("DMX_LOCKSTEP"); a.lockstep = e ? std::atoi(e) : (m->G >= 16 && m->cf.block >= 64 ? 0x1f : 0); }   // phases in lockstep: +8 % on C3, nothing on C2 (8 lanes)
+  CUDA_OK(cudaMemsetAsync(a.queue, 0, sizeof(int), s));
   LaunchCfg c; c.block = m->cf.block; c.smem = m->cf.smem;
   int gpb = groups_per_block(m, c.block);
   c.grid = std::max(1, std::min(m->cf.occ * m->sm_count, (nenv + gpb - 1) / gpb));
   ModelDev<R> md = dev_of<R>(m); md.arena_smem = m->cf.arena;
-  CUDA_OK(launchers_for<R>(m->G).rollout(md, a, c, s));
+  CUDA_OK(launchers_for<R>(m->G, m->shape).rollout(md, a, c, s));
   return 0;
 }
 
 template <class R>
 int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const void* params, const dmx_solver_opts* opts, const void* xT,
-                   const void* dLdxT, int cfd_on, void* dLdx0, void* dLdctrl, void* dLdparams, const int* status, const void* tape,
-                   size_t tape_bytes, cudaStream_t s) {
+                   const void* dLdxT, int cfd_on, void* dLdx0, void* dLdctrl, void* dLdparams, const dmx_stats* st, const void* tape,
+                   size_t tape_bytes, const void* plan, cudaStream_t s) {
   BackwardArgs<R> a; std::memset(&a, 0, sizeof(a));
-  const int rec = m->h.nq + m->h.nv + 2 + (m->tape_stages ? 6 * m->h.nv : 0);
-  size_t hdr = tape_header_bytes(nenv);
-  if (!tape || tape_bytes < hdr + (size_t)nenv * rec * sizeof(R)) return fail("tape missing or too small");
+  if (!tape) return fail("tape missing");
+  if (bind_tape<R>(m, nenv, const_cast<void*>(tape), tape_bytes, plan, a.tp, a.pl)) return -1;
   a.nenv = nenv; a.nknot = nknot; a.want_p = dLdparams != nullptr; a.cfd = cfd_on; a.tape_stages = m->tape_stages;
   { const char* e = std::getenv("DMX_DBG"); a.dbg = e ? std::atoi(e) : 0; }   // timing experiments only (results invalid when set, except bit 8: VJP rebuilds H instead of reusing the Newton factor)
-  a.tape_cap = (int)std::min<size_t>((tape_bytes - hdr) / ((size_t)nenv * rec * sizeof(R)), (size_t)1 << 30);
-  a.tape_hdr = (const int*)tape; a.tape = (const R*)((const unsigned char*)tape + hdr);
   a.ctrl = (const R*)ctrl; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u; a.xT = (const R*)xT; a.dLdxT = (const R*)dLdxT;
-  a.status = status; a.so = opts_of(opts); a.dLdx0 = (R*)dLdx0; a.dLdctrl = (R*)dLdctrl; a.dLdparams = (R*)dLdparams;
+  a.status = st ? st->status : nullptr; a.n_unconv = st ? st->n_newton_unconverged_bwd : nullptr; a.work = st ? st->work : nullptr;
+  a.so = opts_of(opts); a.dLdx0 = (R*)dLdx0; a.dLdctrl = (R*)dLdctrl; a.dLdparams = (R*)dLdparams;
   { const char* e = std::getenv("DMX_LOCKSTEP_BWD"); a.lockstep = e ? std::atoi(e) : 0x1ff; }          // backward: fetch-bound, phases in lockstep (measured 1.6-2.2x)
-  a.queue = m->queue + 1; a.wl = m->wl; a.rl = m->rl;
+  a.queue = next_queue(m); a.wl = m->wl; a.rl = m->rl;
   LaunchCfg c; c.block = m->cb.block; c.smem = m->cb.smem;
   int gpb = groups_per_block(m, c.block);
   c.grid = std::max(1, std::min(m->cb.occ * m->sm_count, (nenv + gpb - 1) / gpb));
-  if (ensure_scratch(m, c.grid, c.block, true)) return -1;
   a.rk_scratch = (double*)m->rk_scratch;
-  CUDA_OK(cudaMemsetAsync(m->queue + 1, 0, sizeof(int), s));
+  CUDA_OK(cudaStreamWaitEvent(s, m->bwd_done, 0));          // the previous reverse sweep of this model (any stream) owns rk_scratch until it ends
+  CUDA_OK(cudaMemsetAsync(a.queue, 0, sizeof(int), s));
   if (dLdctrl && nknot > 0 && m->h.nu > 0) CUDA_OK(cudaMemsetAsync(dLdctrl, 0, (size_t)nenv * nknot * m->h.nu * sizeof(R), s));
   ModelDev<R> md = dev_of<R>(m); md.arena_smem = m->cb.arena;
-  CUDA_OK(launchers_for<R>(m->G).backward(md, a, c, s));
+  CUDA_OK(launchers_for<R>(m->G, m->shape).backward(md, a, c, s));
+  CUDA_OK(cudaEventRecord(m->bwd_done, s));
   return 0;
 }
 
@@ -453,7 +549,7 @@ int field_typed(dmx_model* m, int n, const void* x, const void* u, const void* p
   int gpb = groups_per_block(m, c.block);
   c.grid = std::max(1, std::min(m->cx.occ * m->sm_count, (n + gpb - 1) / gpb));
   ModelDev<R> md = dev_of<R>(m); md.arena_smem = m->cx.arena;
-  CUDA_OK(launchers_for<R>(m->G).field(md, a, c, s));
+  CUDA_OK(launchers_for<R>(m->G, m->shape).field(md, a, c, s));
   return 0;
 }
 
@@ -484,6 +580,24 @@ template <class T> int fma_peak_typed(int iters, double* flops, double* ms_out) 
   return 0;
 }
 
+// Plan of a launch from the accepted-step counts of a previous pass: cap(e) = n(e) + n(e) margin_pct / 100 + pad,
+// offset = exclusive prefix sum of cap in environment order, order = environments by descending n (ties: lower index
+// first).  Rank and prefix by direct counting: nenv^2 integer operations, deterministic, no scratch.
+__global__ void plan_kernel(int nenv, const int* __restrict__ n_acc, int margin_pct, int pad, int* order, int* cap, long long* offset, long long* total) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= nenv) return;
+  const int ne = n_acc[e];
+  auto capof = [=](int n) { return (int)(n + (long long)n * margin_pct / 100 + pad); };
+  int rank = 0; long long off = 0;
+  for (int j = 0; j < nenv; ++j) {
+    const int nj = n_acc[j];
+    rank += (nj > ne) || (nj == ne && j < e);
+    if (j < e) off += capof(nj);
+  }
+  order[rank] = e; cap[e] = capof(ne); offset[e] = off;
+  if (e == nenv - 1) *total = off + capof(ne);
+}
+
 }  // namespace
 
 // ---- C-ABI ------------------------------------------------------------------------------------------------
@@ -498,7 +612,9 @@ int dmx_model_create(const dmx_model_desc* desc, int precision, dmx_model** out)
   try { flatten(desc, m->h); } catch (std::exception& e) { fail("model: %s", e.what()); delete m; return -1; }
   m->precision = precision;
   m->G = pick_lanes(m->h);
-  make_layouts(m->h, m->G, precision / 8, m->wl, m->rwl, m->rl);
+  m->shape = pick_shape(precision, m->G, m->h.nv, m->h.nc, m->h.nrmax);
+  { const char* e = std::getenv("DMX_FWD_RK_GLOBAL"); m->fwd_rk_global = e ? std::atoi(e) : 0; }
+  make_layouts(m->h, m->G, precision / 8, m->shape ? shape_ld(m->shape, m->h.nv) : 0, m->wl, m->wlf, m->rl, m->rlf);
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
     fail("no CUDA device: the dmx library has no CPU fallback"); delete m; return -1;
@@ -506,8 +622,9 @@ int dmx_model_create(const dmx_model_desc* desc, int precision, dmx_model** out)
   m->max_smem = 0; cudaDeviceGetAttribute(&m->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   size_t zbytes = sizeof(double) * (size_t)std::max(std::max(m->h.nu, m->h.nv), 1);
   if (cudaMalloc(&m->zero_u, zbytes) != cudaSuccess || cudaMemset(m->zero_u, 0, zbytes) != cudaSuccess ||
-      cudaMalloc(&m->queue, 4 * sizeof(int)) != cudaSuccess) { fail("cudaMalloc failed"); dmx_model_destroy(m); return -1; }
+      cudaMalloc(&m->queue, N_QUEUE * sizeof(int)) != cudaSuccess) { fail("cudaMalloc failed"); dmx_model_destroy(m); return -1; }
   int rc = precision == 64 ? create_typed<double>(m) : create_typed<float>(m);
+  if (!rc) rc = alloc_scratch(m);
   if (rc) { dmx_model_destroy(m); return -1; }
   *out = m;
   return 0;
@@ -519,6 +636,8 @@ void dmx_model_destroy(dmx_model* m) {
   if (m->queue) cudaFree(m->queue);
   if (m->zero_u) cudaFree(m->zero_u);
   if (m->rk_scratch) cudaFree(m->rk_scratch);
+  if (m->rk_scratch_fwd) cudaFree(m->rk_scratch_fwd);
+  if (m->bwd_done) cudaEventDestroy(m->bwd_done);
   delete m;
 }
 
@@ -538,7 +657,26 @@ int dmx_model_default_params(const dmx_model* m, double* p_host) {
 
 size_t dmx_tape_bytes(const dmx_model* m, int nenv, int tape_steps) {
   if (!m || nenv <= 0 || tape_steps <= 0) return 0;
-  return tape_header_bytes(nenv) + (size_t)nenv * (size_t)tape_steps * (size_t)(m->h.nq + m->h.nv + 2 + (m->tape_stages ? 6 * m->h.nv : 0)) * rsize(m);
+  return tape_header_bytes(nenv) + (size_t)nenv * (size_t)tape_steps * record_bytes(m);
+}
+size_t dmx_tape_bytes_records(const dmx_model* m, int nenv, long long total_records) {
+  if (!m || nenv <= 0 || total_records <= 0) return 0;
+  return tape_header_bytes(nenv) + (size_t)total_records * record_bytes(m);
+}
+size_t dmx_plan_bytes(int nenv) {
+  if (nenv <= 0) return 0;
+  return 256 + 2 * align_up((size_t)nenv * sizeof(int), 256) + align_up((size_t)nenv * sizeof(long long), 256);
+}
+int dmx_tape_plan(const dmx_model* m, int nenv, const int* n_accept, int margin_pct, int pad, void* plan, size_t plan_bytes, void* cuda_stream) {
+  if (!m || nenv <= 0 || !n_accept || !plan) return fail("null argument");
+  if (margin_pct < 0 || pad < 0) return fail("margin_pct and pad must be non-negative");
+  if (plan_bytes < dmx_plan_bytes(nenv)) return fail("plan buffer too small");
+  unsigned char* b = (unsigned char*)plan;
+  size_t a4 = align_up((size_t)nenv * sizeof(int), 256);
+  plan_kernel<<<(nenv + 127) / 128, 128, 0, (cudaStream_t)cuda_stream>>>(nenv, n_accept, margin_pct, pad, (int*)(b + 256), (int*)(b + 256 + a4),
+                                                                          (long long*)(b + 256 + 2 * a4), (long long*)b);
+  CUDA_OK(cudaGetLastError());
+  return 0;
 }
 
 static int check_common(const dmx_model* m, int nenv, const void* x0, const dmx_solver_opts* o, double horizon) {
@@ -552,32 +690,34 @@ static int check_common(const dmx_model* m, int nenv, const void* x0, const dmx_
 
 int dmx_rollout(const dmx_model* m, int nenv, const void* x0, const void* ctrl, int nknot, double knot_dt, const void* params, double horizon,
                 const dmx_solver_opts* opts, const double* h_replay, int n_replay, void* xT, const dmx_stats* stats, void* tape, size_t tape_bytes,
-                void* cuda_stream) {
+                const void* plan, void* cuda_stream) {
   if (check_common(m, nenv, x0, opts, horizon)) return -1;
   if (!xT) return fail("null xT");
   if (ctrl && m->h.nu > 0 && (nknot <= 0 || !(knot_dt > 0))) return fail("ctrl given but nknot / knot_dt invalid");
   cudaStream_t s = (cudaStream_t)cuda_stream;
-  return m->precision == 64 ? rollout_typed<double>(m, nenv, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay, n_replay, xT, stats, tape, tape_bytes, s)
-                            : rollout_typed<float>(m, nenv, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay, n_replay, xT, stats, tape, tape_bytes, s);
+  return m->precision == 64 ? rollout_typed<double>(m, nenv, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay, n_replay, xT, stats, tape, tape_bytes, plan, s)
+                            : rollout_typed<float>(m, nenv, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay, n_replay, xT, stats, tape, tape_bytes, plan, s);
 }
 
 int dmx_rollout_backward(const dmx_model* m, int nenv, const void* ctrl, int nknot, const void* params, const dmx_solver_opts* opts, const void* xT,
-                         const void* dLdxT, int cfd_on, void* dLdx0, void* dLdctrl, void* dLdparams, const int* status, const void* tape,
-                         size_t tape_bytes, void* cuda_stream) {
+                         const void* dLdxT, int cfd_on, void* dLdx0, void* dLdctrl, void* dLdparams, const dmx_stats* stats, const void* tape,
+                         size_t tape_bytes, const void* plan, void* cuda_stream) {
   if (!m || nenv <= 0 || !opts || !xT || !dLdxT || !dLdx0) return fail("null argument");
   cudaStream_t s = (cudaStream_t)cuda_stream;
-  dmx_model* mm = const_cast<dmx_model*>(m);   // scratch is grown lazily
-  return m->precision == 64 ? backward_typed<double>(mm, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, status, tape, tape_bytes, s)
-                            : backward_typed<float>(mm, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, status, tape, tape_bytes, s);
+  dmx_model* mm = const_cast<dmx_model*>(m);
+  return m->precision == 64 ? backward_typed<double>(mm, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, stats, tape, tape_bytes, plan, s)
+                            : backward_typed<float>(mm, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, stats, tape, tape_bytes, plan, s);
 }
 
 int dmx_rollout_grad(const dmx_model* m, int nenv, const void* x0, const void* ctrl, int nknot, double knot_dt, const void* params, double horizon,
                      const dmx_solver_opts* opts, const double* h_replay, int n_replay, const void* dLdxT, int cfd_on, void* xT, void* dLdx0,
-                     void* dLdctrl, void* dLdparams, const dmx_stats* stats, void* tape, size_t tape_bytes, void* cuda_stream) {
+                     void* dLdctrl, void* dLdparams, const dmx_stats* stats, void* tape, size_t tape_bytes, const void* plan, void* cuda_stream) {
   if (!tape) return fail("dmx_rollout_grad needs a tape");
-  int rc = dmx_rollout(m, nenv, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay, n_replay, xT, stats, tape, tape_bytes, cuda_stream);
+  int rc = dmx_rollout(m, nenv, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay, n_replay, xT, stats, tape, tape_bytes, plan, cuda_stream);
   if (rc) return rc;
-  return dmx_rollout_backward(m, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, nullptr, tape, tape_bytes, cuda_stream);
+  dmx_stats bs; std::memset(&bs, 0, sizeof(bs));            // failed environments are marked in the tape header; only the counter is passed on
+  if (stats) { bs.n_newton_unconverged_bwd = stats->n_newton_unconverged_bwd; bs.work = stats->work; }
+  return dmx_rollout_backward(m, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, &bs, tape, tape_bytes, plan, cuda_stream);
 }
 
 int dmx_vector_field(const dmx_model* m, int n, const void* x, const void* u, const void* params, int cfd, void* acc, int* nrow, void* cuda_stream) {
@@ -601,7 +741,7 @@ int dmx_debug_counters(const dmx_model* m, unsigned long long* host32) {
   if (!m || !host32) return fail("null argument");
   unsigned long long* d = nullptr;
   CUDA_OK(cudaMalloc(&d, 32 * sizeof(unsigned long long)));
-  cudaError_t e = m->precision == 64 ? launchers_for<double>(m->G).prof_dump(d, 0) : launchers_for<float>(m->G).prof_dump(d, 0);
+  cudaError_t e = m->precision == 64 ? launchers_for<double>(m->G, m->shape).prof_dump(d, 0) : launchers_for<float>(m->G, m->shape).prof_dump(d, 0);
   if (e == cudaSuccess) e = cudaMemcpy(host32, d, 32 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
   cudaFree(d);
   CUDA_OK(e);

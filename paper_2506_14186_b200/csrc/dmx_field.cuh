@@ -157,9 +157,9 @@ DMX_DI void body_wrench(const ModelDev<R>& m, const IN& in, const WS& ws, int b,
 // world inertias of that subtree.  c_j = sum_b lin_jb . F_b + ang_j . N_b (virtual work).
 template <class WS, class R, int G, class IN>
 DMX_DN void dynamics(const ModelDev<R>& m, const IN& in, const WS& ws, const Grp<G>& gr) {
-  const int ld = ws.L->ld;
+  const int ld = ws.ld();
   typedef typename WS::S S;
-  const int nv = m.nv, nb = m.nbody;
+  const int nv = ws.nv(m), nb = m.nbody;
 #pragma unroll 1
   for (int b = 1 + gr.lane; b < nb; b += G) {
     V3<S> Fb, Nb; M3<S> Iw;
@@ -322,12 +322,22 @@ template <class S, int ST, int G> DMX_DN void chol_solve(const Arr<S, ST>& L, in
 }
 
 // ---- S5: impedance d(r) from solimp (spline: SURVEY G5) and the CFD continuation --
+// general exponent: one out-of-line copy (pow is ~300 instructions; the BASELINE configs use power = 2)
+template <class S> __device__ __noinline__ S imp_spline_pow(S x, S mid, S power) {
+  S one(1.0);
+  if (val(x) <= val(mid)) return m_pow(x, power) / m_pow(mid, power - one);
+  return one - m_pow(one - x, power) / m_pow(one - mid, power - one);
+}
 template <class S> DMX_DI S imp_spline(const S& x, const S& mid, const S& power) {
   if (val(x) <= 0) return S(0.0) * x;
   if (val(x) >= 1) return S(1.0) + S(0.0) * x;
   S one(1.0);
-  if (val(x) <= val(mid)) return m_pow(x, power) / m_pow(mid, power - one);
-  return one - m_pow(one - x, power) / m_pow(one - mid, power - one);
+  if (val(power) == 2.0 && !has_tangent(power)) {   // x^2 / mid and 1 - (1-x)^2 / (1-mid): same values as pow up to its rounding
+    if (val(x) <= val(mid)) return x * x / mid;
+    S y = one - x;
+    return one - y * y / (one - mid);
+  }
+  return imp_spline_pow<S>(x, mid, power);
 }
 template <class S> DMX_DI S clamp_imp(S d) {
   if (val(d) < 0) d = S(0.0);
@@ -419,17 +429,18 @@ DMX_DI V3<typename WS::S> rel_twist(const ModelDev<R>& m, const WS& ws, int j, i
   S z(0.0);
   V3<S> d = mk3<S>(z, z, z);
   int rot = m.dof_rot[j];
-  if (m.tw_idx[b2 * m.nv + j] >= 0) d = twist_lin(ws, j, rot, pos);
-  if (m.tw_idx[b1 * m.nv + j] >= 0) d = d - twist_lin(ws, j, rot, pos);
+  const int nv = ws.nv(m);
+  if (m.tw_idx[b2 * nv + j] >= 0) d = twist_lin(ws, j, rot, pos);
+  if (m.tw_idx[b1 * nv + j] >= 0) d = d - twist_lin(ws, j, rot, pos);
   return d;
 }
 
 // ---- S4+S5: rows of every candidate with r<0 (cfd: r<w_c), compacted in candidate order ----------
 template <class WS, class R, int G, class IN>
 DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, const Grp<G>& gr) {
-  const int ld = ws.L->ld;
+  const int ld = ws.ld();
   typedef typename WS::S S;
-  const int nv = m.nv, nc = m.nc;
+  const int nv = ws.nv(m), nc = ws.nc(m);
 #pragma unroll 1
   for (int c = gr.lane; c < nc; c += G) {
     GeoT<S> g = collide<WS, R>(m, ws, c);
@@ -483,21 +494,250 @@ DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
   return nr;
 }
 
+
+// ---- D1: line search of S6.  phi'(a) = dl^T M (x + a dl - a0) + sum_i D_i p_i min(0, s_i + a p_i) is piecewise linear and
+// increasing; bracketed 1-D Newton from a = 1.  Every lane runs the scalar search redundantly on the group's shared
+// arrays (Md = M dl, xa = x - a0, s, pr = J dl, D) in row order: the summation order of a serial code, uniform result.
+template <class WS>
+DMX_DN typename WS::S line_search(int nv, int nr, int n_ls, const WS& ws) {
+  typedef typename WS::S S;
+  S dMd(0.0), dMxa(0.0);
+#pragma unroll 1
+  for (int a = 0; a < nv; ++a) { dMd = dMd + ws.dl()[a] * ws.Md()[a]; dMxa = dMxa + ws.Md()[a] * ws.xa()[a]; }
+  S lo(0.0), hi(0.0), a(0.0), d2, d1a; bool hi_inf = true, frozen = false;
+  {
+    d1a = dMxa; d2 = dMd;
+#pragma unroll 1
+    for (int i = 0; i < nr; ++i) { S si = ws.s()[i]; if (val(si) < 0) { d1a = d1a + ws.D()[i] * ws.pr()[i] * si; d2 = d2 + ws.D()[i] * ws.pr()[i] * ws.pr()[i]; } }
+  }
+#pragma unroll 1
+  for (int ls = 0; ls < n_ls && !frozen; ++ls) {
+    S an = (ls == 0) ? S(1.0) : a - d1a / d2;
+    if (ls > 0 && val(an) == val(a)) break;      // no representable progress: the root of phi' is reached
+    bool inside = (val(an) > val(lo)) && (hi_inf || val(an) < val(hi));
+    if (!inside) an = hi_inf ? S(2.0) * (val(a) > 1 ? a : S(1.0)) : S(0.5) * (lo + hi);
+    a = an;
+    d1a = dMxa + a * dMd; d2 = dMd;
+#pragma unroll 1
+    for (int i = 0; i < nr; ++i) {
+      S si = ws.s()[i] + a * ws.pr()[i];
+      if (val(si) < 0) { d1a = d1a + ws.D()[i] * ws.pr()[i] * si; d2 = d2 + ws.D()[i] * ws.pr()[i] * ws.pr()[i]; }
+    }
+    if (val(d1a) < 0) lo = a; else if (val(d1a) > 0) { hi = a; hi_inf = false; } else frozen = true;
+  }
+  return a;
+}
+
+// ---- static sizes (Shape): Cholesky and substitutions with the rows in registers ----------------------------------
+// Lane a of the group owns row a of the symmetric matrix (NV <= G).  Right-looking factorisation: once column j is
+// known, every lane updates the rest of its own row, h[k] -= L[a][j] L[k][j], with L[k][j] fetched from lane k by
+// shuffle; there is no shared-memory round trip and no group barrier inside the factorisation.  Every entry sees the
+// operations of the left-looking shared-memory version in the same order (for entry (a,k): subtract L[a][j] L[k][j],
+// j = 0, 1, ...), so the factor is bitwise the same.  The factor is stored with the reciprocal of its diagonal.  On
+// exit the lower triangle of `dst` holds L row-major (for the backward substitution and for vjp_prepare's reuse) and
+// hd the lane's own diagonal entry.
+template <int NV, class S, int ST, int G>
+DMX_DI bool chol_static(const Arr<S, ST>& src, const Arr<S, ST>& dst, int ld, const Grp<G>& gr, S (&h)[NV], S& hd) {
+  const int a = gr.lane, ar = a < NV ? a : NV - 1;
+#pragma unroll
+  for (int b = 0; b < NV; ++b) h[b] = src[ar * ld + b];
+  hd = S(0.0);
+#pragma unroll
+  for (int j = 0; j < NV; ++j) {
+    const S piv = gr.from_lane(h[j], j);
+    if (!(val(piv) > 0)) return false;       // uniform over the group
+    const S il = m_rsqrt(piv);
+    const S lj = (a == j) ? il : h[j] * il;
+    h[j] = lj;
+    if (a == j) hd = il;
+#pragma unroll
+    for (int k = j + 1; k < NV; ++k) h[k] = h[k] - lj * gr.from_lane(lj, k);
+  }
+  if (a < NV) {
+#pragma unroll
+    for (int b = 0; b < NV; ++b) if (b <= a) dst[a * ld + b] = h[b];
+  }
+  gr.sync();
+  return true;
+}
+// bk (lane a holds entry a of the right-hand side) <- (L L^T)^-1 b with lane a's row of L in h, its diagonal in hd, and
+// L row-major in `Lm` (column a of L for the backward substitution).  Same operations per entry as chol_solve.
+template <int NV, class S, int ST, int G>
+DMX_DI S solve_static(const Arr<S, ST>& Lm, int ld, const Grp<G>& gr, const S (&h)[NV], const S& hd, S bk) {
+  const int a = gr.lane, ac = a < NV ? a : 0;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const S bi = gr.from_lane(bk * hd, i);
+    if (a > i) bk = bk - h[i] * bi; else if (a == i) bk = bi;
+  }
+#pragma unroll
+  for (int i = NV - 1; i >= 0; --i) {
+    const S bi = gr.from_lane(bk * hd, i);
+    if (a < i) bk = bk - Lm[i * ld + ac] * bi; else if (a == i) bk = bi;
+  }
+  return bk;
+}
+// row a of a factor left in shared memory by chol_static (reuse by the VJP)
+template <int NV, class S, int ST, int G>
+DMX_DI void load_factor_row(const Arr<S, ST>& Lm, int ld, const Grp<G>& gr, S (&h)[NV], S& hd) {
+  const int a = gr.lane, ar = a < NV ? a : NV - 1;
+#pragma unroll
+  for (int b = 0; b < NV; ++b) h[b] = Lm[ar * ld + b];
+  hd = Lm[ar * ld + ar];
+}
+// One copy per kernel of the unrolled factorisation / substitution code (the instruction cache is the scarce resource:
+// the kernels are fetch-bound when every call site carries its own copy).  ok is uniform over the group.
+template <class S> struct SolveOut { S x; bool ok; };
+template <int NV, class S, int ST, int G>
+__device__ __noinline__ SolveOut<S> factor_solve_static(unsigned src, unsigned dst, int ld, S rhs) {   // offsets in the CTA's dynamic shared memory
+  const Grp<G> gr = make_group<G>();
+  S h[NV], hd;
+  SolveOut<S> o; o.x = rhs;
+  o.ok = chol_static<NV>(Arr<S, ST>(smem_ptr<S>(src)), Arr<S, ST>(smem_ptr<S>(dst)), ld, gr, h, hd);
+  if (o.ok) o.x = solve_static<NV>(Arr<S, ST>(smem_ptr<S>(dst)), ld, gr, h, hd, rhs);
+  return o;
+}
+template <int NV, class S, int ST, int G>
+__device__ __noinline__ S resolve_static(unsigned Lm, int ld, S rhs) {
+  const Grp<G> gr = make_group<G>();
+  S h[NV], hd;
+  load_factor_row<NV>(Arr<S, ST>(smem_ptr<S>(Lm)), ld, gr, h, hd);
+  return solve_static<NV>(Arr<S, ST>(smem_ptr<S>(Lm)), ld, gr, h, hd, rhs);
+}
+// H = M + J^T diag(w) J on the lower triangle: lane per entry; the entry -> (a, b) map of a lane is computed once
+template <int NV, int G> struct TriMap {
+  static const int NT = NV * (NV + 1) / 2, NE = (NT + G - 1) / G;
+  int off[NE], ca[NE], cb[NE];
+  DMX_DI void init(int lane, int ld) {
+#pragma unroll
+    for (int q = 0; q < NE; ++q) {
+      int e = lane + q * G, a = 0, b = 0;
+      if (e < NT) tri_index(e, a, b);
+      off[q] = e < NT ? a * ld + b : -1; ca[q] = a; cb[q] = b;
+    }
+  }
+};
+template <int NV, int G, class WS>
+DMX_DI void build_h_static(const TriMap<NV, G>& tm, int nr, int ld, const WS& ws) {
+  typedef typename WS::S S;
+#pragma unroll
+  for (int q = 0; q < TriMap<NV, G>::NE; ++q) {
+    if (tm.off[q] < 0) continue;
+    S t = ws.M()[tm.off[q]];
+    const int ca = tm.ca[q], cb = tm.cb[q];
+#pragma unroll 4
+    for (int i = 0; i < nr; ++i) t = t + ws.pr()[i] * ws.J()[i * ld + ca] * ws.J()[i * ld + cb];
+    ws.Hc()[tm.off[q]] = t;
+  }
+}
+
+// ---- S6 with static sizes: the Newton iteration of `newton` below with the vectors x, a0, the step and the rows of the
+// factor in registers (lane a owns dof a), the products J x, J dl unrolled over the dofs.  Same operations per entry
+// and the same summation orders as the generic version: results are bitwise equal.
+template <class WS, int G>
+DMX_DN bool newton_static(int nr, int n_it, int n_ls, const WS& ws, const Grp<G>& gr, int& iters) {
+  typedef typename WS::S S;
+  const int NV = WS::SH::NV, ld = WS::SH::LD;
+  const int a = gr.lane, ac = a < NV ? a : NV - 1;
+  const bool own = a < NV;
+  const S a0a = ws.a0()[ac];
+  S xa_ = a0a;                          // x[a]
+  if (own) ws.x()[a] = xa_;
+  gr.sync();
+  iters = 0;
+  if (nr == 0) return true;
+  TriMap<WS::SH::NV, G> tm; tm.init(a, ld);
+  bool conv = false;
+#pragma unroll 1
+  for (int it = 0; it < n_it; ++it) {
+    ++iters;
+    {
+      S xr[WS::SH::NV];
+#pragma unroll
+      for (int j = 0; j < NV; ++j) xr[j] = ws.x()[j];
+#pragma unroll 1
+      for (int i = a; i < nr; i += G) {
+        S t(0.0);
+#pragma unroll
+        for (int j = 0; j < NV; ++j) t = t + ws.J()[i * ld + j] * xr[j];
+        const S si = t - ws.aref()[i];
+        ws.s()[i] = si;
+        ws.active()[i] = val(si) < 0 ? 1 : 0;
+        ws.pr()[i] = val(si) < 0 ? ws.D()[i] : S(0.0);
+      }
+      if (own) ws.xa()[a] = xa_ - a0a;
+      gr.sync();
+    }
+    S dla;
+    {
+      S t(0.0);
+#pragma unroll
+      for (int b = 0; b < NV; ++b) t = t + ws.M()[ac * ld + b] * ws.xa()[b];
+#pragma unroll 4
+      for (int i = 0; i < nr; ++i) t = t + ws.J()[i * ld + ac] * ws.pr()[i] * ws.s()[i];
+      if (own) ws.g()[a] = t;
+      dla = -t;
+    }
+    build_h_static<WS::SH::NV, G>(tm, nr, ld, ws);
+    gr.sync();
+    {
+      const SolveOut<S> so = factor_solve_static<WS::SH::NV, S, WS::ST, G>(smem_off(ws.Hc().p), smem_off(ws.Hc().p), ld, dla);
+      if (!so.ok) break;
+      dla = so.x;
+    }
+    if (own) ws.dl()[a] = dla;
+    gr.sync();
+    bool same = true;
+    {
+      S dr[WS::SH::NV];
+#pragma unroll
+      for (int j = 0; j < NV; ++j) dr[j] = ws.dl()[j];
+#pragma unroll 1
+      for (int i = a; i < nr; i += G) {
+        S t(0.0);
+#pragma unroll
+        for (int j = 0; j < NV; ++j) t = t + ws.J()[i * ld + j] * dr[j];
+        ws.pr()[i] = t;
+        const S si = ws.s()[i];
+        if ((val(si) < 0) != (val(si + t) < 0)) same = false;
+      }
+      same = gr.all(same);
+      if (!same && own) {
+        S t(0.0);
+#pragma unroll
+        for (int b = 0; b < NV; ++b) t = t + ws.M()[a * ld + b] * dr[b];
+        ws.Md()[a] = t;
+      }
+      gr.sync();
+    }
+    S alpha(1.0);
+    if (!same) alpha = line_search<WS>(NV, nr, n_ls, ws);
+    xa_ = xa_ + alpha * dla;
+    if (own) ws.x()[a] = xa_;
+    gr.sync();
+    if (same) { conv = true; break; }
+  }
+  return conv;
+}
+
 // ---- S6: Newton with a fixed iteration budget on the reduced primal problem of Eq. 2 -------------
 //   Phi(x) = 1/2 (x-a0)^T M (x-a0) + 1/2 sum_i D_i min(0, J_i x - aref_i)^2
 // (iterations / ls_iterations PAPER.md:515, 539).
 // Returns true when the last step was a full step inside an unchanged active set.
 template <class WS, int G>
-DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G>& gr) {
-  const int ld = ws.L->ld;
+DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G>& gr, int& iters) {
+  if constexpr (WS::SH::NV > 0 && G > 1) return newton_static<WS, G>(nr, n_it, n_ls, ws, gr, iters);
+  const int ld = ws.ld();
   typedef typename WS::S S;
 #pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) ws.x()[j] = ws.a0()[j];
   gr.sync();
+  iters = 0;
   if (nr == 0) return true;
   bool conv = false;
 #pragma unroll 1
   for (int it = 0; it < n_it; ++it) {
+    ++iters;
 #pragma unroll 1
     for (int i = gr.lane; i < nr; i += G) {
       S t(0.0);
@@ -543,8 +783,6 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
     gr.sync();
     S alpha(1.0);
     if (!same) {
-      // D1: phi'(a) = dl^T M (x + a dl - a0) + sum_i D_i p_i min(0, s_i + a p_i); every lane runs the
-      // scalar line search redundantly in row order (same summation order as a serial code)
 #pragma unroll 1
       for (int a = gr.lane; a < nv; a += G) {
         S t(0.0);
@@ -553,31 +791,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
         ws.Md()[a] = t;
       }
       gr.sync();
-      S dMd(0.0), dMxa(0.0);
-#pragma unroll 1
-      for (int a = 0; a < nv; ++a) { dMd = dMd + ws.dl()[a] * ws.Md()[a]; dMxa = dMxa + ws.Md()[a] * ws.xa()[a]; }
-      S lo(0.0), hi(0.0), a(0.0), d2, d1a; bool hi_inf = true, frozen = false;
-      {
-        d1a = dMxa; d2 = dMd;
-#pragma unroll 1
-        for (int i = 0; i < nr; ++i) { S si = ws.s()[i]; if (val(si) < 0) { d1a = d1a + ws.D()[i] * ws.pr()[i] * si; d2 = d2 + ws.D()[i] * ws.pr()[i] * ws.pr()[i]; } }
-      }
-#pragma unroll 1
-      for (int ls = 0; ls < n_ls && !frozen; ++ls) {
-        S an = (ls == 0) ? S(1.0) : a - d1a / d2;
-        if (ls > 0 && val(an) == val(a)) break;      // no representable progress: the root of phi' is reached
-        bool inside = (val(an) > val(lo)) && (hi_inf || val(an) < val(hi));
-        if (!inside) an = hi_inf ? S(2.0) * (val(a) > 1 ? a : S(1.0)) : S(0.5) * (lo + hi);
-        a = an;
-        d1a = dMxa + a * dMd; d2 = dMd;
-#pragma unroll 1
-        for (int i = 0; i < nr; ++i) {
-          S si = ws.s()[i] + a * ws.pr()[i];
-          if (val(si) < 0) { d1a = d1a + ws.D()[i] * ws.pr()[i] * si; d2 = d2 + ws.D()[i] * ws.pr()[i] * ws.pr()[i]; }
-        }
-        if (val(d1a) < 0) lo = a; else if (val(d1a) > 0) { hi = a; hi_inf = false; } else frozen = true;
-      }
-      alpha = a;
+      alpha = line_search<WS>(nv, nr, n_ls, ws);
     }
 #pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) ws.x()[j] = ws.x()[j] + alpha * ws.dl()[j];
@@ -592,10 +806,10 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
 // xk != nullptr: the solution x* is already known (stage rate read from the tape; element j at xk[j*xst]); the
 // unconstrained solve and the Newton iterations are skipped and only M, the rows and x* are set up for the VJP.
 template <class WS, class R, int G, class IN>
-DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, bool& conv, const Grp<G>& gr,
+DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, bool& conv, int& iters, const Grp<G>& gr,
                         const double* xk = nullptr, int xst = 1) {
-  const int ld = ws.L->ld;
-  const int nv = m.nv;
+  const int ld = ws.ld();
+  const int nv = ws.nv(m);
   phase_sync(0);
   DMX_T0;
   kinematics<WS, R, G, IN, false>(m, in, ws, gr);
@@ -603,14 +817,22 @@ DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool c
   phase_sync(1);
   dynamics<WS, R, G, IN>(m, in, ws, gr);
   DMX_TICK(gr, 1);
-  conv = true;
+  conv = true; iters = 0;
   if (!xk) {
     phase_sync(2);
-    for (int e = gr.lane; e < nv * ld; e += G) ws.Hc()[e] = ws.M()[e];
-    for (int j = gr.lane; j < nv; j += G) ws.a0()[j] = ws.tau()[j] - ws.c()[j];
-    gr.sync();
-    if (!cholesky(ws.Hc(), nv, ld, gr)) return -1;
-    chol_solve(ws.Hc(), nv, ld, ws.a0(), gr);
+    if constexpr (WS::SH::NV > 0 && G > 1) {        // factor of M and a0 = M^-1 (tau - c) with the rows in registers
+      const int a = gr.lane < nv ? gr.lane : nv - 1;
+      const SolveOut<typename WS::S> so = factor_solve_static<WS::SH::NV, typename WS::S, WS::ST, G>(smem_off(ws.M().p), smem_off(ws.Hc().p), ld, ws.tau()[a] - ws.c()[a]);
+      if (!so.ok) return -1;
+      if (gr.lane < nv) ws.a0()[gr.lane] = so.x;
+      gr.sync();
+    } else {
+      for (int e = gr.lane; e < nv * ld; e += G) ws.Hc()[e] = ws.M()[e];
+      for (int j = gr.lane; j < nv; j += G) ws.a0()[j] = ws.tau()[j] - ws.c()[j];
+      gr.sync();
+      if (!cholesky(ws.Hc(), nv, ld, gr)) return -1;
+      chol_solve(ws.Hc(), nv, ld, ws.a0(), gr);
+    }
     DMX_TICK(gr, 2);
   }
   phase_sync(3);
@@ -622,7 +844,7 @@ DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool c
     return nr;
   }
   phase_sync(4);
-  conv = newton<WS, G>(nv, nr, m.newton_iters, m.ls_iters, ws, gr);
+  conv = newton<WS, G>(nv, nr, m.newton_iters, m.ls_iters, ws, gr, iters);
   DMX_TICK(gr, 4);
   bool fin = true;
   for (int j = gr.lane; j < nv; j += G) if (!isfinite(val(ws.x()[j]))) fin = false;
@@ -634,7 +856,7 @@ DMX_DN int vector_field(const ModelDev<R>& m, const IN& in, const WS& ws, bool c
 // ws.kap() holds kappa on entry and w on exit.  Returns false if H is not positive definite.
 template <class WS, int G>
 DMX_DN bool vjp_prepare(int nv, int nr, bool hc_valid, const WS& ws, const Grp<G>& gr) {
-  const int ld = ws.L->ld;
+  const int ld = ws.ld();
   typedef typename WS::S S;
   // hc_valid: Hc still holds the Cholesky factor of the last Newton iteration (or of M when there are no rows) and
   // ws.active the set it was built for.  A converged solve ends on an unchanged active set, so that factor IS the
@@ -654,6 +876,22 @@ DMX_DN bool vjp_prepare(int nv, int nr, bool hc_valid, const WS& ws, const Grp<G
   }
   const bool reuse = gr.all(same);
   gr.sync();
+  if constexpr (WS::SH::NV > 0 && G > 1) {
+    const int a = gr.lane < nv ? gr.lane : nv - 1;
+    S w;
+    if (!reuse) {
+      TriMap<WS::SH::NV, G> tm; tm.init(gr.lane, ld);
+      build_h_static<WS::SH::NV, G>(tm, nr, ld, ws);
+      gr.sync();
+      const SolveOut<S> so = factor_solve_static<WS::SH::NV, S, WS::ST, G>(smem_off(ws.Hc().p), smem_off(ws.Hc().p), ld, ws.kap()[a]);
+      if (!so.ok) return false;
+      w = so.x;
+    } else w = resolve_static<WS::SH::NV, S, WS::ST, G>(smem_off(ws.Hc().p), ld, ws.kap()[a]);
+    gr.sync();                                     // every lane has read kappa before w overwrites it
+    if (gr.lane < nv) ws.kap()[gr.lane] = w;
+    gr.sync();
+    return true;
+  }
   if (!reuse) {
 #pragma unroll 1
     for (int e = gr.lane; e < nv * (nv + 1) / 2; e += G) {
@@ -682,9 +920,9 @@ DMX_DN bool vjp_prepare(int nv, int nr, bool hc_valid, const WS& ws, const Grp<G
 // w in ws.kap.  Uses ws.Fb/ws.Nb for velw/omegaw, ws.Isub for the body adjoints, ws.pr for J_i w.
 template <class WS, class R, int G, class IN, class AOUT>
 DMX_D void vjp_velocity(const ModelDev<R>& m, const IN& in, const WS& ws, int nr, const AOUT& vbar, const Grp<G>& gr) {
-  const int ld = ws.L->ld;
+  const int ld = ws.ld();
   typedef typename WS::S S;
-  const int nv = m.nv, nb = m.nbody;
+  const int nv = ws.nv(m), nb = m.nbody;
   // seeds: cotangents of (omega_b, alpha_b, ap_b) from F_b = m (ac_b - g), N_b = I alpha + omega x I omega
 #pragma unroll 1
   for (int b = 1 + gr.lane; b < nb; b += G) {
@@ -784,7 +1022,7 @@ DMX_D void vjp_velocity(const ModelDev<R>& m, const IN& in, const WS& ws, int nr
 template <class WS, class R, int G, class IN, class AOUT>
 DMX_D void vjp_config_bodies(const ModelDev<R>& m, const IN& in, const WS& ws, const AOUT& qbar, const Grp<G>& gr) {
   typedef typename WS::S S;
-  const int nv = m.nv, nb = m.nbody;
+  const int nv = ws.nv(m), nb = m.nbody;
 #pragma unroll 1
   for (int b = 1 + gr.lane; b < nb; b += G) {
     V3<S> Fb, Nb; M3<S> Iw;
@@ -867,7 +1105,7 @@ DMX_D void vjp_config_bodies(const ModelDev<R>& m, const IN& in, const WS& ws, c
 template <bool PP, class WS, class R, int G, class IN, class AOUT>
 DMX_D void vjp_config_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, const AOUT& qbar, const Grp<G>& gr) {
   typedef typename WS::S S;
-  const int nv = m.nv, nc = m.nc;
+  const int nv = ws.nv(m), nc = ws.nc(m);
 #pragma unroll 1
   for (int c = gr.lane; c < nc; c += G) {
     if (ws.incl()[c] == 0 || (m.ct_kind[c] == CK_POINT_POINT) != PP) continue;
@@ -984,7 +1222,7 @@ DMX_D void vjp_config_rows(const ModelDev<R>& m, const IN& in, const WS& ws, boo
 template <class WS, class R, int G, class IN, class AOUT>
 DMX_D void vjp_params(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd, const AOUT& pbar, const Grp<G>& gr) {
   typedef typename WS::S S;
-  const int nc = m.nc;
+  const int nc = ws.nc(m);
 #pragma unroll 1
   for (int b = gr.lane; b < m.nbody; b += G) {
     S g(0.0);

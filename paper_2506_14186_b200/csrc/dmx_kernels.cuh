@@ -8,61 +8,66 @@ namespace dmx {
 
 // ---- S11/S12: (qbar,vbar,ubar,pbar) = kappa^T dF/d(q,v,u,p), F~ when cfd (Eq. 4) ----------
 // Cooperative solve for x*, the active set and w = H^-1 kappa; then the closed-form gradient of S (dmx_field.cuh).
-template <class R, int G>
+template <class R, int G, class SH>
 DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yqr, const Arr<R, StrideOf<G>::value>& Vr, const R* u, const R* p,
-                      const Arr<double, StrideOf<G>::value>& kappa, bool cfd, bool want_p, const Ws<R, StrideOf<G>::value>& ws,
-                      const Rk<StrideOf<G>::value>& rk, const Grp<G>& gr, int dbg = 0, const double* xk = nullptr) {
+                      const Arr<double, StrideOf<G>::value>& kappa, bool cfd, bool want_p, const Ws<R, StrideOf<G>::value, SH>& ws,
+                      const Rk<StrideOf<G>::value>& rk, const Grp<G>& gr, int dbg = 0, const double* xk = nullptr, int* unconv = nullptr,
+                      unsigned long long* work = nullptr) {
   const int ST = StrideOf<G>::value;
   const int nv = m.nv;
   if (dbg & 4) return true;
   DMX_T0;
   InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
   int conv;
-  int nr = field_eval<R, G>(u, p, cfd ? 1 : 0, &conv, xk);
+  int nr = field_eval<R, G, SH>(u, p, cfd ? 1 : 0, &conv, xk);
   if (nr < 0) return false;
+  if (unconv && !xk && nr > 0 && !(conv & 1)) ++*unconv;     // the implicit-function gradient is taken at a non-stationary point
+  if (work) { work[0] += (unsigned)(conv >> 8); work[1] += (unsigned long long)(conv >> 8) * nr; work[2] += (unsigned)nr; }
   DMX_TICK(gr, 8);
   phase_sync(5);
 #pragma unroll 1
   for (int j = gr.lane; j < nv; j += G) ws.kap()[j] = (R)kappa[j];
   gr.sync();
-  if (!vjp_prepare<Ws<R, ST>, G>(nv, nr, xk == nullptr && conv != 0 && !(dbg & 8), ws, gr)) return false;
+  if (!vjp_prepare<Ws<R, ST, SH>, G>(nv, nr, xk == nullptr && (conv & 1) != 0 && !(dbg & 8), ws, gr)) return false;
   DMX_TICK(gr, 9);
   phase_sync(6);
   // u: closed form; v: reverse sweep over the tree; then the frames at acceleration x* for the tangent passes
 #pragma unroll 1
   for (int i = gr.lane; i < m.nu; i += G)
     rk.ubar()[i] = (double)(ws.kap()[m.jnt_vadr[m.act_jnt[i]]] * (m.act_type[i] == ACT_MOTOR ? m.act_gear[i] : m.act_kp[i]));
-  if (!(dbg & 2)) vjp_velocity<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, nr, rk.vbar(), gr);
+  if (!(dbg & 2)) vjp_velocity<Ws<R, ST, SH>, R, G, InPlain<R, ST> >(m, in, ws, nr, rk.vbar(), gr);
   DMX_TICK(gr, 10);
   phase_sync(7);
   in.aa = ws.x();
-  kinematics<Ws<R, ST>, R, G, InPlain<R, ST>, true>(m, in, ws, gr);
+  kinematics<Ws<R, ST, SH>, R, G, InPlain<R, ST>, true>(m, in, ws, gr);
   DMX_TICK(gr, 11);
   phase_sync(8);
   // q: bodies in closed form (cooperative), then the rows' part and the parameters by one tangent lane per direction
-  vjp_config_bodies<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, rk.qbar(), gr);
-  vjp_config_rows<false, Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.qbar(), gr);                 // point-plane rows
-  if (m.npp > 0) vjp_config_rows<true, Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.qbar(), gr);   // sphere-sphere rows
-  if (want_p) vjp_params<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.pbar(), gr);
+  vjp_config_bodies<Ws<R, ST, SH>, R, G, InPlain<R, ST> >(m, in, ws, rk.qbar(), gr);
+  vjp_config_rows<false, Ws<R, ST, SH>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.qbar(), gr);                 // point-plane rows
+  if (m.npp > 0) vjp_config_rows<true, Ws<R, ST, SH>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.qbar(), gr);   // sphere-sphere rows
+  if (want_p) vjp_params<Ws<R, ST, SH>, R, G, InPlain<R, ST> >(m, in, ws, cfd, rk.pbar(), gr);
   gr.sync();
   DMX_TICK(gr, 12);
   return true;
 }
 
 template <class R> struct BackwardArgs {
-  int nenv, nknot, want_p, cfd, tape_cap, dbg, lockstep, tape_stages;
+  int nenv, nknot, want_p, cfd, dbg, lockstep, tape_stages;
   const R *ctrl, *params, *zero_u, *xT, *dLdxT;
   const int* status;
+  int* n_unconv;            // [nenv] or null: contact solves of the reverse sweep that did not converge
+  unsigned long long* work; // [nenv][6] or null (slots 3..5: Newton iterations, row-iterations and rows of the reverse sweep)
   SolverOpts so;
   R *dLdx0, *dLdctrl, *dLdparams;
-  const int* tape_hdr; const R* tape;
+  TapeView<R> tp; PlanView pl;
   int* queue;
   double* rk_scratch;       // integrator / adjoint arrays of every resident group (global memory: touched once per stage)
   WsLayout wl; RkLayout rl;
 };
 
 // ---- S10: reverse sweep over the tape, frozen step sizes ---------------------------
-template <class R, int G>
+template <class R, int G, class SH>
 __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ BackwardArgs<R> a) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
@@ -71,23 +76,29 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
-  Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
-  bind_shared<R, G>(smem, 0, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
+  Rk<ST> rk; Ws<R, ST, SH> ws; Arr<R, ST> Yqr, Vr;
+  bind_shared<R, G, SH>(smem, 0, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
   if (G == 1) rk.b = a.rk_scratch + ((size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32 * (size_t)a.rl.size_bwd + (threadIdx.x & 31);
   else rk.b = a.rk_scratch + ((size_t)blockIdx.x * (blockDim.x / G) + threadIdx.x / G) * (size_t)a.rl.size_bwd;
-  const int nq = m.nq, nv = m.nv, nu = m.nu, np = m.np, nx = nq + nv, tab = a.so.tableau, rec = nx + 2 + (a.tape_stages ? 6 * nv : 0);
+  const int nq = m.nq, nv = m.nv, nu = m.nu, np = m.np, nx = nq + nv, tab = a.so.tableau, rec = a.tp.rec;
   const bool has_ctrl = a.ctrl != nullptr && a.nknot > 0 && nu > 0;
   const int nknot = has_ctrl ? a.nknot : 0;
+  // the tape must be the one a rollout of this model wrote for this batch, record layout and plan
+  const bool tape_ok = a.tp.meta[0] == TAPE_MAGIC && a.tp.meta[1] == a.nenv && a.tp.meta[2] == rec && a.tp.meta[3] == a.tp.o_A &&
+                       a.tp.meta[4] == (a.pl.offset ? 1 : 0);
 #pragma unroll 1
   for (;;) {
     int e = 0;
-    if (gr.lane == 0) e = atomicAdd(a.queue, 1);
+    if (gr.lane == 0) { e = atomicAdd(a.queue, 1); if (e < a.nenv && a.pl.order) e = a.pl.order[e]; }
     e = gr.bcast_int(e);
     if (e >= a.nenv) break;
     const R* p = a.params ? a.params + (size_t)e * np : m.p_default;
-    const int N = a.tape_hdr[2 * e];
-    int knot = a.tape_hdr[2 * e + 1];
-    bool good = knot >= 0 && (!a.status || a.status[e] == 0);
+    const int N = a.tp.hdr[2 * e];
+    int knot = a.tp.hdr[2 * e + 1], n_unc = 0;
+    unsigned long long work[3] = {0, 0, 0};
+    long long first; int tape_cap;
+    tape_slot(a.tp, a.pl, e, first, tape_cap);
+    bool good = tape_ok && knot >= 0 && N <= tape_cap && (!a.status || a.status[e] == 0);
     if (good) {
       // ambient gradient at x_T -> tangent cotangent: lam = E(q_T)^T g
       const R* xT = a.xT + (size_t)e * nx; const R* gT = a.dLdxT + (size_t)e * nx;
@@ -110,19 +121,20 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
     }
 #pragma unroll 1
     for (int n = N - 1; n >= 0 && good; --n) {
-      const R* r = a.tape + ((size_t)e * a.tape_cap + n) * rec;
+      const R* r = a.tp.data + ((size_t)first + n) * rec;
 #pragma unroll 1
       for (int j = gr.lane; j < nq; j += G) rk.q()[j] = (double)r[j];
 #pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) rk.v()[j] = (double)r[nq + j];
-      double hs = (double)r[nx + 1], h = fabs(hs);
+      double tn, hs; tape_load_th(r, a.tp.o_th, tn, hs);      // t_n, h_n are fp64 on the tape in both precisions (G14)
+      const double h = fabs(hs);
       if (hs < 0) knot--;
       const R* u = has_ctrl ? a.ctrl + ((size_t)e * nknot + knot) * nu : a.zero_u;
-      if (a.tape_stages) for (int j = gr.lane; j < 6 * nv; j += G) rk.A()[j] = (double)r[nx + 2 + j];
+      if (a.tape_stages) for (int j = gr.lane; j < 6 * nv; j += G) rk.A()[j] = (double)r[a.tp.o_A + j];
       gr.sync();
       bool ok; int unc;
       // stage states: recomputed with F from the checkpoint, or rebuilt from the taped stage rates
-      rk_attempt<R, G, true>(m, tab, rk, Yqr, Vr, u, p, h, false, ws, ok, unc, gr, a.tape_stages != 0);
+      rk_attempt<R, G, SH, true>(m, tab, rk, Yqr, Vr, u, p, h, false, ws, ok, unc, gr, a.tape_stages != 0, work);
       // y_{n+1} = (q_n (+) h sum b_i K_i, v_n + h sum b_i A_i), b = row 6 of a
 #pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) {
@@ -151,8 +163,8 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
         for (int j = gr.lane; j < nv; j += G) Vr[j] = (R)rk.sV()[i * nv + j];
         gr.sync();
         // A_i = F(Y_i), or F~ for the straight-through estimator (Eq. 4)
-        if (!vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.Ab().at(i * nv), a.cfd != 0, a.want_p != 0, ws, rk, gr, a.dbg,
-                              (a.tape_stages && !a.cfd) ? rk.A().at(i * nv).p : nullptr)) { good = false; break; }   // F: x* = taped A_i
+        if (!vjp_stage<R, G, SH>(m, Yqr, Vr, u, p, rk.Ab().at(i * nv), a.cfd != 0, a.want_p != 0, ws, rk, gr, a.dbg,
+                              (a.tape_stages && !a.cfd) ? rk.A().at(i * nv).p : nullptr, &n_unc, work)) { good = false; break; }   // F: x* = taped A_i
 #pragma unroll 1
         for (int j = gr.lane; j < nv; j += G) rk.Vb()[j] += rk.vbar()[j];
         if (a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nu; c += G) a.dLdctrl[((size_t)e * nknot + knot) * nu + c] += (R)rk.ubar()[c];
@@ -178,6 +190,8 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
     for (int j = gr.lane; j < 2 * nv; j += G) g0[j] = good ? (R)rk.lam()[j] : R(0);
     if (a.dLdparams) for (int c = gr.lane; c < np; c += G) a.dLdparams[(size_t)e * np + c] = good ? (R)rk.gp()[c] : R(0);
     if (!good && a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nknot * nu; c += G) a.dLdctrl[(size_t)e * nknot * nu + c] = R(0);
+    if (a.n_unconv && gr.lane == 0) a.n_unconv[e] = n_unc;
+    if (a.work && gr.lane == 0) { a.work[6 * (size_t)e + 3] = work[0]; a.work[6 * (size_t)e + 4] = work[1]; a.work[6 * (size_t)e + 5] = work[2]; }
     gr.sync();
   }
   phase_drain();
@@ -190,7 +204,7 @@ template <class R> struct FieldArgs {
   R *acc, *qbar, *vbar, *ubar, *pbar; int* nrow;
   WsLayout wl; RkLayout rl;
 };
-template <class R, int G>
+template <class R, int G, class SH>
 __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ FieldArgs<R> a) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
@@ -199,8 +213,8 @@ __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ Mode
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
-  Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
-  bind_shared<R, G>(smem, a.rl.size_bwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
+  Rk<ST> rk; Ws<R, ST, SH> ws; Arr<R, ST> Yqr, Vr;
+  bind_shared<R, G, SH>(smem, a.rl.size_bwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
   const int nq = m.nq, nv = m.nv, nx = nq + nv;
   const int ngr = (gridDim.x * blockDim.x) / G;
 #pragma unroll 1
@@ -215,7 +229,7 @@ __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ Mode
     gr.sync();
     if (!a.kappa) {
       int conv;
-      int nr = field_eval<R, G>(u, p, a.cfd, &conv);
+      int nr = field_eval<R, G, SH>(u, p, a.cfd, &conv);
 #pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) a.acc[(size_t)e * nv + j] = nr < 0 ? R(nan("")) : ws.x()[j];
       if (gr.lane == 0 && a.nrow) a.nrow[e] = nr;
@@ -223,7 +237,7 @@ __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ Mode
 #pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) rk.lam()[j] = (double)a.kappa[(size_t)e * nv + j];
       gr.sync();
-      bool ok = vjp_stage<R, G>(m, Yqr, Vr, u, p, rk.lam(), a.cfd != 0, a.want_p != 0, ws, rk, gr);
+      bool ok = vjp_stage<R, G, SH>(m, Yqr, Vr, u, p, rk.lam(), a.cfd != 0, a.want_p != 0, ws, rk, gr);
       R bad = R(nan(""));
 #pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) { a.qbar[(size_t)e * nv + j] = ok ? (R)rk.qbar()[j] : bad; a.vbar[(size_t)e * nv + j] = ok ? (R)rk.vbar()[j] : bad; }
@@ -236,7 +250,7 @@ __global__ void __launch_bounds__(128) field_kernel(const __grid_constant__ Mode
 }
 
 // ---- A^: w(b) = mean diagonal of the translational block of Jc_b M(qpos0)^-1 Jc_b^T -------
-template <class R, int G>
+template <class R, int G, class SH>
 __global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ ModelDev<R> m_, const R* qpos0, const R* zero_v, R* body_w,
                                                         const __grid_constant__ WsLayout wl, const __grid_constant__ RkLayout rl) {
   unsigned char* smem = dyn_smem;
@@ -246,8 +260,8 @@ __global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ 
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
-  Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
-  bind_shared<R, G>(smem, rl.size_bwd, wl.size + rl.rsize, wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
+  Rk<ST> rk; Ws<R, ST, SH> ws; Arr<R, ST> Yqr, Vr;
+  bind_shared<R, G, SH>(smem, rl.size_bwd, wl.size + rl.rsize, wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
   if (blockIdx.x != 0 || threadIdx.x >= G) return;
   const int nv = m.nv;
 #pragma unroll 1
@@ -256,8 +270,8 @@ __global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ 
   for (int j = gr.lane; j < nv; j += G) Vr[j] = R(0);
   gr.sync();
   InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = zero_v; in.pa = m.p_default;
-  kinematics<Ws<R, ST>, R, G, InPlain<R, ST>, false>(m, in, ws, gr);
-  dynamics<Ws<R, ST>, R, G, InPlain<R, ST> >(m, in, ws, gr);
+  kinematics<Ws<R, ST, SH>, R, G, InPlain<R, ST>, false>(m, in, ws, gr);
+  dynamics<Ws<R, ST, SH>, R, G, InPlain<R, ST> >(m, in, ws, gr);
   const int ld = ws.L->ld;
 #pragma unroll 1
   for (int e = gr.lane; e < nv * ld; e += G) ws.Hc()[e] = ws.M()[e];
@@ -285,19 +299,19 @@ __global__ void __launch_bounds__(128) invweight_kernel(const __grid_constant__ 
   }
 }
 
-template <class R, int G> __global__ void prof_dump_kernel(unsigned long long* out) {
+template <class R, int G, class SH> __global__ void prof_dump_kernel(unsigned long long* out) {
   if (threadIdx.x < 32) { out[threadIdx.x] = g_prof[threadIdx.x]; g_prof[threadIdx.x] = 0; }
 }
 
 // ---- host launchers (defined per instantiation in dmx_inst.cuh) -----------------------------------------
 struct LaunchCfg { int block, grid; size_t smem; };
 
-template <class R, int G> cudaError_t launch_rollout(const ModelDev<R>& m, const RolloutArgs<R>& a, LaunchCfg c, cudaStream_t s);
-template <class R, int G> cudaError_t launch_backward(const ModelDev<R>& m, const BackwardArgs<R>& a, LaunchCfg c, cudaStream_t s);
-template <class R, int G> cudaError_t launch_field(const ModelDev<R>& m, const FieldArgs<R>& a, LaunchCfg c, cudaStream_t s);
-template <class R, int G> cudaError_t launch_invweight(const ModelDev<R>& m, const R* qpos0, const R* zero_v, R* body_w, const WsLayout& wl,
-                                                       const RkLayout& rl, LaunchCfg c, cudaStream_t s);
-template <class R, int G> cudaError_t launch_prof_dump(unsigned long long* out, cudaStream_t s);
-template <class R, int G> cudaError_t kernel_occupancy(int block, size_t smem_fwd, size_t smem_bwd, size_t smem_field, int* occ_fwd, int* occ_bwd, int* occ_field);
+template <class R, int G, class SH> cudaError_t launch_rollout(const ModelDev<R>& m, const RolloutArgs<R>& a, LaunchCfg c, cudaStream_t s);
+template <class R, int G, class SH> cudaError_t launch_backward(const ModelDev<R>& m, const BackwardArgs<R>& a, LaunchCfg c, cudaStream_t s);
+template <class R, int G, class SH> cudaError_t launch_field(const ModelDev<R>& m, const FieldArgs<R>& a, LaunchCfg c, cudaStream_t s);
+template <class R, int G, class SH> cudaError_t launch_invweight(const ModelDev<R>& m, const R* qpos0, const R* zero_v, R* body_w, const WsLayout& wl,
+                                                                 const RkLayout& rl, LaunchCfg c, cudaStream_t s);
+template <class R, int G, class SH> cudaError_t launch_prof_dump(unsigned long long* out, cudaStream_t s);
+template <class R, int G, class SH> cudaError_t kernel_occupancy(int block, size_t smem_fwd, size_t smem_bwd, size_t smem_field, int* occ_fwd, int* occ_bwd, int* occ_field);
 
 }  // namespace dmx

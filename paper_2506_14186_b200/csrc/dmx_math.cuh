@@ -46,6 +46,11 @@ DMX_DI int cta_barrier_and(int p) {
 DMX_DI void phase_sync(int id) { if (g_lockstep & (1 << id)) cta_barrier_and(0); }   // g_lockstep: mask of synchronised phases
 DMX_DI void phase_drain() { if (g_lockstep) while (!cta_barrier_and(1)) {} }
 
+// the CTA's dynamic shared memory: per-group workspaces (and, optionally, the constant arena at its end)
+extern __shared__ __align__(16) unsigned char dyn_smem[];
+template <class T> DMX_DI unsigned smem_off(const T* p) { return (unsigned)(reinterpret_cast<const unsigned char*>(p) - dyn_smem); }
+template <class T> DMX_DI T* smem_ptr(unsigned off) { return reinterpret_cast<T*>(dyn_smem + off); }
+
 // ---- tangent scalar: value and one directional derivative -------------------------------
 template <class T> struct Dual {
   T v, d;
@@ -67,6 +72,10 @@ template <class T> DMX_DI Dual<T>& operator-=(Dual<T>& a, const Dual<T>& b) { a.
 DMX_DI double val(double a) { return a; }
 DMX_DI float val(float a) { return a; }
 template <class T> DMX_DI T val(const Dual<T>& a) { return a.v; }
+
+DMX_DI bool has_tangent(double) { return false; }
+DMX_DI bool has_tangent(float) { return false; }
+template <class T> DMX_DI bool has_tangent(const Dual<T>& a) { return a.d != T(0); }
 
 template <class S> struct RealOf { typedef S type; };
 template <class T> struct RealOf<Dual<T> > { typedef T type; };
@@ -110,27 +119,32 @@ template <class S, int ST> struct Arr {
 
 // ---- lane group ----------------------------------------------------------------------------
 template <int G> struct Grp {
-  int lane; unsigned mask;
-  DMX_DI void sync() const { if (G > 1) __syncwarp(mask); }
+  int lane; unsigned mask_;
+  // A 32-lane group is the whole warp: the literal mask lets the compiler emit plain SHFL / WARPSYNC instead of the
+  // WARPSYNC.COLLECTIVE ... ENDCOLLECTIVE sequence it needs around a shuffle whose mask is a run-time value.
+  DMX_DI unsigned mask() const { return G == 32 ? 0xffffffffu : mask_; }
+  DMX_DI void sync() const { if (G > 1) __syncwarp(mask()); }
   DMX_DI bool all(bool pred) const {
     if (G == 1) return pred;
-    unsigned b = __ballot_sync(mask, pred);
-    return (b & mask) == mask;
+    unsigned b = __ballot_sync(mask(), pred);
+    return (b & mask()) == mask();
   }
   template <class T> DMX_DI T from_lane(T x, int src) const {   // value held by the group's lane `src` (uniform over the group)
     if (G == 1) return x;
-    return __shfl_sync(mask, x, ((threadIdx.x & 31) & ~(G - 1)) + src);
+    if (G == 32) return __shfl_sync(0xffffffffu, x, src);
+    return __shfl_sync(mask_, x, ((threadIdx.x & 31) & ~(G - 1)) + src);
   }
   DMX_DI int bcast_int(int x) const {            // value of the group's lane 0
     if (G == 1) return x;
-    return __shfl_sync(mask, x, (threadIdx.x & 31) & ~(G - 1));
+    if (G == 32) return __shfl_sync(0xffffffffu, x, 0);
+    return __shfl_sync(mask_, x, (threadIdx.x & 31) & ~(G - 1));
   }
 };
 template <int G> DMX_DI Grp<G> make_group() {
   Grp<G> g;
   int wl = threadIdx.x & 31;
   g.lane = wl & (G - 1);
-  g.mask = (G == 32) ? 0xffffffffu : (((1u << G) - 1u) << (wl & ~(G - 1)));
+  g.mask_ = (G == 32) ? 0xffffffffu : (((1u << G) - 1u) << (wl & ~(G - 1)));
   return g;
 }
 

@@ -64,13 +64,28 @@ struct WsLayout {
   int i_incl, i_rowstart, i_rowcand, i_active, isize;
 };
 
+// Compile-time sizes of a model (0: taken from the model at run time).  The kernels are instantiated once with
+// ShapeDyn for any model and once per BASELINE configuration with its sizes, so that the loops over dofs unroll, the
+// offsets i*ld+j fold into the instructions and the rows of M / H / L live in registers.  The tree,
+// joint and candidate tables stay run-time data: any model with these sizes takes the static instantiation.
+template <int NV_, int LD_, int NC_, int NR_> struct Shape { static const int NV = NV_, LD = LD_, NC = NC_, NR = NR_; };
+typedef Shape<0, 0, 0, 0> ShapeDyn;
+typedef Shape<8, 9, 2, 8> ShapeC2;        // planar push: 2 hinges + free sphere, 2 candidates x 4 rows
+typedef Shape<6, 7, 8, 32> ShapeC3;       // cube toss: free box, 8 corners x 4 rows
+typedef Shape<13, 13, 12, 48> ShapeC4;    // 7-hinge arm + free sphere, 12 candidates x 4 rows
+typedef Shape<18, 19, 4, 16> ShapeC5;     // quadruped: free trunk + 12 hinges, 4 feet x 4 rows
+
 // View of one workspace: base pointer + layout (kept in shared memory); arrays are resolved on use.
 #define DMX_WS_ARR(name) DMX_DI Arr<S, ST> name() const { return Arr<S, ST>(b + L->name * ST); }
 #define DMX_WS_INT(name) DMX_DI Arr<int, ST> name() const { return Arr<int, ST>(ib + L->i_##name * ST); }
-template <class S_, int ST_> struct Ws {
+template <class S_, int ST_, class SH_ = ShapeDyn> struct Ws {
   typedef S_ S;
+  typedef SH_ SH;
   static const int ST = ST_;
   S* b; int* ib; const WsLayout* L;
+  DMX_DI int ld() const { return SH::NV ? SH::LD : L->ld; }
+  template <class M> DMX_DI int nv(const M& m) const { return SH::NV ? SH::NV : m.nv; }
+  template <class M> DMX_DI int nc(const M& m) const { return SH::NV ? SH::NC : m.nc; }
   DMX_WS_ARR(fp) DMX_WS_ARR(fR) DMX_WS_ARR(fw) DMX_WS_ARR(fal) DMX_WS_ARR(fvp) DMX_WS_ARR(fap) DMX_WS_ARR(com) DMX_WS_ARR(dax) DMX_WS_ARR(dan)
   DMX_WS_ARR(Fb) DMX_WS_ARR(Nb) DMX_WS_ARR(Iw) DMX_WS_ARR(Isub) DMX_WS_ARR(tw)
   DMX_WS_ARR(M) DMX_WS_ARR(Hc) DMX_WS_ARR(tau) DMX_WS_ARR(c) DMX_WS_ARR(a0) DMX_WS_ARR(x) DMX_WS_ARR(g) DMX_WS_ARR(dl) DMX_WS_ARR(Md) DMX_WS_ARR(xa) DMX_WS_ARR(kap)

@@ -124,14 +124,15 @@ template <int ST_> struct Rk {
 // stride of the cooperative workspaces: contiguous per group, warp-interleaved for one-lane groups
 template <int G> struct StrideOf { static const int value = (G == 1) ? 32 : 1; };
 
-template <class R, int G> __device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* conv_out, const double* xk = nullptr);
+template <class R, int G, class SH> __device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* conv_out, const double* xk = nullptr);
 
 // ---- S7: one attempted step: stages 1..7 (stage 1 reused when have_k1), proposal, error vector -----
 // KEEP: also store every stage's (Yq, V, Dl) for the reverse sweep.
-template <class R, int G, bool KEEP>
+template <class R, int G, class SH, bool KEEP>
 DMX_DN void rk_attempt(const ModelDev<R>& m, int tab, const Rk<StrideOf<G>::value>& rk, const Arr<R, StrideOf<G>::value>& Yqr,
                        const Arr<R, StrideOf<G>::value>& Vr, const R* u, const R* p, double h, bool have_k1,
-                       const Ws<R, StrideOf<G>::value>& ws, bool& ok, int& unconverged, const Grp<G>& gr, bool restore = false) {
+                       const Ws<R, StrideOf<G>::value, SH>& ws, bool& ok, int& unconverged, const Grp<G>& gr, bool restore = false,
+                       unsigned long long* work = nullptr) {
   const int ST = StrideOf<G>::value;
   const int nv = m.nv, nq = m.nq;
   ok = true; unconverged = 0;
@@ -160,9 +161,13 @@ DMX_DN void rk_attempt(const ModelDev<R>& m, int tab, const Rk<StrideOf<G>::valu
     if (restore) continue;       // stage rates A_i come from the tape: stage states only
     if (i == 0 && have_k1) { for (int k = 0; k < 5; ++k) phase_sync(k); continue; }   // keep the CTA's phases aligned
     int conv;
-    int nr = field_eval<R, G>(u, p, 0, &conv);
+    int nr = field_eval<R, G, SH>(u, p, 0, &conv);
     if (nr < 0) { ok = false; for (int j = gr.lane; j < nv; j += G) rk.A()[i * nv + j] = nan(""); }
-    else { for (int j = gr.lane; j < nv; j += G) rk.A()[i * nv + j] = (double)ws.x()[j]; if (nr > 0 && !conv) unconverged++; }
+    else {
+      for (int j = gr.lane; j < nv; j += G) rk.A()[i * nv + j] = (double)ws.x()[j];
+      if (nr > 0 && !(conv & 1)) unconverged++;
+      if (work) { work[0] += (unsigned)(conv >> 8); work[1] += (unsigned long long)(conv >> 8) * nr; work[2] += (unsigned)nr; }
+    }
     gr.sync();
   }
   if (!KEEP) {
@@ -204,8 +209,27 @@ DMX_DN double error_norm(const ModelDev<R>& m, const Rk<ST>& rk, double rtol, do
 }
 
 // ---- kernel arguments ------------------------------------------------------------------------------
+// ---- S9: the tape in HBM ------------------------------------------------------
+// [meta 256 B | (n_acc, final knot)[nenv] | records].  A record is `rec` reals, a multiple of 16 bytes, written with
+// 16-byte stores: [q(nq) v(nv) | pad | t_n, h_n as two DOUBLES | A_1..A_6 (6 nv, when the stage rates are taped) | pad].
+// Environment e owns records [offset(e), offset(e) + cap(e)): uniform (e * cap) or, with a plan (dmx_tape_plan), the
+// prefix sum of per-environment capacities sized from a previous pass, so that one long environment does not size
+// every slot ("memory = number of checkpoints x state size").
+enum { TAPE_MAGIC = 0x646d7832, TAPE_META_INTS = 64 };
+template <class R> struct TapeView {
+  int rec, o_th, o_A;          // reals per record; offsets of (t, h) and of the stage rates (o_A < 0: not taped)
+  int uniform_cap;             // records per environment without a plan
+  long long capacity;          // records the buffer holds
+  int* meta;                   // [TAPE_META_INTS]: magic, nenv, rec, o_A, planned
+  int* hdr;                    // [nenv*2]: accepted steps on tape, final knot (-1-knot: failed)
+  R* data;
+};
+// Plan of a launch (dmx_tape_plan): hand-out order of the work queue (longest environment first, so that the launch
+// does not end on a lone long chain) and per-environment tape slots.  All null: identity / uniform.
+struct PlanView { const int* order; const int* cap; const long long* offset; };
+
 template <class R> struct RolloutArgs {
-  int nenv, nknot, n_replay, tape_cap, want_tape, lockstep, tape_stages;
+  int nenv, nknot, n_replay, want_tape, lockstep;
   const R *x0, *ctrl, *params, *zero_u;
   const double* h_replay;
   double knot_dt, horizon;
@@ -213,18 +237,50 @@ template <class R> struct RolloutArgs {
   R* xT;
   int *n_accept, *n_reject, *n_feval, *n_unconv, *status;
   double *h_min, *h_max, *t_end;
-  int* tape_hdr;          // [nenv*2]: accepted steps on tape, final knot
-  R* tape;                // [nenv][tape_cap][nq+nv+2]
+  unsigned long long* work;     // [nenv][6] or null: Newton iterations, row-iterations and rows, forward [0..2] / reverse sweep [3..5]
+  TapeView<R> tp; PlanView pl;
   int* queue;
+  double* rk_scratch;           // null: integrator arrays in shared memory; else [resident groups][size_fwd] in global memory
   WsLayout wl; RkLayout rl;
 };
+
+// slot of environment e: first record and capacity (0 when the plan does not fit the buffer)
+template <class R> DMX_DI void tape_slot(const TapeView<R>& tp, const PlanView& pl, int e, long long& first, int& cap) {
+  if (pl.offset) { first = pl.offset[e]; cap = pl.cap[e]; if (first + cap > tp.capacity) cap = 0; }
+  else { first = (long long)e * tp.uniform_cap; cap = tp.uniform_cap; }
+}
+// 16-byte chunk c of the record of the step (q_n, v_n, t_n, hs, A_1..6) held in the integrator arrays
+template <int ST> DMX_DI double tape_elem(const Rk<ST>& rk, int i, int nq, int nx, int o_A, int nA) {
+  if (i < nq) return rk.q()[i];
+  if (i < nx) return rk.v()[i - nq];
+  if (o_A >= 0 && i >= o_A && i < o_A + nA) return rk.A()[i - o_A];
+  return 0.0;
+}
+template <int ST> DMX_DI void tape_store_chunk(double* r, int c, const Rk<ST>& rk, int nq, int nx, int o_th, int o_A, int nA, double t, double hs) {
+  const int i = 2 * c;
+  double2 v;
+  if (i == o_th) { v.x = t; v.y = hs; }
+  else { v.x = tape_elem(rk, i, nq, nx, o_A, nA); v.y = tape_elem(rk, i + 1, nq, nx, o_A, nA); }
+  reinterpret_cast<double2*>(r)[c] = v;
+}
+template <int ST> DMX_DI void tape_store_chunk(float* r, int c, const Rk<ST>& rk, int nq, int nx, int o_th, int o_A, int nA, double t, double hs) {
+  const int i = 4 * c;
+  float4 v;
+  if (i == o_th) { double2 d; d.x = t; d.y = hs; v = *reinterpret_cast<float4*>(&d); }
+  else { v.x = (float)tape_elem(rk, i, nq, nx, o_A, nA); v.y = (float)tape_elem(rk, i + 1, nq, nx, o_A, nA);
+         v.z = (float)tape_elem(rk, i + 2, nq, nx, o_A, nA); v.w = (float)tape_elem(rk, i + 3, nq, nx, o_A, nA); }
+  reinterpret_cast<float4*>(r)[c] = v;
+}
+template <class R> DMX_DI void tape_load_th(const R* r, int o_th, double& t, double& hs) {
+  const double* d = reinterpret_cast<const double*>(r + o_th);
+  t = d[0]; hs = d[1];
+}
 
 // Shared-memory copies of the model header and the layouts (one per CTA), so that the non-inlined device
 // functions read them with plain shared loads.
 template <class R> struct CtaConst { ModelDev<R> m; WsLayout wl, rwl; RkLayout rl; int nd; };
 static __shared__ CtaConst<double> g_cc64;
 static __shared__ CtaConst<float> g_cc32;
-extern __shared__ __align__(16) unsigned char dyn_smem[];
 template <class R> DMX_DI CtaConst<R>& cta_const();
 template <> DMX_DI CtaConst<double>& cta_const<double>() { return g_cc64; }
 template <> DMX_DI CtaConst<float>& cta_const<float>() { return g_cc32; }
@@ -255,8 +311,8 @@ DMX_DI void load_cta_const(CtaConst<R>& c, const ModelDev<R>& m, const WsLayout&
 
 // workspace bases of this thread's lane group inside the CTA's dynamic shared memory:
 // [doubles | reals | ints], each region holding all groups of the CTA
-template <class R, int G>
-DMX_DI void bind_shared(unsigned char* smem, int nd, int nr_, int ni, Rk<StrideOf<G>::value>& rk, Ws<R, StrideOf<G>::value>& ws,
+template <class R, int G, class SH>
+DMX_DI void bind_shared(unsigned char* smem, int nd, int nr_, int ni, Rk<StrideOf<G>::value>& rk, Ws<R, StrideOf<G>::value, SH>& ws,
                         Arr<R, StrideOf<G>::value>& Yqr, Arr<R, StrideOf<G>::value>& Vr, const RkLayout* rl, const WsLayout* wl) {
   const int ST = StrideOf<G>::value;
   const int ngr = (G == 1) ? blockDim.x : blockDim.x / G;
@@ -272,39 +328,47 @@ DMX_DI void bind_shared(unsigned char* smem, int nd, int nr_, int ni, Rk<StrideO
 
 // F or F~ at the stage state held in this group's (Yqr, Vr); one copy per kernel, shared by the stage recomputation
 // and the VJP.  All pointers are re-derived from the CTA's shared memory, so the accesses stay shared-space loads.
-template <class R, int G>
+template <class R, int G, class SH>
 __device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* conv_out, const double* xk) {
   const int ST = StrideOf<G>::value;
   CtaConst<R>& cc = cta_const<R>();
   const Grp<G> gr = make_group<G>();
-  Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
-  bind_shared<R, G>(dyn_smem, cc.nd, cc.wl.size + cc.rl.rsize, cc.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
+  Rk<ST> rk; Ws<R, ST, SH> ws; Arr<R, ST> Yqr, Vr;
+  bind_shared<R, G, SH>(dyn_smem, cc.nd, cc.wl.size + cc.rl.rsize, cc.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
   InPlain<R, ST> in; in.qa = Yqr; in.va = Vr; in.aa = Vr; in.ua = u; in.pa = p;
-  bool conv;
-  int nr = vector_field<Ws<R, ST>, R, G, InPlain<R, ST> >(cc.m, in, ws, cfd != 0, conv, gr, xk, ST);
-  *conv_out = conv ? 1 : 0;
+  bool conv; int iters;
+  int nr = vector_field<Ws<R, ST, SH>, R, G, InPlain<R, ST> >(cc.m, in, ws, cfd != 0, conv, iters, gr, xk, ST);
+  *conv_out = (conv ? 1 : 0) | (iters << 8);       // bit 0: converged; bits 8..: Newton iterations taken
   return nr;
 }
 
 // ---- forward rollout: persistent lane groups pulling environments from a global queue --------------
-template <class R, int G>
+template <class R, int G, class SH>
 __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ RolloutArgs<R> a) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
   if (threadIdx.x == 0) g_lockstep = a.lockstep;
-  load_cta_const<R>(cc, m_, a.wl, a.wl, a.rl, a.rl.size_fwd);
+  const int nd_smem = a.rk_scratch ? 0 : a.rl.size_fwd;
+  load_cta_const<R>(cc, m_, a.wl, a.wl, a.rl, nd_smem);
   const ModelDev<R>& m = cc.m;
   const int ST = StrideOf<G>::value;
   const Grp<G> gr = make_group<G>();
-  Rk<ST> rk; Ws<R, ST> ws; Arr<R, ST> Yqr, Vr;
-  bind_shared<R, G>(smem, a.rl.size_fwd, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
-  const int nq = m.nq, nv = m.nv, nu = m.nu, nx = nq + nv, tab = a.so.tableau, rec = nx + 2 + (a.tape_stages ? 6 * nv : 0);
+  Rk<ST> rk; Ws<R, ST, SH> ws; Arr<R, ST> Yqr, Vr;
+  bind_shared<R, G, SH>(smem, nd_smem, a.wl.size + a.rl.rsize, a.wl.isize, rk, ws, Yqr, Vr, &cc.rl, &cc.wl);
+  if (a.rk_scratch) {
+    if (G == 1) rk.b = a.rk_scratch + ((size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32 * (size_t)a.rl.size_fwd + (threadIdx.x & 31);
+    else rk.b = a.rk_scratch + ((size_t)blockIdx.x * (blockDim.x / G) + threadIdx.x / G) * (size_t)a.rl.size_fwd;
+  }
+  const int nq = m.nq, nv = m.nv, nu = m.nu, nx = nq + nv, tab = a.so.tableau, rec = a.tp.rec;
   const bool has_ctrl = a.ctrl != nullptr && a.nknot > 0 && nu > 0;
   const int nknot = has_ctrl ? a.nknot : 0;
+  if (a.want_tape && blockIdx.x == 0 && threadIdx.x == 0) {   // what this tape holds; checked by the reverse sweep
+    a.tp.meta[0] = TAPE_MAGIC; a.tp.meta[1] = a.nenv; a.tp.meta[2] = rec; a.tp.meta[3] = a.tp.o_A; a.tp.meta[4] = a.pl.offset ? 1 : 0;
+  }
 #pragma unroll 1
   for (;;) {
     int e = 0;
-    if (gr.lane == 0) e = atomicAdd(a.queue, 1);
+    if (gr.lane == 0) { e = atomicAdd(a.queue, 1); if (e < a.nenv && a.pl.order) e = a.pl.order[e]; }
     e = gr.bcast_int(e);
     if (e >= a.nenv) break;
     const R* x0 = a.x0 + (size_t)e * nx;
@@ -316,9 +380,11 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
     gr.sync();
     double t = 0.0, hprop = a.so.h0, Eprev = 1.0, hmin = INFINITY, hmax = 0.0;
     int knot = 0, attempts = 0, ir = 0, status = 0, n_acc = 0, n_rej = 0, n_feval = 0, n_unc = 0;
+    unsigned long long work[3] = {0, 0, 0};
     bool have_k1 = false, last_nonfinite = false;
     const double* hr = a.h_replay ? a.h_replay + (size_t)e * a.n_replay : nullptr;
-    R* tape = a.want_tape ? a.tape + (size_t)e * a.tape_cap * rec : nullptr;
+    R* tape = nullptr; int tape_cap = 0;
+    if (a.want_tape) { long long first; tape_slot(a.tp, a.pl, e, first, tape_cap); tape = a.tp.data + (size_t)first * rec; }
     while (t < a.horizon) {
       double tb = has_ctrl ? fmin((knot + 1) * a.knot_dt, a.horizon) : a.horizon;
       if (knot + 1 >= nknot) tb = a.horizon;
@@ -332,10 +398,10 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
         if (hprop * (1.0 + 1e-7) >= rem) { h = rem; hits = true; } else { h = hprop; hits = false; }
         if (!hits && h < 1e-14 * fmax(1.0, fabs(t))) { status = last_nonfinite ? 3 : 2; break; }
       }
-      if (tape && n_acc >= a.tape_cap) { status = 4; break; }
+      if (tape && n_acc >= tape_cap) { status = 4; break; }
       attempts++;
       bool ok; int unc;
-      rk_attempt<R, G, false>(m, tab, rk, Yqr, Vr, u, p, h, have_k1, ws, ok, unc, gr);
+      rk_attempt<R, G, SH, false>(m, tab, rk, Yqr, Vr, u, p, h, have_k1, ws, ok, unc, gr, false, work);
       n_feval += have_k1 ? 6 : 7; n_unc += unc;
       have_k1 = true;
       bool finite = ok;
@@ -354,12 +420,9 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
       bool knot_up = hits && tb < a.horizon;
       if (tape) {   // S9: checkpoint record (y_n, t_n, +-h_n); a negative h marks a step that ends a control interval
         R* r = tape + (size_t)n_acc * rec;
+        const int nchunk = rec * (int)sizeof(R) / 16;
 #pragma unroll 1
-        for (int j = gr.lane; j < nq; j += G) r[j] = (R)rk.q()[j];
-#pragma unroll 1
-        for (int j = gr.lane; j < nv; j += G) r[nq + j] = (R)rk.v()[j];
-        if (gr.lane == 0) { r[nx] = (R)t; r[nx + 1] = (R)(knot_up ? -h : h); }
-        if (a.tape_stages) for (int j = gr.lane; j < 6 * nv; j += G) r[nx + 2 + j] = (R)rk.A()[j];   // stage rates A_1..A_6
+        for (int c = gr.lane; c < nchunk; c += G) tape_store_chunk(r, c, rk, nq, nx, a.tp.o_th, a.tp.o_A, 6 * nv, t, knot_up ? -h : h);
       }
       gr.sync();
 #pragma unroll 1
@@ -388,7 +451,8 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
       if (a.h_min) a.h_min[e] = hmin;
       if (a.h_max) a.h_max[e] = hmax;
       if (a.t_end) a.t_end[e] = t;
-      if (a.want_tape) { a.tape_hdr[2 * e] = n_acc; a.tape_hdr[2 * e + 1] = (status == 0) ? knot : -1 - knot; }
+      if (a.work) { a.work[6 * (size_t)e] = work[0]; a.work[6 * (size_t)e + 1] = work[1]; a.work[6 * (size_t)e + 2] = work[2]; }
+      if (a.want_tape) { a.tp.hdr[2 * e] = n_acc; a.tp.hdr[2 * e + 1] = (status == 0) ? knot : -1 - knot; }
     }
     gr.sync();
   }

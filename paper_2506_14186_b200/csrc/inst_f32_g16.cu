@@ -1,2 +1,2 @@
 #include "dmx_inst.cuh"
-DMX_INSTANTIATE(float, 16)
+DMX_INSTANTIATE(float, 16, ShapeDyn)

@@ -1,0 +1,2 @@
+#include "dmx_inst.cuh"
+DMX_INSTANTIATE(float, 16, ShapeC3)

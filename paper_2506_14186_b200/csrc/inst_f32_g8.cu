@@ -1,2 +1,2 @@
 #include "dmx_inst.cuh"
-DMX_INSTANTIATE(float, 8)
+DMX_INSTANTIATE(float, 8, ShapeDyn)

@@ -1,2 +1,2 @@
 #include "dmx_inst.cuh"
-DMX_INSTANTIATE(double, 1)
+DMX_INSTANTIATE(double, 1, ShapeDyn)

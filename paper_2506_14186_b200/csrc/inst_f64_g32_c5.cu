@@ -1,0 +1,2 @@
+#include "dmx_inst.cuh"
+DMX_INSTANTIATE(double, 32, ShapeC5)
