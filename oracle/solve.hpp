@@ -73,10 +73,17 @@ inline SolveResult contact_solve(int nv, int nr, const std::vector<double>& M, c
       for (int a = 0; a < nv; ++a) { double t = 0; for (int b = 0; b < nv; ++b) t += M[a * nv + b] * dl[b]; Md[a] = t; }
       double dMd = 0, dMxa = 0;
       for (int a = 0; a < nv; ++a) { dMd += dl[a] * Md[a]; dMxa += Md[a] * xa[a]; }
+      // Row sums in the fixed "32-slot" order that both sides document (D1/D4; SURVEY D4 allows any fixed
+      // shared order): row i goes to slot i mod 32 in increasing i, the slots are then combined pairwise,
+      // slot[k] += slot[k xor s] for s = 1, 2, 4, 8, 16.
       auto d1 = [&](double a, double& d2) {
-        double v1 = dMxa + a * dMd; d2 = dMd;
-        for (int i = 0; i < nr; ++i) { double si = s[i] + a * p[i]; if (si < 0.0) { v1 += D[i] * p[i] * si; d2 += D[i] * p[i] * p[i]; } }
-        return v1;
+        double s1[32], s2[32];
+        for (int k = 0; k < 32; ++k) { s1[k] = 0.0; s2[k] = 0.0; }
+        for (int i = 0; i < nr; ++i) { double si = s[i] + a * p[i]; if (si < 0.0) { s1[i % 32] += D[i] * p[i] * si; s2[i % 32] += D[i] * p[i] * p[i]; } }
+        for (int sft = 1; sft < 32; sft <<= 1)
+          for (int k = 0; k < 32; ++k) if (!(k & sft)) { s1[k] = s1[k] + s1[k ^ sft]; s2[k] = s2[k] + s2[k ^ sft]; }
+        d2 = dMd + s2[0];
+        return (dMxa + a * dMd) + s1[0];
       };
       double lo = 0.0, hi = INFINITY, a = 0.0, d2; double d1a = d1(0.0, d2);
       bool frozen = false;

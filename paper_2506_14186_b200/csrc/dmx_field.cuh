@@ -496,20 +496,46 @@ DMX_DN int build_rows(const ModelDev<R>& m, const IN& in, const WS& ws, bool cfd
 
 
 // ---- D1: line search of S6.  phi'(a) = dl^T M (x + a dl - a0) + sum_i D_i p_i min(0, s_i + a p_i) is piecewise linear and
-// increasing; bracketed 1-D Newton from a = 1.  Every lane runs the scalar search redundantly on the group's shared
-// arrays (Md = M dl, xa = x - a0, s, pr = J dl, D) in row order: the summation order of a serial code, uniform result.
-template <class WS>
-DMX_DN typename WS::S line_search(int nv, int nr, int n_ls, const WS& ws) {
+// increasing; bracketed 1-D Newton from a = 1.  The two row sums of an iterate (phi' and phi'') are taken cooperatively
+// in the fixed order both sides document (D1/D4, "32-slot order"): row i is added to slot i mod 32 in
+// increasing i, then the slots are combined by the butterfly slot[k] += slot[k xor s], s = 1, 2, 4, 8, 16.  A group of
+// G lanes holds slots lane, lane + G, ... (32 / G per lane): the steps s < G are shuffles, the others in-lane adds.
+// The butterfly leaves the same bits in every lane, so the search stays uniform over the group.
+template <class WS, int G>
+DMX_DI void ls_row_sums(int nr, const WS& ws, const Grp<G>& gr, const typename WS::S& a, typename WS::S& r1, typename WS::S& r2) {
+  typedef typename WS::S S;
+  const int NCOMP = 32 / G;
+  S p1[NCOMP], p2[NCOMP];
+#pragma unroll
+  for (int c = 0; c < NCOMP; ++c) {
+    p1[c] = S(0.0); p2[c] = S(0.0);
+#pragma unroll 1
+    for (int i = gr.lane + c * G; i < nr; i += 32) {
+      const S pi = ws.pr()[i], si = ws.s()[i] + a * pi;
+      if (val(si) < 0) { const S dp = ws.D()[i] * pi; p1[c] = p1[c] + dp * si; p2[c] = p2[c] + dp * pi; }
+    }
+  }
+#pragma unroll
+  for (int sft = 1; sft < G; sft <<= 1) {
+#pragma unroll
+    for (int c = 0; c < NCOMP; ++c) { p1[c] = p1[c] + gr.xor_lane(p1[c], sft); p2[c] = p2[c] + gr.xor_lane(p2[c], sft); }
+  }
+#pragma unroll
+  for (int sft = 1; sft < NCOMP; sft <<= 1) {
+#pragma unroll
+    for (int c = 0; c < NCOMP; c += 2 * sft) { p1[c] = p1[c] + p1[c + sft]; p2[c] = p2[c] + p2[c + sft]; }
+  }
+  r1 = p1[0]; r2 = p2[0];
+}
+template <class WS, int G>
+DMX_DN typename WS::S line_search(int nv, int nr, int n_ls, const WS& ws, const Grp<G>& gr) {
   typedef typename WS::S S;
   S dMd(0.0), dMxa(0.0);
 #pragma unroll 1
   for (int a = 0; a < nv; ++a) { dMd = dMd + ws.dl()[a] * ws.Md()[a]; dMxa = dMxa + ws.Md()[a] * ws.xa()[a]; }
-  S lo(0.0), hi(0.0), a(0.0), d2, d1a; bool hi_inf = true, frozen = false;
-  {
-    d1a = dMxa; d2 = dMd;
-#pragma unroll 1
-    for (int i = 0; i < nr; ++i) { S si = ws.s()[i]; if (val(si) < 0) { d1a = d1a + ws.D()[i] * ws.pr()[i] * si; d2 = d2 + ws.D()[i] * ws.pr()[i] * ws.pr()[i]; } }
-  }
+  S lo(0.0), hi(0.0), a(0.0), d2, d1a, r1, r2; bool hi_inf = true, frozen = false;
+  ls_row_sums<WS, G>(nr, ws, gr, a, r1, r2);
+  d1a = dMxa + r1; d2 = dMd + r2;
 #pragma unroll 1
   for (int ls = 0; ls < n_ls && !frozen; ++ls) {
     S an = (ls == 0) ? S(1.0) : a - d1a / d2;
@@ -517,12 +543,8 @@ DMX_DN typename WS::S line_search(int nv, int nr, int n_ls, const WS& ws) {
     bool inside = (val(an) > val(lo)) && (hi_inf || val(an) < val(hi));
     if (!inside) an = hi_inf ? S(2.0) * (val(a) > 1 ? a : S(1.0)) : S(0.5) * (lo + hi);
     a = an;
-    d1a = dMxa + a * dMd; d2 = dMd;
-#pragma unroll 1
-    for (int i = 0; i < nr; ++i) {
-      S si = ws.s()[i] + a * ws.pr()[i];
-      if (val(si) < 0) { d1a = d1a + ws.D()[i] * ws.pr()[i] * si; d2 = d2 + ws.D()[i] * ws.pr()[i] * ws.pr()[i]; }
-    }
+    ls_row_sums<WS, G>(nr, ws, gr, a, r1, r2);
+    d1a = (dMxa + a * dMd) + r1; d2 = dMd + r2;
     if (val(d1a) < 0) lo = a; else if (val(d1a) > 0) { hi = a; hi_inf = false; } else frozen = true;
   }
   return a;
@@ -711,7 +733,7 @@ DMX_DN bool newton_static(int nr, int n_it, int n_ls, const WS& ws, const Grp<G>
       gr.sync();
     }
     S alpha(1.0);
-    if (!same) alpha = line_search<WS>(NV, nr, n_ls, ws);
+    if (!same) alpha = line_search<WS, G>(NV, nr, n_ls, ws, gr);
     xa_ = xa_ + alpha * dla;
     if (own) ws.x()[a] = xa_;
     gr.sync();
@@ -791,7 +813,7 @@ DMX_DN bool newton(int nv, int nr, int n_it, int n_ls, const WS& ws, const Grp<G
         ws.Md()[a] = t;
       }
       gr.sync();
-      alpha = line_search<WS>(nv, nr, n_ls, ws);
+      alpha = line_search<WS, G>(nv, nr, n_ls, ws, gr);
     }
 #pragma unroll 1
     for (int j = gr.lane; j < nv; j += G) ws.x()[j] = ws.x()[j] + alpha * ws.dl()[j];

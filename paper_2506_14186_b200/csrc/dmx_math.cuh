@@ -134,6 +134,10 @@ template <int G> struct Grp {
     if (G == 32) return __shfl_sync(0xffffffffu, x, src);
     return __shfl_sync(mask_, x, ((threadIdx.x & 31) & ~(G - 1)) + src);
   }
+  template <class T> DMX_DI T xor_lane(T x, int s) const {       // value held by the group's lane (lane xor s), s < G
+    if (G == 1) return x;
+    return __shfl_xor_sync(mask(), x, s);
+  }
   DMX_DI int bcast_int(int x) const {            // value of the group's lane 0
     if (G == 1) return x;
     if (G == 32) return __shfl_sync(0xffffffffu, x, 0);

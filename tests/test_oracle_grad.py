@@ -222,3 +222,41 @@ def test_P12_batch_independence(oracle_mod):
     assert np.array_equal(part["xT"], full["xT"][perm])
     assert np.array_equal(part["stats"]["n_accept"], full["stats"]["n_accept"][perm])
     assert len(set(full["stats"]["n_accept"].tolist())) > 1      # step sizes are per environment
+
+
+def test_unconverged_newton_gradient_is_flagged_and_quantified(oracle_mod):
+    """Reading G9 (PAPER.md:68, 515, 539 fixed iteration counts; PAPER.md:543 implicit differentiation): the VJP is the
+    implicit-function gradient at the final active set, which is the gradient of the computed F only when the fixed
+    budget of Newton iterations ended on a full step inside an unchanged active set.  Otherwise the evaluation is counted
+    (n_newton_unconverged, n_newton_unconverged_bwd) and this test quantifies what the count means, on a state of the
+    BASELINE workload itself: C3 environment 2022 lands flat on a face at t = 0.5145 s (16 rows), where 4 iterations
+    are not enough.  Measured there: F differs from the converged solution by 0.8 %; the implicit gradient differs from
+    central differences of the 4-iteration map by 7.5 % (and that map is discontinuous: on neighbouring states of the same
+    impact the difference quotient grows without bound as eps -> 0) and from the converged gradient by 21 %; with 50
+    iterations the solve converges and the implicit gradient equals central differences to 1e-7.  The same environment
+    takes 11 007 accepted steps with the 4-iteration budget and 450 with 8 iterations (step size collapses to 2e-8 s while
+    F is noisy): DESIGN.md section 5."""
+    w = W.make("C3")                               # the draws of an environment depend on the batch size: BASELINE batch
+    x0 = w["x0"][2022:2023]
+    orc = oracle_mod.Oracle(w["model"])
+    r = orc.rollout(x0, None, 0, 0.0, None, 0.5145, w["opts"])
+    assert r["stats"]["status"][0] == 0 and r["stats"]["n_newton_unconverged"][0] > 0        # the forward pass counts it
+    x = r["xT"][0]; q, v = x[:7], x[7:]
+    p = orc.default_params()
+    a4, nr, conv = orc.vector_field(q, v, None, p, False)
+    assert nr == 16 and not conv
+    kap = np.random.default_rng(0).normal(size=6)
+    g4 = np.concatenate(orc.vjp_field(q, v, None, p, kap, False)[:2])
+    fd4 = np.concatenate(fd_vjp_field(orc, q, v, None, p, kap, False, eps=1e-7)[:2])
+    e4 = np.abs(g4 - fd4).max() / np.abs(fd4).max()
+    mdl = dict(w["model"]); mdl["newton_iters"] = 50
+    o50 = oracle_mod.Oracle(mdl)
+    a50, _, conv50 = o50.vector_field(q, v, None, p, False)
+    g50 = np.concatenate(o50.vjp_field(q, v, None, p, kap, False)[:2])
+    fd50 = np.concatenate(fd_vjp_field(o50, q, v, None, p, kap, False, eps=1e-7)[:2])
+    e50 = np.abs(g50 - fd50).max() / np.abs(fd50).max()
+    print("unconverged state: |F4-F50|/|F50| = %.2e, implicit gradient vs FD of the 4-iteration map %.2e, vs converged gradient %.2e; "
+          "50 iterations: vs FD %.2e" % (np.abs(a4 - a50).max() / np.abs(a50).max(), e4, np.abs(g4 - g50).max() / np.abs(g50).max(), e50))
+    assert conv50 and e50 < 1e-5
+    assert 1e-3 < e4 < 1.0                         # a real discrepancy, of the size recorded above
+    assert 1e-4 < np.abs(a4 - a50).max() / np.abs(a50).max() < 0.1
