@@ -328,14 +328,15 @@ template <class S> __device__ __noinline__ S imp_spline_pow(S x, S mid, S power)
   if (val(x) <= val(mid)) return m_pow(x, power) / m_pow(mid, power - one);
   return one - m_pow(one - x, power) / m_pow(one - mid, power - one);
 }
+template <class S> DMX_DI S int_pow(const S& x, int n) { S r = x; for (int k = 1; k < n; ++k) r = r * x; return r; }   // n >= 1
 template <class S> DMX_DI S imp_spline(const S& x, const S& mid, const S& power) {
   if (val(x) <= 0) return S(0.0) * x;
   if (val(x) >= 1) return S(1.0) + S(0.0) * x;
   S one(1.0);
-  if (val(power) == 2.0 && !has_tangent(power)) {   // x^2 / mid and 1 - (1-x)^2 / (1-mid): same values as pow up to its rounding
-    if (val(x) <= val(mid)) return x * x / mid;
-    S y = one - x;
-    return one - y * y / (one - mid);
+  const int n = (int)val(power);
+  if (n >= 2 && n <= 8 && val(power) == (double)n && !has_tangent(power)) {   // integer exponent (2: PAPER.md:347, 537; 4: the CFD
+    if (val(x) <= val(mid)) return int_pow(x, n) / int_pow(mid, n - 1);       // spline): products instead of pow
+    return one - int_pow(one - x, n) / int_pow(one - mid, n - 1);
   }
   return imp_spline_pow<S>(x, mid, power);
 }

@@ -9,7 +9,7 @@
 namespace dmx {
 
 // ---- Butcher tableaus: index 0 Dopri5 (Dormand & Prince 1980), 1 Tsit5 (Tsitouras 2011)
-static __device__ const double TAB_A[2][7][7] = {
+static __constant__ double TAB_A[2][7][7] = {
     {{0},
      {1.0 / 5},
      {3.0 / 40, 9.0 / 40},
@@ -25,7 +25,7 @@ static __device__ const double TAB_A[2][7][7] = {
      {5.86145544294642, -12.92096931784711, 8.159367898576159, -0.071584973281401, -0.028269050394068383},
      {0.09646076681806523, 0.01, 0.4798896504144996, 1.379008574103742, -3.290069515436081, 2.324710524099774}}};
 // e = b - bhat; b is row 6 of a (FSAL)
-static __device__ const double TAB_E[2][7] = {
+static __constant__ double TAB_E[2][7] = {
     {35.0 / 384 - 5179.0 / 57600, 0.0, 500.0 / 1113 - 7571.0 / 16695, 125.0 / 192 - 393.0 / 640,
      -2187.0 / 6784 - (-92097.0 / 339200), 11.0 / 84 - 187.0 / 2100, 0.0 - 1.0 / 40},
     {-0.00178001105222577714, -0.0008164344596567469, 0.007880878010261995, -0.1447110071732629,
