@@ -6,6 +6,7 @@
 #include <cstring>
 #include <cstdio>
 #include "rk.hpp"
+#include "adjoint.hpp"
 
 using namespace orc;
 
@@ -259,6 +260,42 @@ int orc_rollout_grad(void* h, int e0, int e1, const double* x0, const double* ct
       if (gc) for (int i = 0; i < nknot * m.nu; ++i) gc[i] = 0.0;
       if (gp) for (int i = 0; i < m.np; ++i) gp[i] = 0.0;
     }
+    for (int i = 0; i < 2 * nv; ++i) dLdx0[(size_t)e * 2 * nv + i] = lam[i];
+  }
+  return 0;
+}
+
+// forward with tape, then the continuous adjoint solved backwards with its own steps (adjoint.hpp; PAPER.md:435-448,
+// 462-477).  adj: solver options of the backward solve.  asub [nenv,3]: accepted / rejected sub-steps, status.
+int orc_rollout_grad_adjoint(void* h, int e0, int e1, const double* x0, const double* ctrl, int nknot, double knot_dt, const double* params,
+                             double horizon, const orc_opts* opts, const orc_opts* adj, const double* h_replay, int n_replay, const double* dLdxT,
+                             int cfd_on, double* xT, int* istats, double* dstats, int* asub, double* dLdx0, double* dLdctrl, double* dLdparams) {
+  Model& m = *(Model*)h; SolverOpts so = so_of(opts), sa = so_of(adj); int nx = m.nq + m.nv, nv = m.nv;
+  for (int e = e0; e < e1; ++e) {
+    EnvStats st; std::vector<TapeRec> tape;
+    const double* ce = ctrl ? ctrl + (size_t)e * nknot * m.nu : nullptr;
+    const double* pe = params ? params + (size_t)e * m.np : m.p_default.data();
+    rollout_env(m, x0 + (size_t)e * nx, ce, ctrl ? nknot : 0, knot_dt, pe, horizon, so,
+                h_replay ? h_replay + (size_t)e * n_replay : nullptr, n_replay, xT + (size_t)e * nx, st, &tape);
+    istats[5 * e] = st.n_accept; istats[5 * e + 1] = st.n_reject; istats[5 * e + 2] = st.n_feval; istats[5 * e + 3] = st.n_unconv; istats[5 * e + 4] = st.status;
+    dstats[3 * e] = st.h_min; dstats[3 * e + 1] = st.h_max; dstats[3 * e + 2] = st.t_end;
+    std::vector<double> lam(2 * nv, 0.0);
+    double* gc = dLdctrl ? dLdctrl + (size_t)e * nknot * m.nu : nullptr;
+    double* gp = dLdparams ? dLdparams + (size_t)e * m.np : nullptr;
+    if (gc) for (int i = 0; i < nknot * m.nu; ++i) gc[i] = 0.0;
+    if (gp) for (int i = 0; i < m.np; ++i) gp[i] = 0.0;
+    bool ok = st.status == 0;
+    AdjStats as;
+    if (ok) {
+      ambient_to_tangent(m, xT + (size_t)e * nx, dLdxT + (size_t)e * nx, lam.data());
+      ok = reverse_sweep_continuous(m, tape, ce, ctrl ? nknot : 0, pe, so, sa, cfd_on != 0, lam.data(), gc, gp, as);
+    }
+    if (!ok) {
+      for (auto& l : lam) l = 0.0;
+      if (gc) for (int i = 0; i < nknot * m.nu; ++i) gc[i] = 0.0;
+      if (gp) for (int i = 0; i < m.np; ++i) gp[i] = 0.0;
+    }
+    if (asub) { asub[3 * e] = as.n_accept; asub[3 * e + 1] = as.n_reject; asub[3 * e + 2] = ok ? 0 : (as.status ? as.status : 3); }
     for (int i = 0; i < 2 * nv; ++i) dLdx0[(size_t)e * 2 * nv + i] = lam[i];
   }
   return 0;

@@ -13,7 +13,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = os.path.join(_HERE, "liboracle.so")
-_SRC = ["capi.cpp", "rk.hpp", "field.hpp", "solve.hpp", "contact.hpp", "kin.hpp", "model.hpp", "dual.hpp"]
+_SRC = ["capi.cpp", "adjoint.hpp", "rk.hpp", "field.hpp", "solve.hpp", "contact.hpp", "kin.hpp", "model.hpp", "dual.hpp"]
 
 
 def build(force=False):
@@ -215,6 +215,31 @@ class Oracle:
                                C.byref(o), _p(h_replay), nrep, _p(dLdxT), int(cfd_on), _p(xT), _p(ist), _p(dst), _p(g0), _p(gc), _p(gp))
         self._run(fn, nenv, threads)
         return dict(xT=xT, stats=_stats(ist, dst), dLdx0=g0, dLdctrl=gc, dLdparams=gp)
+
+
+def _adjoint(self, x0, ctrl, nknot, knot_dt, params, horizon, opts, adj_opts, dLdxT, cfd_on=False, h_replay=None, want_params=True, threads=1):
+    """Optimize-then-discretize gradient (adjoint.hpp): forward with tape, then the continuous adjoint solved backwards
+    with its own error-controlled steps under adj_opts.  Returns the fields of rollout_grad plus adj_accept / adj_reject /
+    adj_status per environment."""
+    x0 = _f8(x0); nenv = x0.shape[0]
+    ctrl, params, h_replay, dLdxT = _f8(ctrl), _f8(params), _f8(h_replay), _f8(dLdxT)
+    xT = np.zeros_like(x0); ist = np.zeros((nenv, 5), dtype=np.int32); dst = np.zeros((nenv, 3)); asub = np.zeros((nenv, 3), dtype=np.int32)
+    g0 = np.zeros((nenv, 2 * self.nv))
+    gc = np.zeros((nenv, nknot, self.nu)) if (ctrl is not None and nknot > 0) else None
+    gp = np.zeros((nenv, self.np_)) if want_params else None
+    o, oa = self._opts(opts), self._opts(adj_opts); nrep = 0 if h_replay is None else h_replay.shape[1]
+    L = lib()
+
+    def fn(e0, e1):
+        L.orc_rollout_grad_adjoint(self.h, e0, e1, _p(x0), _p(ctrl), int(nknot), C.c_double(knot_dt), _p(params), C.c_double(horizon),
+                                   C.byref(o), C.byref(oa), _p(h_replay), nrep, _p(dLdxT), int(cfd_on), _p(xT), _p(ist), _p(dst), _p(asub),
+                                   _p(g0), _p(gc), _p(gp))
+    self._run(fn, nenv, threads)
+    return dict(xT=xT, stats=_stats(ist, dst), dLdx0=g0, dLdctrl=gc, dLdparams=gp, adj_accept=asub[:, 0].copy(), adj_reject=asub[:, 1].copy(),
+                adj_status=asub[:, 2].copy())
+
+
+Oracle.rollout_grad_adjoint = _adjoint
 
 
 def _stats(ist, dst):
