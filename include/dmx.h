@@ -180,6 +180,33 @@ int dmx_rollout_backward(const dmx_model *m, int nenv, const void *ctrl, int nkn
                          void *dLdx0, void *dLdctrl, void *dLdparams, const dmx_stats *stats,
                          const void *tape, size_t tape_bytes, const void *plan, void *cuda_stream);
 
+/* Optimize-then-discretize (Eq. 6-7; with cfd_on the altered adjoint equations PAPER.md:462-477,
+ * Eq. 8-9): the gradient as the solution of the continuous adjoint equations, solved BACKWARDS with its own
+ * error-controlled steps under adj_opts (tableau, rtol, atol over the 2*nv adjoint components, controller constants,
+ * max_steps = budget of attempted sub-steps per environment; h0 is not used: the first proposal is the last forward
+ * step).  Inside an accepted forward step the state is the cubic Hermite interpolant, in the step's chart, of the end
+ * values and rates held on the tape (plus one evaluation of F at the end of the step); sub-steps are clipped to the
+ * tape's checkpoints.  PAPER.md:452, 473-475 (Fig. 19): with CFD the adjoint equation can be stiff where the forward one
+ * is not, and unrolling the (large) forward steps gives wrong gradients whatever the forward tolerance; this call is the
+ * remedy.  Same arguments and outputs as dmx_rollout_backward / dmx_rollout_grad, plus
+ *   adj_info  device int [nenv, 3] or NULL (out): accepted sub-steps, rejected sub-steps, status (0 ok, 1 sub-step
+ *             budget, 2 sub-step underflow, 3 evaluation failed); a failed environment returns zero gradients.
+ *   adj_replay device double [nenv, n_adj_replay] or NULL: if given, exactly these sub-steps are taken in order, without
+ *             error control (each must end inside or at the end of the current forward step; a non-positive entry or a
+ *             sub-step that overshoots fails the environment) - the backward counterpart of h_replay.
+ * xT, stats and the tape do not depend on the gradient mode. */
+int dmx_rollout_backward_adjoint(const dmx_model *m, int nenv, const void *ctrl, int nknot, const void *params,
+                                 const dmx_solver_opts *opts, const dmx_solver_opts *adj_opts, const void *xT,
+                                 const void *dLdxT, int cfd_on, void *dLdx0, void *dLdctrl, void *dLdparams,
+                                 const dmx_stats *stats, int *adj_info, const double *adj_replay, int n_adj_replay,
+                                 const void *tape, size_t tape_bytes, const void *plan, void *cuda_stream);
+int dmx_rollout_grad_adjoint(const dmx_model *m, int nenv, const void *x0, const void *ctrl, int nknot, double knot_dt,
+                             const void *params, double horizon, const dmx_solver_opts *opts,
+                             const dmx_solver_opts *adj_opts, const double *h_replay, int n_replay, const void *dLdxT,
+                             int cfd_on, void *xT, void *dLdx0, void *dLdctrl, void *dLdparams, const dmx_stats *stats,
+                             int *adj_info, const double *adj_replay, int n_adj_replay, void *tape, size_t tape_bytes,
+                             const void *plan, void *cuda_stream);
+
 /* Building blocks exposed for parity tests (one lane-group per state, same device code as the
  * rollouts).  All pointers DEVICE, real typed; n states.
  *   dmx_vector_field: acc[n,nv] = F(q,v,u,p) or F~ when cfd (Eq. 1, 2, 4); nrow[n] rows in the solve.

@@ -58,13 +58,16 @@ struct AdjStep {
 // lam (2 nv) in: cotangent at x_T, out: cotangent at x_0.  gctrl[nknot*nu], gp[np] accumulated (may be null).
 inline bool reverse_sweep_continuous(const Model& m, const std::vector<TapeRec>& tape, const double* ctrl, int nknot,
                                      const double* p, const SolverOpts& so, const SolverOpts& sa, bool cfd, double* lam,
-                                     double* gctrl, double* gp, AdjStats& st) {
+                                     double* gctrl, double* gp, AdjStats& st, const double* hs_replay = nullptr, int n_replay = 0,
+                                     std::vector<double>* hs_out = nullptr) {
+  // hs_replay: if non-null, exactly these sub-steps are taken in order (no error control), like h_replay of the forward
+  // solve; hs_out collects the accepted sub-steps
   Tableau T = sa.tableau == 0 ? dopri5() : tsit5();
   Tableau Tf = so.tableau == 0 ? dopri5() : tsit5();
   int nv = m.nv, nu = m.nu, np = m.np, n2 = 2 * nv;
   std::vector<double> uzero(nu > 0 ? nu : 1, 0.0);
   StepWork W;
-  double hprop = -1.0, Eprev = 1.0; int attempts = 0;
+  double hprop = -1.0, Eprev = 1.0; int attempts = 0, ir = 0;
   st = AdjStats();
   std::vector<std::vector<double>> k(7, std::vector<double>(n2)), ub(7, std::vector<double>(nu > 0 ? nu : 1)), pb(7, std::vector<double>(np));
   std::vector<double> mu(n2), mus(n2), munew(n2), err(n2);
@@ -91,8 +94,14 @@ inline bool reverse_sweep_continuous(const Model& m, const std::vector<TapeRec>&
     while (s < h) {
       if (attempts >= sa.max_steps) { st.status = 1; return false; }
       double rem = h - s, hs; bool hits;
-      if (hprop * (1.0 + 1e-7) >= rem) { hs = rem; hits = true; } else { hs = hprop; hits = false; }
-      if (!hits && hs < 1e-14 * std::fmax(1.0, h)) { st.status = 2; return false; }
+      if (hs_replay) {
+        if (ir >= n_replay || !(hs_replay[ir] > 0.0)) { st.status = 1; return false; }
+        hs = hs_replay[ir++]; hits = (hs == rem);
+        if (hs > rem) { st.status = 3; return false; }
+      } else {
+        if (hprop * (1.0 + 1e-7) >= rem) { hs = rem; hits = true; } else { hs = hprop; hits = false; }
+        if (!hits && hs < 1e-14 * std::fmax(1.0, h)) { st.status = 2; return false; }
+      }
       attempts++;
       for (int i = 0; i < 7; ++i) {
         if (i == 0 && have_k1) continue;
@@ -110,7 +119,8 @@ inline bool reverse_sweep_continuous(const Model& m, const std::vector<TapeRec>&
         if (!std::isfinite(err[j]) || !std::isfinite(munew[j])) finite = false;
       }
       double E = INFINITY; bool accept = false;
-      if (finite) {
+      if (hs_replay) { if (!finite) return false; accept = true; E = 1.0; }
+      else if (finite) {
         double acc = 0.0;
         for (int j = 0; j < n2; ++j) { double q = err[j] / (sa.atol + sa.rtol * std::fmax(std::fabs(mu[j]), std::fabs(munew[j]))); acc = acc + q * q; }
         E = std::sqrt(acc / n2); accept = E <= 1.0;
@@ -121,6 +131,7 @@ inline bool reverse_sweep_continuous(const Model& m, const std::vector<TapeRec>&
       if (!accept || !hits) hprop = hs * fac;
       if (!accept) { st.n_reject++; continue; }
       Eprev = Ec; st.n_accept++;
+      if (hs_out) hs_out->push_back(hs);
       if (gctrl && nknot > 0) for (int a = 0; a < nu; ++a) { double t = 0; for (int i = 0; i < 6; ++i) t += T.b[i] * ub[i][a]; gctrl[(size_t)r.knot * nu + a] += hs * t; }
       if (gp) for (int a = 0; a < np; ++a) { double t = 0; for (int i = 0; i < 6; ++i) t += T.b[i] * pb[i][a]; gp[a] += hs * t; }
       mu = munew; k[0] = k[6]; ub[0] = ub[6]; pb[0] = pb[6];      // FSAL inside the step

@@ -269,7 +269,8 @@ int orc_rollout_grad(void* h, int e0, int e1, const double* x0, const double* ct
 // 462-477).  adj: solver options of the backward solve.  asub [nenv,3]: accepted / rejected sub-steps, status.
 int orc_rollout_grad_adjoint(void* h, int e0, int e1, const double* x0, const double* ctrl, int nknot, double knot_dt, const double* params,
                              double horizon, const orc_opts* opts, const orc_opts* adj, const double* h_replay, int n_replay, const double* dLdxT,
-                             int cfd_on, double* xT, int* istats, double* dstats, int* asub, double* dLdx0, double* dLdctrl, double* dLdparams) {
+                             int cfd_on, double* xT, int* istats, double* dstats, int* asub, double* dLdx0, double* dLdctrl, double* dLdparams,
+                             const double* adj_replay, int n_adj_replay, double* adj_hout, int n_adj_hout) {
   Model& m = *(Model*)h; SolverOpts so = so_of(opts), sa = so_of(adj); int nx = m.nq + m.nv, nv = m.nv;
   for (int e = e0; e < e1; ++e) {
     EnvStats st; std::vector<TapeRec> tape;
@@ -285,11 +286,13 @@ int orc_rollout_grad_adjoint(void* h, int e0, int e1, const double* x0, const do
     if (gc) for (int i = 0; i < nknot * m.nu; ++i) gc[i] = 0.0;
     if (gp) for (int i = 0; i < m.np; ++i) gp[i] = 0.0;
     bool ok = st.status == 0;
-    AdjStats as;
+    AdjStats as; std::vector<double> hsub;
     if (ok) {
       ambient_to_tangent(m, xT + (size_t)e * nx, dLdxT + (size_t)e * nx, lam.data());
-      ok = reverse_sweep_continuous(m, tape, ce, ctrl ? nknot : 0, pe, so, sa, cfd_on != 0, lam.data(), gc, gp, as);
+      ok = reverse_sweep_continuous(m, tape, ce, ctrl ? nknot : 0, pe, so, sa, cfd_on != 0, lam.data(), gc, gp, as,
+                                    adj_replay ? adj_replay + (size_t)e * n_adj_replay : nullptr, n_adj_replay, adj_hout ? &hsub : nullptr);
     }
+    if (adj_hout) for (int i = 0; i < n_adj_hout; ++i) adj_hout[(size_t)e * n_adj_hout + i] = i < (int)hsub.size() ? hsub[i] : 0.0;
     if (!ok) {
       for (auto& l : lam) l = 0.0;
       if (gc) for (int i = 0; i < nknot * m.nu; ++i) gc[i] = 0.0;

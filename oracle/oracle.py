@@ -217,7 +217,8 @@ class Oracle:
         return dict(xT=xT, stats=_stats(ist, dst), dLdx0=g0, dLdctrl=gc, dLdparams=gp)
 
 
-def _adjoint(self, x0, ctrl, nknot, knot_dt, params, horizon, opts, adj_opts, dLdxT, cfd_on=False, h_replay=None, want_params=True, threads=1):
+def _adjoint(self, x0, ctrl, nknot, knot_dt, params, horizon, opts, adj_opts, dLdxT, cfd_on=False, h_replay=None, want_params=True, threads=1,
+             adj_replay=None, n_adj_hout=0):
     """Optimize-then-discretize gradient (adjoint.hpp): forward with tape, then the continuous adjoint solved backwards
     with its own error-controlled steps under adj_opts.  Returns the fields of rollout_grad plus adj_accept / adj_reject /
     adj_status per environment."""
@@ -228,15 +229,17 @@ def _adjoint(self, x0, ctrl, nknot, knot_dt, params, horizon, opts, adj_opts, dL
     gc = np.zeros((nenv, nknot, self.nu)) if (ctrl is not None and nknot > 0) else None
     gp = np.zeros((nenv, self.np_)) if want_params else None
     o, oa = self._opts(opts), self._opts(adj_opts); nrep = 0 if h_replay is None else h_replay.shape[1]
+    adj_replay = _f8(adj_replay); narep = 0 if adj_replay is None else adj_replay.shape[1]
+    hout = np.zeros((nenv, n_adj_hout)) if n_adj_hout > 0 else None
     L = lib()
 
     def fn(e0, e1):
         L.orc_rollout_grad_adjoint(self.h, e0, e1, _p(x0), _p(ctrl), int(nknot), C.c_double(knot_dt), _p(params), C.c_double(horizon),
                                    C.byref(o), C.byref(oa), _p(h_replay), nrep, _p(dLdxT), int(cfd_on), _p(xT), _p(ist), _p(dst), _p(asub),
-                                   _p(g0), _p(gc), _p(gp))
+                                   _p(g0), _p(gc), _p(gp), _p(adj_replay), narep, _p(hout), int(n_adj_hout))
     self._run(fn, nenv, threads)
     return dict(xT=xT, stats=_stats(ist, dst), dLdx0=g0, dLdctrl=gc, dLdparams=gp, adj_accept=asub[:, 0].copy(), adj_reject=asub[:, 1].copy(),
-                adj_status=asub[:, 2].copy())
+                adj_status=asub[:, 2].copy(), adj_h=hout)
 
 
 Oracle.rollout_grad_adjoint = _adjoint

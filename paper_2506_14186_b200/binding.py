@@ -14,7 +14,7 @@ LIB_PATH = os.environ.get("DMX_LIB", os.path.join(_HERE, "libdmx.so"))
 
 SYMBOLS = ["dmx_model_create", "dmx_model_destroy", "dmx_model_set_tape_stages", "dmx_model_np", "dmx_model_nc", "dmx_model_default_params",
            "dmx_model_lanes", "dmx_tape_bytes", "dmx_tape_bytes_records", "dmx_plan_bytes", "dmx_tape_plan",
-           "dmx_rollout", "dmx_rollout_grad", "dmx_rollout_backward",
+           "dmx_rollout", "dmx_rollout_grad", "dmx_rollout_backward", "dmx_rollout_backward_adjoint", "dmx_rollout_grad_adjoint",
            "dmx_vector_field", "dmx_vjp_field", "dmx_fma_peak", "dmx_debug_counters", "dmx_last_error"]
 
 _pd, _pi = C.POINTER(C.c_double), C.POINTER(C.c_int)
@@ -77,6 +77,10 @@ def load():
         L.dmx_rollout_grad.argtypes = [vp, i, vp, vp, i, d, vp, d, C.POINTER(SolverOpts), vp, i, vp, i, vp, vp, vp, vp,
                                        C.POINTER(Stats), vp, sz, vp, vp]
         L.dmx_rollout_backward.argtypes = [vp, i, vp, i, vp, C.POINTER(SolverOpts), vp, vp, i, vp, vp, vp, C.POINTER(Stats), vp, sz, vp, vp]
+        L.dmx_rollout_backward_adjoint.argtypes = [vp, i, vp, i, vp, C.POINTER(SolverOpts), C.POINTER(SolverOpts), vp, vp, i, vp, vp, vp,
+                                                   C.POINTER(Stats), vp, vp, i, vp, sz, vp, vp]
+        L.dmx_rollout_grad_adjoint.argtypes = [vp, i, vp, vp, i, d, vp, d, C.POINTER(SolverOpts), C.POINTER(SolverOpts), vp, i, vp, i, vp, vp, vp, vp,
+                                               C.POINTER(Stats), vp, vp, i, vp, sz, vp, vp]
         L.dmx_vector_field.argtypes = [vp, i, vp, vp, vp, i, vp, vp, vp]
         L.dmx_vjp_field.argtypes = [vp, i, vp, vp, vp, vp, i, vp, vp, vp, vp, vp]
         L.dmx_fma_peak.argtypes = [i, i, _pd, _pd]
@@ -272,6 +276,52 @@ class Model:
                                      _ptr(out["dLdparams"]), C.byref(st) if st else None, _ptr(tape), tape.numel(), _ptr(plan), self._stream(stream))
         if rc != 0:
             raise RuntimeError("dmx_rollout_grad: " + _err())
+        return out
+
+    def _adj_out(self, nenv, ctrl, nknot, want_params, with_xT, like):
+        T = self.torch
+        out = dict(dLdx0=T.empty((nenv, 2 * self.nv), dtype=self.dtype, device=self.device),
+                   dLdctrl=T.empty((nenv, nknot, self.nu), dtype=self.dtype, device=self.device) if (ctrl is not None and nknot > 0) else None,
+                   dLdparams=T.empty((nenv, self.np_), dtype=self.dtype, device=self.device) if want_params else None,
+                   adj_info=T.zeros((nenv, 3), dtype=T.int32, device=self.device))
+        if with_xT:
+            out["xT"] = T.empty_like(like)
+        return out
+
+    def rollout_grad_adjoint(self, x0, ctrl, nknot, knot_dt, params, horizon, opts, adj_opts, dLdxT, cfd_on, tape, h_replay=None,
+                             want_params=True, stats=None, stream=None, plan=None, adj_replay=None):
+        """dmx_rollout_grad_adjoint: forward with tape, then the continuous adjoint solved backwards under adj_opts.
+        Returns the dict of rollout_grad plus adj_info (int32 [nenv, 3]: accepted / rejected sub-steps, status)."""
+        nenv = x0.shape[0]
+        out = self._adj_out(nenv, ctrl, nknot, want_params, True, x0)
+        st = self._stats_struct(stats)
+        o, oa = _opts(opts), _opts(adj_opts)
+        nrep = 0 if h_replay is None else h_replay.shape[1]
+        rc = load().dmx_rollout_grad_adjoint(self.h, nenv, _ptr(x0), _ptr(ctrl), int(nknot), float(knot_dt), _ptr(params), float(horizon),
+                                             C.byref(o), C.byref(oa), _ptr(h_replay), nrep, _ptr(dLdxT), int(cfd_on), _ptr(out["xT"]),
+                                             _ptr(out["dLdx0"]), _ptr(out["dLdctrl"]), _ptr(out["dLdparams"]), C.byref(st) if st else None,
+                                             _ptr(out["adj_info"]), _ptr(adj_replay), 0 if adj_replay is None else adj_replay.shape[1],
+                                             _ptr(tape), tape.numel(), _ptr(plan), self._stream(stream))
+        if rc != 0:
+            raise RuntimeError("dmx_rollout_grad_adjoint: " + _err())
+        return out
+
+    def rollout_backward_adjoint(self, ctrl, nknot, params, opts, adj_opts, xT, dLdxT, cfd_on, tape, want_params=True, stream=None, plan=None,
+                                 stats=None, adj_replay=None):
+        nenv = xT.shape[0]
+        out = self._adj_out(nenv, ctrl, nknot, want_params, False, xT)
+        o, oa = _opts(opts), _opts(adj_opts)
+        st = Stats()
+        if stats is not None and stats.get("n_newton_unconverged_bwd") is not None:
+            st.n_newton_unconverged_bwd = stats["n_newton_unconverged_bwd"].data_ptr()
+        if stats is not None and stats.get("work") is not None:
+            st.work = stats["work"].data_ptr()
+        rc = load().dmx_rollout_backward_adjoint(self.h, nenv, _ptr(ctrl), int(nknot), _ptr(params), C.byref(o), C.byref(oa), _ptr(xT), _ptr(dLdxT),
+                                                 int(cfd_on), _ptr(out["dLdx0"]), _ptr(out["dLdctrl"]), _ptr(out["dLdparams"]), C.byref(st),
+                                                 _ptr(out["adj_info"]), _ptr(adj_replay), 0 if adj_replay is None else adj_replay.shape[1],
+                                                 _ptr(tape), tape.numel(), _ptr(plan), self._stream(stream))
+        if rc != 0:
+            raise RuntimeError("dmx_rollout_backward_adjoint: " + _err())
         return out
 
     def vector_field(self, x, u=None, params=None, cfd=False, stream=None):

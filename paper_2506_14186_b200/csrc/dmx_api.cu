@@ -10,7 +10,7 @@
 #include <atomic>
 #include <stdexcept>
 #include "../../include/dmx.h"
-#include "dmx_kernels.cuh"
+#include "dmx_adjoint.cuh"
 
 using namespace dmx;
 
@@ -24,6 +24,7 @@ namespace {
 template <class R> struct Launchers {
   cudaError_t (*rollout)(const ModelDev<R>&, const RolloutArgs<R>&, LaunchCfg, cudaStream_t);
   cudaError_t (*backward)(const ModelDev<R>&, const BackwardArgs<R>&, LaunchCfg, cudaStream_t);
+  cudaError_t (*adjoint)(const ModelDev<R>&, const AdjointArgs<R>&, LaunchCfg, cudaStream_t);
   cudaError_t (*field)(const ModelDev<R>&, const FieldArgs<R>&, LaunchCfg, cudaStream_t);
   cudaError_t (*invweight)(const ModelDev<R>&, const R*, const R*, R*, const WsLayout&, const RkLayout&, LaunchCfg, cudaStream_t);
   cudaError_t (*occupancy)(int, size_t, size_t, size_t, int*, int*, int*);
@@ -31,7 +32,7 @@ template <class R> struct Launchers {
 };
 template <class R, int G, class SH> Launchers<R> make_launchers() {
   Launchers<R> l;
-  l.rollout = &launch_rollout<R, G, SH>; l.backward = &launch_backward<R, G, SH>; l.field = &launch_field<R, G, SH>;
+  l.rollout = &launch_rollout<R, G, SH>; l.backward = &launch_backward<R, G, SH>; l.adjoint = &launch_adjoint<R, G, SH>; l.field = &launch_field<R, G, SH>;
   l.invweight = &launch_invweight<R, G, SH>; l.occupancy = &kernel_occupancy<R, G, SH>; l.prof_dump = &launch_prof_dump<R, G, SH>;
   return l;
 }
@@ -246,6 +247,10 @@ void make_layouts(const HostModel& h, int G, int real_bytes, int static_ld, WsLa
   take(rl.qb, nv); take(rl.vb, nv); take(rl.dbar, nv); take(rl.Vb, nv); take(rl.lam, 2 * nv); take(rl.delta, nv);
   take(rl.qbar, nv); take(rl.vbar, nv); take(rl.ubar, std::max(h.nu, 1)); take(rl.pbar, h.np); take(rl.gp, h.np);
   rl.size_bwd = stagger(o, 8);
+  o = rl.size_bwd;
+  take(rl.ak, 14 * nv); take(rl.aub, 7 * std::max(h.nu, 1)); take(rl.apb, 7 * std::max(h.np, 1));
+  take(rl.amu, 2 * nv); take(rl.amus, 2 * nv); take(rl.amunew, 2 * nv); take(rl.az1, 2 * nv); take(rl.adz1, 2 * nv);
+  rl.size_adj = o;
   wlf = wl; rlf = rl;
   const char* ea = std::getenv("DMX_FWD_ALIAS");
   if (ea && std::atoi(ea) == 0) return;
@@ -348,7 +353,7 @@ int* next_queue(const dmx_model* m) { return m->queue + (m->qnext.fetch_add(1) %
 int alloc_scratch(dmx_model* m) {
   size_t groups = (size_t)m->cb.occ * m->sm_count * groups_per_block(m, m->cb.block);
   if (m->G == 1) groups = (groups + 31) / 32 * 32;
-  m->rk_scratch_bytes = std::max<size_t>(groups * (size_t)m->rl.size_bwd * sizeof(double), 256);
+  m->rk_scratch_bytes = std::max<size_t>(groups * (size_t)m->rl.size_adj * sizeof(double), 256);      // size_adj >= size_bwd
   CUDA_OK(cudaMalloc(&m->rk_scratch, m->rk_scratch_bytes));
   CUDA_OK(cudaEventCreateWithFlags(&m->bwd_done, cudaEventDisableTiming));
   if (m->fwd_rk_global) {
@@ -514,8 +519,10 @@ int rollout_typed(const dmx_model* m, int nenv, const void* x0, const void* ctrl
 template <class R>
 int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const void* params, const dmx_solver_opts* opts, const void* xT,
                    const void* dLdxT, int cfd_on, void* dLdx0, void* dLdctrl, void* dLdparams, const dmx_stats* st, const void* tape,
-                   size_t tape_bytes, const void* plan, cudaStream_t s) {
-  BackwardArgs<R> a; std::memset(&a, 0, sizeof(a));
+                   size_t tape_bytes, const void* plan, cudaStream_t s, const dmx_solver_opts* adj = nullptr, int* adj_info = nullptr,
+                   const double* adj_replay = nullptr, int n_adj_replay = 0) {
+  AdjointArgs<R> aa; std::memset(&aa, 0, sizeof(aa));
+  BackwardArgs<R>& a = aa.b;
   if (!tape) return fail("tape missing");
   if (bind_tape<R>(m, nenv, const_cast<void*>(tape), tape_bytes, plan, a.tp, a.pl)) return -1;
   a.nenv = nenv; a.nknot = nknot; a.want_p = dLdparams != nullptr; a.cfd = cfd_on; a.tape_stages = m->tape_stages;
@@ -533,7 +540,10 @@ int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const vo
   CUDA_OK(cudaMemsetAsync(a.queue, 0, sizeof(int), s));
   if (dLdctrl && nknot > 0 && m->h.nu > 0) CUDA_OK(cudaMemsetAsync(dLdctrl, 0, (size_t)nenv * nknot * m->h.nu * sizeof(R), s));
   ModelDev<R> md = dev_of<R>(m); md.arena_smem = m->cb.arena;
-  CUDA_OK(launchers_for<R>(m->G, m->shape).backward(md, a, c, s));
+  if (adj) {                       // optimize-then-discretize: same arguments plus the options of the backward solve
+    aa.sa = opts_of(adj); aa.info = adj_info; aa.replay = adj_replay; aa.n_replay = adj_replay ? n_adj_replay : 0;
+    CUDA_OK(launchers_for<R>(m->G, m->shape).adjoint(md, aa, c, s));
+  } else CUDA_OK(launchers_for<R>(m->G, m->shape).backward(md, a, c, s));
   CUDA_OK(cudaEventRecord(m->bwd_done, s));
   return 0;
 }
@@ -718,6 +728,39 @@ int dmx_rollout_grad(const dmx_model* m, int nenv, const void* x0, const void* c
   dmx_stats bs; std::memset(&bs, 0, sizeof(bs));            // failed environments are marked in the tape header; only the counter is passed on
   if (stats) { bs.n_newton_unconverged_bwd = stats->n_newton_unconverged_bwd; bs.work = stats->work; }
   return dmx_rollout_backward(m, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, &bs, tape, tape_bytes, plan, cuda_stream);
+}
+
+static int check_adj(const dmx_solver_opts* o) {
+  if (!o) return fail("null adjoint options");
+  if (o->tableau != DMX_DOPRI5 && o->tableau != DMX_TSIT5) return fail("unknown tableau");
+  if (!(o->rtol >= 0) || !(o->atol >= 0) || !(o->rtol + o->atol > 0) || o->max_steps <= 0) return fail("bad adjoint tolerances / budget");
+  return 0;
+}
+
+int dmx_rollout_backward_adjoint(const dmx_model* m, int nenv, const void* ctrl, int nknot, const void* params, const dmx_solver_opts* opts,
+                                 const dmx_solver_opts* adj_opts, const void* xT, const void* dLdxT, int cfd_on, void* dLdx0, void* dLdctrl,
+                                 void* dLdparams, const dmx_stats* stats, int* adj_info, const double* adj_replay, int n_adj_replay, const void* tape,
+                                 size_t tape_bytes, const void* plan, void* cuda_stream) {
+  if (!m || nenv <= 0 || !opts || !xT || !dLdxT || !dLdx0) return fail("null argument");
+  if (check_adj(adj_opts)) return -1;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  dmx_model* mm = const_cast<dmx_model*>(m);
+  return m->precision == 64 ? backward_typed<double>(mm, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, stats, tape, tape_bytes, plan, s, adj_opts, adj_info, adj_replay, n_adj_replay)
+                            : backward_typed<float>(mm, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, stats, tape, tape_bytes, plan, s, adj_opts, adj_info, adj_replay, n_adj_replay);
+}
+
+int dmx_rollout_grad_adjoint(const dmx_model* m, int nenv, const void* x0, const void* ctrl, int nknot, double knot_dt, const void* params, double horizon,
+                             const dmx_solver_opts* opts, const dmx_solver_opts* adj_opts, const double* h_replay, int n_replay, const void* dLdxT,
+                             int cfd_on, void* xT, void* dLdx0, void* dLdctrl, void* dLdparams, const dmx_stats* stats, int* adj_info,
+                             const double* adj_replay, int n_adj_replay, void* tape, size_t tape_bytes, const void* plan, void* cuda_stream) {
+  if (!tape) return fail("dmx_rollout_grad_adjoint needs a tape");
+  if (check_adj(adj_opts)) return -1;
+  int rc = dmx_rollout(m, nenv, x0, ctrl, nknot, knot_dt, params, horizon, opts, h_replay, n_replay, xT, stats, tape, tape_bytes, plan, cuda_stream);
+  if (rc) return rc;
+  dmx_stats bs; std::memset(&bs, 0, sizeof(bs));
+  if (stats) { bs.n_newton_unconverged_bwd = stats->n_newton_unconverged_bwd; bs.work = stats->work; }
+  return dmx_rollout_backward_adjoint(m, nenv, ctrl, nknot, params, opts, adj_opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, &bs, adj_info,
+                                      adj_replay, n_adj_replay, tape, tape_bytes, plan, cuda_stream);
 }
 
 int dmx_vector_field(const dmx_model* m, int n, const void* x, const void* u, const void* params, int cfd, void* acc, int* nrow, void* cuda_stream) {

@@ -1,7 +1,7 @@
 // dmx_inst.cuh — launcher definitions; each inst_*.cu instantiates them for one (real type, lanes)
 // pair so that the translation units compile in parallel.
 #pragma once
-#include "dmx_kernels.cuh"
+#include "dmx_adjoint.cuh"
 
 namespace dmx {
 
@@ -15,6 +15,12 @@ template <class R, int G, class SH> cudaError_t launch_backward(const ModelDev<R
   cudaError_t e = cudaFuncSetAttribute(backward_kernel<R, G, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
   if (e != cudaSuccess) return e;
   backward_kernel<R, G, SH><<<c.grid, c.block, c.smem, s>>>(m, a);
+  return cudaGetLastError();
+}
+template <class R, int G, class SH> cudaError_t launch_adjoint(const ModelDev<R>& m, const AdjointArgs<R>& a, LaunchCfg c, cudaStream_t s) {
+  cudaError_t e = cudaFuncSetAttribute(adjoint_kernel<R, G, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+  if (e != cudaSuccess) return e;
+  adjoint_kernel<R, G, SH><<<c.grid, c.block, c.smem, s>>>(m, a);
   return cudaGetLastError();
 }
 template <class R, int G, class SH> cudaError_t launch_field(const ModelDev<R>& m, const FieldArgs<R>& a, LaunchCfg c, cudaStream_t s) {
@@ -53,6 +59,7 @@ template <class R, int G, class SH> cudaError_t kernel_occupancy(int block, size
 #define DMX_INSTANTIATE(R, G, SH)                                                                                                  \
   template cudaError_t dmx::launch_rollout<R, G, dmx::SH>(const dmx::ModelDev<R>&, const dmx::RolloutArgs<R>&, dmx::LaunchCfg, cudaStream_t);   \
   template cudaError_t dmx::launch_backward<R, G, dmx::SH>(const dmx::ModelDev<R>&, const dmx::BackwardArgs<R>&, dmx::LaunchCfg, cudaStream_t); \
+  template cudaError_t dmx::launch_adjoint<R, G, dmx::SH>(const dmx::ModelDev<R>&, const dmx::AdjointArgs<R>&, dmx::LaunchCfg, cudaStream_t); \
   template cudaError_t dmx::launch_field<R, G, dmx::SH>(const dmx::ModelDev<R>&, const dmx::FieldArgs<R>&, dmx::LaunchCfg, cudaStream_t);       \
   template cudaError_t dmx::launch_invweight<R, G, dmx::SH>(const dmx::ModelDev<R>&, const R*, const R*, R*, const dmx::WsLayout&,             \
                                                             const dmx::RkLayout&, dmx::LaunchCfg, cudaStream_t);                             \

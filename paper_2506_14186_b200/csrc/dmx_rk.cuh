@@ -112,6 +112,9 @@ struct RkLayout {
   int Kb, Ab, qb, vb, dbar, Vb, lam, delta, qbar, vbar, ubar, pbar, gp;
   int size_fwd, size_bwd;
   int Yqr, Vr, rsize;                        // stage inputs in the real type R
+  // continuous adjoint (adjoint_kernel): stage rates of the backward solve k[7][2nv], their control / parameter parts,
+  // the adjoint in chart coordinates (current, stage, proposal) and the Hermite end data of the forward step
+  int ak, aub, apb, amu, amus, amunew, az1, adz1, size_adj;
 };
 #define DMX_RK_ARR(name) DMX_DI Arr<double, ST> name() const { return Arr<double, ST>(b + L->name * ST); }
 template <int ST_> struct Rk {
@@ -120,6 +123,7 @@ template <int ST_> struct Rk {
   DMX_RK_ARR(q) DMX_RK_ARR(v) DMX_RK_ARR(Yq) DMX_RK_ARR(V) DMX_RK_ARR(Dl) DMX_RK_ARR(K) DMX_RK_ARR(A) DMX_RK_ARR(err)
   DMX_RK_ARR(sYq) DMX_RK_ARR(sV) DMX_RK_ARR(sDl) DMX_RK_ARR(Kb) DMX_RK_ARR(Ab) DMX_RK_ARR(qb) DMX_RK_ARR(vb) DMX_RK_ARR(dbar)
   DMX_RK_ARR(Vb) DMX_RK_ARR(lam) DMX_RK_ARR(delta) DMX_RK_ARR(qbar) DMX_RK_ARR(vbar) DMX_RK_ARR(ubar) DMX_RK_ARR(pbar) DMX_RK_ARR(gp)
+  DMX_RK_ARR(ak) DMX_RK_ARR(aub) DMX_RK_ARR(apb) DMX_RK_ARR(amu) DMX_RK_ARR(amus) DMX_RK_ARR(amunew) DMX_RK_ARR(az1) DMX_RK_ARR(adz1)
 };
 // stride of the cooperative workspaces: contiguous per group, warp-interleaved for one-lane groups
 template <int G> struct StrideOf { static const int value = (G == 1) ? 32 : 1; };
