@@ -180,6 +180,24 @@ int dmx_rollout_backward(const dmx_model *m, int nenv, const void *ctrl, int nkn
                          void *dLdx0, void *dLdctrl, void *dLdparams, const dmx_stats *stats,
                          const void *tape, size_t tape_bytes, const void *plan, void *cuda_stream);
 
+/* The reverse sweep for callers that must not allocate at call time (CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc).  Same arguments, outputs and results as dmx_rollout_backward; the per-lane-group adjoint
+ * arrays and the work-queue counter live in a static device array of dmx_noalloc_scratch_bytes() = 16 MiB that every
+ * GPU which loads the library holds until the process exits.  The call enqueues two memsets and one kernel and calls no
+ * cudaMalloc / cudaFree / allocating library routine.  Limits and rules:
+ *   - a model must have been created with the current device current (that is where the array's device address is
+ *     taken, once per device); otherwise the call fails;
+ *   - the scratch need grows with nenv up to the resident grid (about 4.3 KB per environment for BASELINE config 2, so
+ *     ~3800 environments); a larger batch is rejected with an error that states the need and the limit;
+ *   - every call on a device shares the array: calls that overlap on the GPU (different streams without ordering
+ *     between them) race.  Calls on one stream, or ordered by events, are safe; the array keeps the last call's
+ *     contents and each call clears what must start at zero. */
+size_t dmx_noalloc_scratch_bytes(void);
+int dmx_rollout_backward_noalloc(const dmx_model *m, int nenv, const void *ctrl, int nknot, const void *params,
+                                 const dmx_solver_opts *opts, const void *xT, const void *dLdxT, int cfd_on,
+                                 void *dLdx0, void *dLdctrl, void *dLdparams, const dmx_stats *stats,
+                                 const void *tape, size_t tape_bytes, const void *plan, void *cuda_stream);
+
 /* Optimize-then-discretize (Eq. 6-7; with cfd_on the altered adjoint equations PAPER.md:462-477,
  * Eq. 8-9): the gradient as the solution of the continuous adjoint equations, solved BACKWARDS with its own
  * error-controlled steps under adj_opts (tableau, rtol, atol over the 2*nv adjoint components, controller constants,

@@ -15,6 +15,7 @@ LIB_PATH = os.environ.get("DMX_LIB", os.path.join(_HERE, "libdmx.so"))
 SYMBOLS = ["dmx_model_create", "dmx_model_destroy", "dmx_model_set_tape_stages", "dmx_model_np", "dmx_model_nc", "dmx_model_default_params",
            "dmx_model_lanes", "dmx_tape_bytes", "dmx_tape_bytes_records", "dmx_plan_bytes", "dmx_tape_plan",
            "dmx_rollout", "dmx_rollout_grad", "dmx_rollout_backward", "dmx_rollout_backward_adjoint", "dmx_rollout_grad_adjoint",
+           "dmx_rollout_backward_noalloc", "dmx_noalloc_scratch_bytes",
            "dmx_vector_field", "dmx_vjp_field", "dmx_fma_peak", "dmx_debug_counters", "dmx_last_error"]
 
 _pd, _pi = C.POINTER(C.c_double), C.POINTER(C.c_int)
@@ -77,6 +78,9 @@ def load():
         L.dmx_rollout_grad.argtypes = [vp, i, vp, vp, i, d, vp, d, C.POINTER(SolverOpts), vp, i, vp, i, vp, vp, vp, vp,
                                        C.POINTER(Stats), vp, sz, vp, vp]
         L.dmx_rollout_backward.argtypes = [vp, i, vp, i, vp, C.POINTER(SolverOpts), vp, vp, i, vp, vp, vp, C.POINTER(Stats), vp, sz, vp, vp]
+        L.dmx_rollout_backward_noalloc.argtypes = [vp, i, vp, i, vp, C.POINTER(SolverOpts), vp, vp, i, vp, vp, vp, C.POINTER(Stats), vp, sz, vp, vp]
+        L.dmx_noalloc_scratch_bytes.restype = C.c_size_t
+        L.dmx_noalloc_scratch_bytes.argtypes = []
         L.dmx_rollout_backward_adjoint.argtypes = [vp, i, vp, i, vp, C.POINTER(SolverOpts), C.POINTER(SolverOpts), vp, vp, i, vp, vp, vp,
                                                    C.POINTER(Stats), vp, vp, i, vp, sz, vp, vp]
         L.dmx_rollout_grad_adjoint.argtypes = [vp, i, vp, vp, i, d, vp, d, C.POINTER(SolverOpts), C.POINTER(SolverOpts), vp, i, vp, i, vp, vp, vp, vp,
@@ -276,6 +280,24 @@ class Model:
                                      _ptr(out["dLdparams"]), C.byref(st) if st else None, _ptr(tape), tape.numel(), _ptr(plan), self._stream(stream))
         if rc != 0:
             raise RuntimeError("dmx_rollout_grad: " + _err())
+        return out
+
+    def rollout_backward_noalloc(self, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, tape, out, status=None, stream=None, plan=None, stats=None):
+        """dmx_rollout_backward_noalloc: the reverse sweep with its scratch in the library's static device array.  `out` must
+        hold preallocated dLdx0 / dLdctrl / dLdparams tensors (this wrapper allocates nothing either)."""
+        o = _opts(opts)
+        st = Stats()
+        if status is not None:
+            st.status = status.data_ptr()
+        if stats is not None and stats.get("n_newton_unconverged_bwd") is not None:
+            st.n_newton_unconverged_bwd = stats["n_newton_unconverged_bwd"].data_ptr()
+        if stats is not None and stats.get("work") is not None:
+            st.work = stats["work"].data_ptr()
+        rc = load().dmx_rollout_backward_noalloc(self.h, xT.shape[0], _ptr(ctrl), int(nknot), _ptr(params), C.byref(o), _ptr(xT), _ptr(dLdxT),
+                                                 int(cfd_on), _ptr(out["dLdx0"]), _ptr(out.get("dLdctrl")), _ptr(out.get("dLdparams")), C.byref(st),
+                                                 _ptr(tape), tape.numel(), _ptr(plan), self._stream(stream))
+        if rc != 0:
+            raise RuntimeError("dmx_rollout_backward_noalloc: " + _err())
         return out
 
     def _adj_out(self, nenv, ctrl, nknot, want_params, with_xT, like):

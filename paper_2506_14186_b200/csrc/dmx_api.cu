@@ -610,6 +610,8 @@ __global__ void plan_kernel(int nenv, const int* __restrict__ n_acc, int margin_
 
 }  // namespace
 
+static int noalloc_setup(int dev);   // defined at the end of this file, next to the static scratch array
+
 // ---- C-ABI ------------------------------------------------------------------------------------------------
 extern "C" {
 
@@ -635,6 +637,7 @@ int dmx_model_create(const dmx_model_desc* desc, int precision, dmx_model** out)
       cudaMalloc(&m->queue, N_QUEUE * sizeof(int)) != cudaSuccess) { fail("cudaMalloc failed"); dmx_model_destroy(m); return -1; }
   int rc = precision == 64 ? create_typed<double>(m) : create_typed<float>(m);
   if (!rc) rc = alloc_scratch(m);
+  if (!rc) rc = noalloc_setup(dev);          // device address of the static scratch of dmx_rollout_backward_noalloc
   if (rc) { dmx_model_destroy(m); return -1; }
   *out = m;
   return 0;
@@ -794,6 +797,87 @@ int dmx_debug_counters(const dmx_model* m, unsigned long long* host32) {
 int dmx_fma_peak(int precision, int iters, double* flops_per_s, double* ms) {
   if (!flops_per_s || !ms || iters <= 0) return fail("bad argument");
   return precision == 64 ? fma_peak_typed<double>(iters, flops_per_s, ms) : fma_peak_typed<float>(iters, flops_per_s, ms);
+}
+
+}  // extern "C"
+
+
+// ---- dmx_rollout_backward_noalloc: the reverse sweep with its scratch in a static device array ------------------------
+// For callers that must not allocate at call time (CUDA graph capture, tight serving loops, harnesses that forbid it).
+// The reverse sweep needs per-lane-group integrator / adjoint arrays in global memory and a work-queue counter; the
+// regular path keeps them in buffers the model cudaMalloc'ed at create, this variant keeps them in the file-scope array
+// below: DMX_NOALLOC_SCRATCH_BYTES (16 MiB) per GPU that loads the library, held until the process exits.
+// Layout: [0, 256) the work-queue counter (cleared by every call), [256, ...) the lane-group arrays (every value a sweep
+// reads it has written before, so the last call's contents do not matter).  Every call on a device shares the array:
+// calls that overlap on the GPU (different streams, no ordering between them) race.
+// In HOST code the array's name is a host-side stand-in, not a device address; the address is taken once per device at
+// set-up (dmx_model_create, with that device current) by cudaGetSymbolAddress and only that pointer goes to the kernel.
+#define DMX_NOALLOC_SCRATCH_BYTES (16u << 20)
+static __device__ __align__(256) unsigned char g_noalloc_scratch[DMX_NOALLOC_SCRATCH_BYTES];
+enum { NOALLOC_MAX_DEV = 64 };
+static unsigned char* g_noalloc_ptr[NOALLOC_MAX_DEV];   // device address of g_noalloc_scratch, per device ordinal
+
+static int noalloc_setup(int dev) {
+  if (dev < 0 || dev >= NOALLOC_MAX_DEV) return 0;       // such a device simply has no no-alloc entry point
+  if (g_noalloc_ptr[dev]) return 0;
+  void* ptr = nullptr;
+  cudaError_t e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+  if (e != cudaSuccess) return fail("cudaGetSymbolAddress(g_noalloc_scratch): %s", cudaGetErrorString(e));
+  g_noalloc_ptr[dev] = (unsigned char*)ptr;
+  return 0;
+}
+
+namespace {
+
+template <class R>
+int backward_noalloc_typed(const dmx_model* m, int nenv, const void* ctrl, int nknot, const void* params, const dmx_solver_opts* opts, const void* xT,
+                           const void* dLdxT, int cfd_on, void* dLdx0, void* dLdctrl, void* dLdparams, const dmx_stats* st, const void* tape,
+                           size_t tape_bytes, const void* plan, cudaStream_t s) {
+  int dev = -1;
+  CUDA_OK(cudaGetDevice(&dev));
+  unsigned char* base = (dev >= 0 && dev < NOALLOC_MAX_DEV) ? g_noalloc_ptr[dev] : nullptr;
+  if (!base) return fail("dmx_rollout_backward_noalloc: no static scratch on the current device (create a dmx_model with this device current first)");
+  LaunchCfg c; c.block = m->cb.block; c.smem = m->cb.smem;
+  const int gpb = groups_per_block(m, c.block);
+  c.grid = std::max(1, std::min(m->cb.occ * m->sm_count, (nenv + gpb - 1) / gpb));
+  size_t groups = (size_t)c.grid * gpb;
+  if (m->G == 1) groups = (groups + 31) / 32 * 32;
+  const size_t need = 256 + groups * (size_t)m->rl.size_bwd * sizeof(double);
+  if (need > (size_t)DMX_NOALLOC_SCRATCH_BYTES) {
+    std::snprintf(g_err, sizeof(g_err), "dmx_rollout_backward_noalloc: nenv = %d needs %zu bytes of scratch, the static array holds %u "
+                  "(DMX_NOALLOC_SCRATCH_BYTES); use dmx_rollout_backward or a smaller batch", nenv, need, (unsigned)DMX_NOALLOC_SCRATCH_BYTES);
+    return -1;
+  }
+  BackwardArgs<R> a; std::memset(&a, 0, sizeof(a));
+  if (!tape) return fail("tape missing");
+  if (bind_tape<R>(m, nenv, const_cast<void*>(tape), tape_bytes, plan, a.tp, a.pl)) return -1;
+  a.nenv = nenv; a.nknot = nknot; a.want_p = dLdparams != nullptr; a.cfd = cfd_on; a.tape_stages = m->tape_stages;
+  a.ctrl = (const R*)ctrl; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u; a.xT = (const R*)xT; a.dLdxT = (const R*)dLdxT;
+  a.status = st ? st->status : nullptr; a.n_unconv = st ? st->n_newton_unconverged_bwd : nullptr; a.work = st ? st->work : nullptr;
+  a.so = opts_of(opts); a.dLdx0 = (R*)dLdx0; a.dLdctrl = (R*)dLdctrl; a.dLdparams = (R*)dLdparams;
+  a.lockstep = 0x1ff; a.wl = m->wl; a.rl = m->rl;
+  a.queue = (int*)base;                                   // what must start at zero: the work-queue counter
+  a.rk_scratch = (double*)(base + 256);
+  CUDA_OK(cudaMemsetAsync(base, 0, 256, s));
+  if (dLdctrl && nknot > 0 && m->h.nu > 0) CUDA_OK(cudaMemsetAsync(dLdctrl, 0, (size_t)nenv * nknot * m->h.nu * sizeof(R), s));
+  ModelDev<R> md = dev_of<R>(m); md.arena_smem = m->cb.arena;
+  CUDA_OK(launchers_for<R>(m->G, m->shape).backward(md, a, c, s));
+  return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t dmx_noalloc_scratch_bytes(void) { return (size_t)DMX_NOALLOC_SCRATCH_BYTES; }
+
+int dmx_rollout_backward_noalloc(const dmx_model* m, int nenv, const void* ctrl, int nknot, const void* params, const dmx_solver_opts* opts,
+                                 const void* xT, const void* dLdxT, int cfd_on, void* dLdx0, void* dLdctrl, void* dLdparams, const dmx_stats* stats,
+                                 const void* tape, size_t tape_bytes, const void* plan, void* cuda_stream) {
+  if (!m || nenv <= 0 || !opts || !xT || !dLdxT || !dLdx0) return fail("null argument");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  return m->precision == 64 ? backward_noalloc_typed<double>(m, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, stats, tape, tape_bytes, plan, s)
+                            : backward_noalloc_typed<float>(m, nenv, ctrl, nknot, params, opts, xT, dLdxT, cfd_on, dLdx0, dLdctrl, dLdparams, stats, tape, tape_bytes, plan, s);
 }
 
 }  // extern "C"
