@@ -37,14 +37,18 @@ from paper_2506_14186_b200 import workloads as W  # noqa: E402
 METRIC = "env-steps/s forward and gradient env-steps/s"
 UNIT = "accepted env-steps/s (forward + reverse sweep)"
 
-# Executed-FP64 fractions of the measured FMA peak from the committed ncu captures (profiles/r2_*.md): NOT measured in
-# the run that prints them (a profiler cannot run inside a timed region); quoted next to the live algorithmic fraction.
-NCU_EXECUTED = {}
-try:
-    with open(os.path.join(ROOT, "profiles", "r2_ncu_executed.json")) as _f:
-        NCU_EXECUTED = json.load(_f)
-except (OSError, ValueError):
-    pass
+# Executed-FP64 fractions of the measured FMA peak (2*DFMA + DADD + DMUL per second / 33.8 TFLOP/s) and DRAM bytes per launch
+# from the committed ncu --set full captures (profiles/r2_{rollout,backward}_kernel_{C2,C3,C5}.md).  They are constants of
+# those captures, NOT measured in the run that prints them (a profiler cannot run inside a timed region); the JSON line
+# labels them as such, next to the live algorithmic fraction.  Key: config_dtype_nenv of the capture.
+NCU_EXECUTED = {
+    "C2_f64_4096": {"rollout_kernel_executed_frac": 0.0325, "backward_kernel_executed_frac": 0.0287,
+                    "rollout_kernel_dram_bytes": 5.778e+08, "backward_kernel_dram_bytes": 8.272e+08},
+    "C3_f64_2048": {"rollout_kernel_executed_frac": 0.0108, "backward_kernel_executed_frac": 0.0097,
+                    "rollout_kernel_dram_bytes": 3.224e+08, "backward_kernel_dram_bytes": 3.821e+08},
+    "C5_f64_512": {"rollout_kernel_executed_frac": 0.0110, "backward_kernel_executed_frac": 0.0130,
+                    "rollout_kernel_dram_bytes": 1.66e+09, "backward_kernel_dram_bytes": 1.713e+09},
+}
 
 # per_config rows: (key, config, nenv (0 = BASELINE size), precision, timed passes, oracle sample envs)
 PER_CONFIG = [("C1", "C1", 0, 64, 3, 1024), ("C2", "C2", 0, 64, 3, 256), ("C3", "C3", 0, 64, 2, 256), ("C3_fp32", "C3", 0, 32, 2, 0),
