@@ -50,10 +50,12 @@ NCU_EXECUTED = {
                     "rollout_kernel_dram_bytes": 1.66e+09, "backward_kernel_dram_bytes": 1.713e+09},
 }
 
-# per_config rows: (key, config, nenv (0 = BASELINE size), precision, timed passes, oracle sample envs)
-PER_CONFIG = [("C1", "C1", 0, 64, 3, 1024), ("C2", "C2", 0, 64, 3, 256), ("C3", "C3", 0, 64, 2, 256), ("C3_fp32", "C3", 0, 32, 2, 0),
-              ("C4", "C4", 0, 64, 1, 16), ("C5", "C5", 0, 64, 2, 16),
-              ("C1_saturating_65536", "C1", 65536, 64, 2, 0), ("C2_saturating_32768", "C2", 32768, 64, 2, 0)]
+# per_config rows: (key, config, nenv (0 = BASELINE size), precision, timed passes, oracle sample envs, checkpoint stride)
+PER_CONFIG = [("C1", "C1", 0, 64, 3, 1024, 1), ("C2", "C2", 0, 64, 3, 256, 1), ("C3", "C3", 0, 64, 2, 256, 1), ("C3_fp32", "C3", 0, 32, 2, 0, 1),
+              ("C4", "C4", 0, 64, 1, 16, 1), ("C5", "C5", 0, 64, 2, 16, 1),
+              ("C1_saturating_65536", "C1", 65536, 64, 2, 0, 1), ("C2_saturating_32768", "C2", 32768, 64, 2, 0, 1),
+              # the checkpoint-count knob: a checkpoint every 16 accepted steps, segments recomputed in the sweep
+              ("C3_checkpoint_stride16", "C3", 0, 64, 1, 0, 16), ("C4_checkpoint_stride16", "C4", 0, 64, 1, 0, 16)]
 
 
 # ---- algorithmic FP64 work: analytic flop counts of the operations the method defines, FMA = 2, times
@@ -211,9 +213,11 @@ def run_reference(args, rank, world):
 class Runner:
     """One workload on one device: sizing pass, plan, tape, and the timed pass."""
 
-    def __init__(self, torch, B, dev, cfg, w, precision, cfd):
-        self.torch, self.cfg, self.w, self.cfd, self.dev = torch, cfg, w, cfd, dev
+    def __init__(self, torch, B, dev, cfg, w, precision, cfd, stride=1):
+        self.torch, self.cfg, self.w, self.cfd, self.dev, self.stride = torch, cfg, w, cfd, dev, stride
         self.m = m = B.Model(w["model"], precision=precision, device=dev)
+        if stride > 1:
+            m.set_checkpoint_stride(stride)
         self.nenv = w["nenv"]
         np_dt = np.float64 if precision == 64 else np.float32
         self.x0_h = torch.from_numpy(np.ascontiguousarray(w["x0"], dtype=np_dt)).pin_memory()
@@ -282,6 +286,7 @@ class Runner:
         na = st["n_accept"]
         return {
             "workload": w["name"], "nenv": self.nenv, "dtype": "f64" if m.precision == 64 else "f32", "lanes_per_env": m.lanes,
+            "checkpoint_stride": self.stride,
             "cfd_backward": bool(self.cfd), "param_grads": bool(self.want_p),
             "ms_forward": 1e3 * t_f, "ms_backward": 1e3 * t_b, "ms_step": 1e3 * t_s,
             "forward_env_steps_per_s": acc / t_f, "forward_attempted_steps_per_s": (acc + rej) / t_f, "backward_env_steps_per_s": acc / t_b,
@@ -314,6 +319,7 @@ def main():
     ap.add_argument("--no-per-config", action="store_true")
     ap.add_argument("--per-config", default="", help="comma-separated subset of per_config keys")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
+    ap.add_argument("--checkpoint-stride", type=int, default=1, help="tape keeps every k-th accepted step; segments recomputed in the sweep")
     args = ap.parse_args()
     rank, world, local = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1)), int(os.environ.get("LOCAL_RANK", 0))
     if args.impl == "reference":
@@ -335,7 +341,7 @@ def main():
     strong = args.scaling == "strong"
     w = make_workload(cfg, args.nenv, rank, world, strong)
     cfd = w["cfd"] and not args.no_cfd
-    run = Runner(torch, B, dev, cfg, w, args.precision, cfd)
+    run = Runner(torch, B, dev, cfg, w, args.precision, cfd, args.checkpoint_stride)
     m, nenv = run.m, run.nenv
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
     stream = run.stream
@@ -400,7 +406,8 @@ def main():
         "config": {"workload": w["name"], "nenv_per_gpu": nenv, "horizon_s": w["horizon"], "rtol": w["opts"]["rtol"], "cfd_backward": bool(cfd),
                    "lanes_per_env": m.lanes, "l2": "flushed between timed iterations (256 MiB write)",
                    "tape": "planned slots (dmx_tape_plan from a sizing pass, 25 %% + 16 records margin), %d B" % run.tape.numel(),
-                   "tape_record": "checkpoint + 6 stage rates", "param_grads": bool(run.want_p),
+                   "tape_record": "checkpoint + 6 stage rates" if args.checkpoint_stride == 1 else "checkpoint + first-stage rate every %d steps, 8-byte step schedule" % args.checkpoint_stride,
+                   "param_grads": bool(run.want_p),
                    "headline": "C2 is the timed headline; the largest single-GPU config C4 (16384 envs) takes seconds per pass and is measured in "
                                "per_config with its own repeat count (1 warm-up + the stated timed passes)"},
         "forward_env_steps_per_s": head["forward_env_steps_per_s"], "forward_attempted_steps_per_s": head["forward_attempted_steps_per_s"],
@@ -430,13 +437,13 @@ def main():
         per = {}
         del run
         torch.cuda.empty_cache()
-        for key_, c, n, prec, reps, n_orc in PER_CONFIG:
+        for key_, c, n, prec, reps, n_orc, stride_ in PER_CONFIG:
             if want and key_ not in want:
                 continue
             try:
                 wc = make_workload(c, n, 0)
-                rc = Runner(torch, B, dev, c, wc, prec, wc["cfd"])
-                warm = 0 if key_ == "C4" else 1          # C4: the sizing pass is the only warm-up (a pass takes minutes)
+                rc = Runner(torch, B, dev, c, wc, prec, wc["cfd"], stride_)
+                warm = 0 if c == "C4" else 1             # C4: the sizing pass is the only warm-up (a pass takes a minute)
                 tf_, tb_, ts_ = rc.timed(flush, warm, reps)
                 ent = rc.summary(tf_, tb_, ts_, peak64 if prec == 64 else peak32)
                 ent["timed_passes"] = reps; ent["warmup_passes"] = warm

@@ -121,6 +121,17 @@ int dmx_model_lanes(const dmx_model *m);
  * the reverse sweep recomputes the stages with six F evaluations per step.  Set before sizing / writing a tape. */
 int dmx_model_set_tape_stages(dmx_model *m, int on);
 
+/* Checkpoint count knob (PAPER.md:371-375 "memory = number of checkpoints x size of the ODE state", :431 checkpointing
+ * trades memory for recomputation).  k = 1 (default): one record per accepted step.  k > 1: the tape keeps a full
+ * checkpoint (y_n, t_n, h_n and the first-stage rate) only for the accepted steps 0, k, 2k, ... and, for every step, its signed
+ * step size (8 bytes); the reverse sweep re-runs each segment of k steps forward from its checkpoint (same stages, same
+ * FSAL rule and step sizes, hence the same states) into a buffer of k full records per resident lane group and sweeps
+ * that.  Memory per environment goes from N records to N/k records + 8N bytes (+ k records of scratch per resident
+ * group); the sweep costs one extra forward pass.  Gradients equal those of k = 1.  Set before sizing / writing a tape;
+ * the call synchronises the device and (re)allocates the segment buffers.  dmx_rollout_*_adjoint and
+ * dmx_rollout_backward_noalloc need k = 1. */
+int dmx_model_set_checkpoint_stride(dmx_model *m, int k);
+
 /* Bytes of tape for nenv environments with room for tape_steps accepted steps each (uniform slots; no plan). */
 size_t dmx_tape_bytes(const dmx_model *m, int nenv, int tape_steps);
 

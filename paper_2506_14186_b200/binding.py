@@ -12,7 +12,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("DMX_LIB", os.path.join(_HERE, "libdmx.so"))
 
-SYMBOLS = ["dmx_model_create", "dmx_model_destroy", "dmx_model_set_tape_stages", "dmx_model_np", "dmx_model_nc", "dmx_model_default_params",
+SYMBOLS = ["dmx_model_create", "dmx_model_destroy", "dmx_model_set_tape_stages", "dmx_model_set_checkpoint_stride", "dmx_model_np", "dmx_model_nc", "dmx_model_default_params",
            "dmx_model_lanes", "dmx_tape_bytes", "dmx_tape_bytes_records", "dmx_plan_bytes", "dmx_tape_plan",
            "dmx_rollout", "dmx_rollout_grad", "dmx_rollout_backward", "dmx_rollout_backward_adjoint", "dmx_rollout_grad_adjoint",
            "dmx_rollout_backward_noalloc", "dmx_noalloc_scratch_bytes",
@@ -73,6 +73,7 @@ def load():
             getattr(L, f).argtypes = [C.c_void_p]
         L.dmx_model_default_params.argtypes = [C.c_void_p, C.c_void_p]
         L.dmx_model_set_tape_stages.argtypes = [C.c_void_p, C.c_int]
+        L.dmx_model_set_checkpoint_stride.argtypes = [C.c_void_p, C.c_int]
         vp, i, d, sz = C.c_void_p, C.c_int, C.c_double, C.c_size_t
         L.dmx_rollout.argtypes = [vp, i, vp, vp, i, d, vp, d, C.POINTER(SolverOpts), vp, i, vp, C.POINTER(Stats), vp, sz, vp, vp]
         L.dmx_rollout_grad.argtypes = [vp, i, vp, vp, i, d, vp, d, C.POINTER(SolverOpts), vp, i, vp, i, vp, vp, vp, vp,
@@ -163,6 +164,12 @@ class Model:
         """1 (default): tape also holds the stage rates, no recomputation in the reverse sweep; 0: checkpoints only."""
         if load().dmx_model_set_tape_stages(self.h, int(bool(on))) != 0:
             raise RuntimeError("dmx_model_set_tape_stages: " + _err())
+
+    def set_checkpoint_stride(self, k):
+        """1 (default): a tape record per accepted step; k > 1: a checkpoint every k steps + the step schedule, segments
+        recomputed in the reverse sweep (dmx.h)."""
+        if load().dmx_model_set_checkpoint_stride(self.h, int(k)) != 0:
+            raise RuntimeError("dmx_model_set_checkpoint_stride: " + _err())
 
     def default_params(self):
         p = np.zeros(self.np_)

@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(256) adjoint_kernel(const __grid_constant__ Mo
   const int nknot = has_ctrl ? a.nknot : 0;
   const SolverOpts& sa = aa.sa;
   const bool tape_ok = a.tp.meta[0] == TAPE_MAGIC && a.tp.meta[1] == a.nenv && a.tp.meta[2] == rec && a.tp.meta[3] == a.tp.o_A &&
-                       a.tp.meta[4] == (a.pl.offset ? 1 : 0);
+                       a.tp.meta[4] == (a.pl.offset ? 1 : 0) && a.tp.meta[5] == 1 && a.tp.stride == 1;
 #pragma unroll 1
   for (;;) {
     int e = 0;

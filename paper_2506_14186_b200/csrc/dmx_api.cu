@@ -24,6 +24,7 @@ namespace {
 template <class R> struct Launchers {
   cudaError_t (*rollout)(const ModelDev<R>&, const RolloutArgs<R>&, LaunchCfg, cudaStream_t);
   cudaError_t (*backward)(const ModelDev<R>&, const BackwardArgs<R>&, LaunchCfg, cudaStream_t);
+  cudaError_t (*backward_ckpt)(const ModelDev<R>&, const BackwardArgs<R>&, LaunchCfg, cudaStream_t);
   cudaError_t (*adjoint)(const ModelDev<R>&, const AdjointArgs<R>&, LaunchCfg, cudaStream_t);
   cudaError_t (*field)(const ModelDev<R>&, const FieldArgs<R>&, LaunchCfg, cudaStream_t);
   cudaError_t (*invweight)(const ModelDev<R>&, const R*, const R*, R*, const WsLayout&, const RkLayout&, LaunchCfg, cudaStream_t);
@@ -32,7 +33,7 @@ template <class R> struct Launchers {
 };
 template <class R, int G, class SH> Launchers<R> make_launchers() {
   Launchers<R> l;
-  l.rollout = &launch_rollout<R, G, SH>; l.backward = &launch_backward<R, G, SH>; l.adjoint = &launch_adjoint<R, G, SH>; l.field = &launch_field<R, G, SH>;
+  l.rollout = &launch_rollout<R, G, SH>; l.backward = &launch_backward<R, G, SH>; l.adjoint = &launch_adjoint<R, G, SH>; l.backward_ckpt = &launch_backward_ckpt<R, G, SH>; l.field = &launch_field<R, G, SH>;
   l.invweight = &launch_invweight<R, G, SH>; l.occupancy = &kernel_occupancy<R, G, SH>; l.prof_dump = &launch_prof_dump<R, G, SH>;
   return l;
 }
@@ -318,6 +319,8 @@ template <class R> void build_dev(const HostModel& h, Arena& ar, ModelDev<R>& m,
 // ---- the model object -------------------------------------------------------------------------------------
 struct dmx_model {
   int precision, G, shape = 0, sm_count, max_smem, tape_stages = 1;
+  int stride = 1;                  // checkpoint stride of the tape (dmx_model_set_checkpoint_stride)
+  void* seg_scratch = nullptr;     // stride > 1: segment buffers of the reverse sweep, [resident groups][stride][seg record]
   int fwd_rk_global = 0;           // forward integrator arrays in global memory (like the reverse sweep's) instead of shared memory
   void* rk_scratch_fwd = nullptr;
   HostModel h;
@@ -366,14 +369,25 @@ int alloc_scratch(dmx_model* m) {
 
 // ---- tape geometry ---------------------------------------------------------------------------------------------
 size_t align_up(size_t b, size_t a) { return (b + a - 1) / a * a; }
+size_t record_bytes(const dmx_model* m);
 size_t tape_header_bytes(int nenv) { return 256 + align_up((size_t)nenv * 2 * sizeof(int), 256); }
 template <class R> void tape_geometry(const dmx_model* m, TapeView<R>& tp) {
   const int per16 = 16 / (int)sizeof(R), per8 = 8 / (int)sizeof(R), nx = m->h.nq + m->h.nv;
   tp.o_th = (nx + per16 - 1) / per16 * per16;
-  int o = tp.o_th + 2 * per8;
-  tp.o_A = m->tape_stages ? o : -1;
-  if (m->tape_stages) o += 6 * m->h.nv;
-  tp.rec = (o + per16 - 1) / per16 * per16;
+  const int o = tp.o_th + 2 * per8;
+  const int rec_plain = (o + per16 - 1) / per16 * per16, rec_rates = (o + 6 * m->h.nv + per16 - 1) / per16 * per16;
+  tp.stride = m->stride;
+  const int rec_k1 = (o + m->h.nv + per16 - 1) / per16 * per16;
+  const bool rates = m->tape_stages && m->stride == 1;        // a strided tape keeps checkpoints with the first-stage rate only (the
+  tp.o_A = (rates || m->stride > 1) ? o : -1;                 // FSAL value the forward pass used); the segment buffer holds all six
+  tp.rec = rates ? rec_rates : (m->stride > 1 ? rec_k1 : rec_plain);
+  tp.seg_rec = rec_rates; tp.seg_oA = o;
+}
+// bytes of a tape that holds `steps` accepted steps in total for nenv environments (without the header)
+size_t tape_payload_bytes(const dmx_model* m, int nenv, long long steps) {
+  const size_t rb = record_bytes(m);
+  if (m->stride == 1) return (size_t)steps * rb;
+  return align_up((size_t)steps * sizeof(double), 16) + ((size_t)(steps / m->stride) + (size_t)nenv) * rb;
 }
 size_t record_bytes(const dmx_model* m) {
   if (m->precision == 64) { TapeView<double> t; tape_geometry(m, t); return (size_t)t.rec * 8; }
@@ -387,13 +401,24 @@ template <class R> int bind_tape(const dmx_model* m, int nenv, void* tape, size_
     size_t a4 = align_up((size_t)nenv * sizeof(int), 256);
     pl.order = (const int*)(b + 256); pl.cap = (const int*)(b + 256 + a4); pl.offset = (const long long*)(b + 256 + 2 * a4);
   }
-  tp.meta = nullptr; tp.hdr = nullptr; tp.data = nullptr; tp.capacity = 0; tp.uniform_cap = 0;
+  tp.meta = nullptr; tp.hdr = nullptr; tp.data = nullptr; tp.sched = nullptr; tp.capacity = 0; tp.uniform_cap = 0;
   if (!tape) return 0;
   size_t hdr = tape_header_bytes(nenv), rb = (size_t)tp.rec * sizeof(R);
-  if (tape_bytes < hdr + (plan ? rb : (size_t)nenv * rb)) return fail("tape too small");
+  if (tape_bytes < hdr + tape_payload_bytes(m, nenv, plan ? 1 : nenv)) return fail("tape too small");
   if (((size_t)tape & 15) != 0) return fail("tape must be 16-byte aligned");
-  tp.meta = (int*)tape; tp.hdr = (int*)((unsigned char*)tape + 256); tp.data = (R*)((unsigned char*)tape + hdr);
-  tp.capacity = (long long)((tape_bytes - hdr) / rb);
+  tp.meta = (int*)tape; tp.hdr = (int*)((unsigned char*)tape + 256);
+  const size_t avail = tape_bytes - hdr;
+  if (m->stride == 1) {
+    tp.sched = nullptr; tp.data = (R*)((unsigned char*)tape + hdr);
+    tp.capacity = (long long)(avail / rb);
+  } else {                        // [schedule: capacity doubles | checkpoints: capacity / stride + nenv records]
+    long long cap = (long long)(((avail - (size_t)nenv * rb) * (size_t)m->stride) / (8 * (size_t)m->stride + rb));
+    while (cap > 0 && tape_payload_bytes(m, nenv, cap) > avail) --cap;
+    while (tape_payload_bytes(m, nenv, cap + 1) <= avail) ++cap;          // the estimate floors steps / stride: it can be a few steps short
+    tp.capacity = cap;
+    tp.sched = (double*)((unsigned char*)tape + hdr);
+    tp.data = (R*)((unsigned char*)tape + hdr + align_up((size_t)cap * sizeof(double), 16));
+  }
   tp.uniform_cap = (int)std::min<long long>(tp.capacity / nenv, (long long)1 << 30);
   return 0;
 }
@@ -540,9 +565,13 @@ int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const vo
   CUDA_OK(cudaMemsetAsync(a.queue, 0, sizeof(int), s));
   if (dLdctrl && nknot > 0 && m->h.nu > 0) CUDA_OK(cudaMemsetAsync(dLdctrl, 0, (size_t)nenv * nknot * m->h.nu * sizeof(R), s));
   ModelDev<R> md = dev_of<R>(m); md.arena_smem = m->cb.arena;
+  if (adj && m->stride > 1) return fail("the continuous adjoint needs a tape with checkpoint stride 1");
   if (adj) {                       // optimize-then-discretize: same arguments plus the options of the backward solve
     aa.sa = opts_of(adj); aa.info = adj_info; aa.replay = adj_replay; aa.n_replay = adj_replay ? n_adj_replay : 0;
     CUDA_OK(launchers_for<R>(m->G, m->shape).adjoint(md, aa, c, s));
+  } else if (m->stride > 1) {
+    a.seg_scratch = (R*)m->seg_scratch;
+    CUDA_OK(launchers_for<R>(m->G, m->shape).backward_ckpt(md, a, c, s));
   } else CUDA_OK(launchers_for<R>(m->G, m->shape).backward(md, a, c, s));
   CUDA_OK(cudaEventRecord(m->bwd_done, s));
   return 0;
@@ -650,6 +679,7 @@ void dmx_model_destroy(dmx_model* m) {
   if (m->zero_u) cudaFree(m->zero_u);
   if (m->rk_scratch) cudaFree(m->rk_scratch);
   if (m->rk_scratch_fwd) cudaFree(m->rk_scratch_fwd);
+  if (m->seg_scratch) cudaFree(m->seg_scratch);
   if (m->bwd_done) cudaEventDestroy(m->bwd_done);
   delete m;
 }
@@ -657,6 +687,20 @@ void dmx_model_destroy(dmx_model* m) {
 int dmx_model_set_tape_stages(dmx_model* m, int on) {
   if (!m) return fail("null model");
   m->tape_stages = on ? 1 : 0;
+  return 0;
+}
+int dmx_model_set_checkpoint_stride(dmx_model* m, int k) {
+  if (!m) return fail("null model");
+  if (k < 1 || k > 65536) return fail("checkpoint stride must be in [1, 65536]");
+  CUDA_OK(cudaDeviceSynchronize());                       // set-up call: no sweep may still use the old buffers
+  if (m->seg_scratch) { cudaFree(m->seg_scratch); m->seg_scratch = nullptr; }
+  m->stride = k;
+  if (k > 1) {
+    size_t groups = (size_t)m->cb.occ * m->sm_count * groups_per_block(m, m->cb.block), seg_rec;
+    if (m->precision == 64) { TapeView<double> t; tape_geometry(m, t); seg_rec = (size_t)t.seg_rec * 8; }
+    else { TapeView<float> t; tape_geometry(m, t); seg_rec = (size_t)t.seg_rec * 4; }
+    CUDA_OK(cudaMalloc(&m->seg_scratch, groups * (size_t)k * seg_rec));
+  }
   return 0;
 }
 int dmx_model_np(const dmx_model* m) { return m ? m->h.np : -1; }
@@ -670,11 +714,11 @@ int dmx_model_default_params(const dmx_model* m, double* p_host) {
 
 size_t dmx_tape_bytes(const dmx_model* m, int nenv, int tape_steps) {
   if (!m || nenv <= 0 || tape_steps <= 0) return 0;
-  return tape_header_bytes(nenv) + (size_t)nenv * (size_t)tape_steps * record_bytes(m);
+  return tape_header_bytes(nenv) + tape_payload_bytes(m, nenv, (long long)nenv * tape_steps);
 }
 size_t dmx_tape_bytes_records(const dmx_model* m, int nenv, long long total_records) {
   if (!m || nenv <= 0 || total_records <= 0) return 0;
-  return tape_header_bytes(nenv) + (size_t)total_records * record_bytes(m);
+  return tape_header_bytes(nenv) + tape_payload_bytes(m, nenv, total_records);
 }
 size_t dmx_plan_bytes(int nenv) {
   if (nenv <= 0) return 0;
@@ -843,6 +887,7 @@ int backward_noalloc_typed(const dmx_model* m, int nenv, const void* ctrl, int n
   size_t groups = (size_t)c.grid * gpb;
   if (m->G == 1) groups = (groups + 31) / 32 * 32;
   const size_t need = 256 + groups * (size_t)m->rl.size_bwd * sizeof(double);
+  if (m->stride > 1) return fail("dmx_rollout_backward_noalloc needs a tape with checkpoint stride 1");
   if (need > (size_t)DMX_NOALLOC_SCRATCH_BYTES) {
     std::snprintf(g_err, sizeof(g_err), "dmx_rollout_backward_noalloc: nenv = %d needs %zu bytes of scratch, the static array holds %u "
                   "(DMX_NOALLOC_SCRATCH_BYTES); use dmx_rollout_backward or a smaller batch", nenv, need, (unsigned)DMX_NOALLOC_SCRATCH_BYTES);

@@ -17,6 +17,12 @@ template <class R, int G, class SH> cudaError_t launch_backward(const ModelDev<R
   backward_kernel<R, G, SH><<<c.grid, c.block, c.smem, s>>>(m, a);
   return cudaGetLastError();
 }
+template <class R, int G, class SH> cudaError_t launch_backward_ckpt(const ModelDev<R>& m, const BackwardArgs<R>& a, LaunchCfg c, cudaStream_t s) {
+  cudaError_t e = cudaFuncSetAttribute(backward_kernel<R, G, SH, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
+  if (e != cudaSuccess) return e;
+  backward_kernel<R, G, SH, true><<<c.grid, c.block, c.smem, s>>>(m, a);
+  return cudaGetLastError();
+}
 template <class R, int G, class SH> cudaError_t launch_adjoint(const ModelDev<R>& m, const AdjointArgs<R>& a, LaunchCfg c, cudaStream_t s) {
   cudaError_t e = cudaFuncSetAttribute(adjoint_kernel<R, G, SH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem);
   if (e != cudaSuccess) return e;
@@ -59,6 +65,7 @@ template <class R, int G, class SH> cudaError_t kernel_occupancy(int block, size
 #define DMX_INSTANTIATE(R, G, SH)                                                                                                  \
   template cudaError_t dmx::launch_rollout<R, G, dmx::SH>(const dmx::ModelDev<R>&, const dmx::RolloutArgs<R>&, dmx::LaunchCfg, cudaStream_t);   \
   template cudaError_t dmx::launch_backward<R, G, dmx::SH>(const dmx::ModelDev<R>&, const dmx::BackwardArgs<R>&, dmx::LaunchCfg, cudaStream_t); \
+  template cudaError_t dmx::launch_backward_ckpt<R, G, dmx::SH>(const dmx::ModelDev<R>&, const dmx::BackwardArgs<R>&, dmx::LaunchCfg, cudaStream_t); \
   template cudaError_t dmx::launch_adjoint<R, G, dmx::SH>(const dmx::ModelDev<R>&, const dmx::AdjointArgs<R>&, dmx::LaunchCfg, cudaStream_t); \
   template cudaError_t dmx::launch_field<R, G, dmx::SH>(const dmx::ModelDev<R>&, const dmx::FieldArgs<R>&, dmx::LaunchCfg, cudaStream_t);       \
   template cudaError_t dmx::launch_invweight<R, G, dmx::SH>(const dmx::ModelDev<R>&, const R*, const R*, R*, const dmx::WsLayout&,             \

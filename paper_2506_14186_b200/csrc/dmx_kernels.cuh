@@ -63,11 +63,15 @@ template <class R> struct BackwardArgs {
   TapeView<R> tp; PlanView pl;
   int* queue;
   double* rk_scratch;       // integrator / adjoint arrays of every resident group (global memory: touched once per stage)
+  R* seg_scratch;           // checkpoint stride > 1: [resident groups][stride][seg_rec] segment buffers
   WsLayout wl; RkLayout rl;
 };
 
 // ---- S10: reverse sweep over the tape, frozen step sizes ---------------------------
-template <class R, int G, class SH>
+// CKPT: the tape holds a checkpoint every a.tp.stride steps and the step schedule (TapeView); the sweep re-runs each
+// segment forward from its checkpoint (same stages, same FSAL rule as rollout_kernel, step sizes from the schedule)
+// into this group's buffer of `stride` full records, then sweeps the buffer exactly as it would sweep a full tape.
+template <class R, int G, class SH, bool CKPT = false>
 __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ BackwardArgs<R> a) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
@@ -85,7 +89,11 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
   const int nknot = has_ctrl ? a.nknot : 0;
   // the tape must be the one a rollout of this model wrote for this batch, record layout and plan
   const bool tape_ok = a.tp.meta[0] == TAPE_MAGIC && a.tp.meta[1] == a.nenv && a.tp.meta[2] == rec && a.tp.meta[3] == a.tp.o_A &&
-                       a.tp.meta[4] == (a.pl.offset ? 1 : 0);
+                       a.tp.meta[4] == (a.pl.offset ? 1 : 0) && a.tp.meta[5] == a.tp.stride && (CKPT == (a.tp.stride > 1));
+  const int stride = CKPT ? a.tp.stride : 1, srec = CKPT ? a.tp.seg_rec : rec, o_A = CKPT ? a.tp.seg_oA : a.tp.o_A;
+  R* segbuf = nullptr;
+  if (CKPT) segbuf = a.seg_scratch + ((size_t)blockIdx.x * (G == 1 ? blockDim.x : blockDim.x / G) + (G == 1 ? threadIdx.x : threadIdx.x / G)) * (size_t)stride * srec;
+  const bool restore = CKPT || a.tape_stages != 0;
 #pragma unroll 1
   for (;;) {
     int e = 0;
@@ -121,7 +129,45 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
     }
 #pragma unroll 1
     for (int n = N - 1; n >= 0 && good; --n) {
-      const R* r = a.tp.data + ((size_t)first + n) * rec;
+      if (CKPT && (n == N - 1 || (n + 1) % stride == 0)) {       // first visit of segment n / stride: re-run it forward
+        const int s0 = (n / stride) * stride;
+        const double* sch = a.tp.sched + first;
+        int kj = knot;                                            // knot in effect after step n; minus the intervals ended inside
+#pragma unroll 1
+        for (int j = s0; j <= n; ++j) if (sch[j] < 0) --kj;
+        const R* c = a.tp.data + ((size_t)(first / stride + e) + n / stride) * rec;
+#pragma unroll 1
+        for (int j = gr.lane; j < nq; j += G) rk.q()[j] = (double)c[j];
+#pragma unroll 1
+        for (int j = gr.lane; j < nv; j += G) rk.v()[j] = (double)c[nq + j];
+        // the forward pass reused the previous step's last stage as A_1 here (FSAL) unless that step ended a control
+        // interval (or this is the first step): take the taped A_1 in the first case, evaluate afresh in the second
+        bool have_k1 = s0 > 0 && !(sch[s0 - 1] < 0);
+        if (have_k1) for (int j = gr.lane; j < nv; j += G) rk.A()[j] = (double)c[a.tp.o_A + j];
+        gr.sync();
+#pragma unroll 1
+        for (int j = s0; j <= n && good; ++j) {
+          const double hsj = sch[j];
+          const R* uj = has_ctrl ? a.ctrl + ((size_t)e * nknot + kj) * nu : a.zero_u;
+          bool okf; int uncf;
+          rk_attempt<R, G, SH, false>(m, tab, rk, Yqr, Vr, uj, p, fabs(hsj), have_k1, ws, okf, uncf, gr);
+          if (!okf) { good = false; break; }
+          R* w = segbuf + (size_t)(j - s0) * srec;
+          const int nchunk = srec * (int)sizeof(R) / 16;
+#pragma unroll 1
+          for (int ch = gr.lane; ch < nchunk; ch += G) tape_store_chunk(w, ch, rk, nq, nx, a.tp.o_th, o_A, 6 * nv, 0.0, hsj);
+          gr.sync();
+#pragma unroll 1
+          for (int i = gr.lane; i < nq; i += G) rk.q()[i] = rk.Yq()[i];
+#pragma unroll 1
+          for (int i = gr.lane; i < nv; i += G) rk.v()[i] = rk.V()[i];
+          if (hsj < 0) { ++kj; have_k1 = false; }                 // the step ended a control interval: the FSAL stage is stale
+          else { have_k1 = true; for (int i = gr.lane; i < nv; i += G) rk.A()[i] = rk.A()[6 * nv + i]; }
+          gr.sync();
+        }
+        if (!good) break;
+      }
+      const R* r = CKPT ? segbuf + (size_t)(n % stride) * srec : a.tp.data + ((size_t)first + n) * rec;
 #pragma unroll 1
       for (int j = gr.lane; j < nq; j += G) rk.q()[j] = (double)r[j];
 #pragma unroll 1
@@ -130,11 +176,11 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
       const double h = fabs(hs);
       if (hs < 0) knot--;
       const R* u = has_ctrl ? a.ctrl + ((size_t)e * nknot + knot) * nu : a.zero_u;
-      if (a.tape_stages) for (int j = gr.lane; j < 6 * nv; j += G) rk.A()[j] = (double)r[a.tp.o_A + j];
+      if (restore) for (int j = gr.lane; j < 6 * nv; j += G) rk.A()[j] = (double)r[o_A + j];
       gr.sync();
       bool ok; int unc;
       // stage states: recomputed with F from the checkpoint, or rebuilt from the taped stage rates
-      rk_attempt<R, G, SH, true>(m, tab, rk, Yqr, Vr, u, p, h, false, ws, ok, unc, gr, a.tape_stages != 0, work);
+      rk_attempt<R, G, SH, true>(m, tab, rk, Yqr, Vr, u, p, h, false, ws, ok, unc, gr, restore, work);
       // y_{n+1} = (q_n (+) h sum b_i K_i, v_n + h sum b_i A_i), b = row 6 of a
 #pragma unroll 1
       for (int j = gr.lane; j < nv; j += G) {
@@ -164,7 +210,7 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
         gr.sync();
         // A_i = F(Y_i), or F~ for the straight-through estimator (Eq. 4)
         if (!vjp_stage<R, G, SH>(m, Yqr, Vr, u, p, rk.Ab().at(i * nv), a.cfd != 0, a.want_p != 0, ws, rk, gr, a.dbg,
-                              (a.tape_stages && !a.cfd) ? rk.A().at(i * nv).p : nullptr, &n_unc, work)) { good = false; break; }   // F: x* = taped A_i
+                              (restore && !a.cfd) ? rk.A().at(i * nv).p : nullptr, &n_unc, work)) { good = false; break; }   // F: x* = taped A_i
 #pragma unroll 1
         for (int j = gr.lane; j < nv; j += G) rk.Vb()[j] += rk.vbar()[j];
         if (a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nu; c += G) a.dLdctrl[((size_t)e * nknot + knot) * nu + c] += (R)rk.ubar()[c];
@@ -308,6 +354,7 @@ struct LaunchCfg { int block, grid; size_t smem; };
 
 template <class R, int G, class SH> cudaError_t launch_rollout(const ModelDev<R>& m, const RolloutArgs<R>& a, LaunchCfg c, cudaStream_t s);
 template <class R, int G, class SH> cudaError_t launch_backward(const ModelDev<R>& m, const BackwardArgs<R>& a, LaunchCfg c, cudaStream_t s);
+template <class R, int G, class SH> cudaError_t launch_backward_ckpt(const ModelDev<R>& m, const BackwardArgs<R>& a, LaunchCfg c, cudaStream_t s);
 template <class R, int G, class SH> cudaError_t launch_field(const ModelDev<R>& m, const FieldArgs<R>& a, LaunchCfg c, cudaStream_t s);
 template <class R, int G, class SH> cudaError_t launch_invweight(const ModelDev<R>& m, const R* qpos0, const R* zero_v, R* body_w, const WsLayout& wl,
                                                                  const RkLayout& rl, LaunchCfg c, cudaStream_t s);

@@ -219,12 +219,21 @@ DMX_DN double error_norm(const ModelDev<R>& m, const Rk<ST>& rk, double rtol, do
 // Environment e owns records [offset(e), offset(e) + cap(e)): uniform (e * cap) or, with a plan (dmx_tape_plan), the
 // prefix sum of per-environment capacities sized from a previous pass, so that one long environment does not size
 // every slot ("memory = number of checkpoints x state size").
+// Checkpoint stride k > 1 (dmx_model_set_checkpoint_stride; PAPER.md:371-375 "number of checkpoints", :431): a full
+// record is kept only for the accepted steps n = 0, k, 2k, ... (record ckpt(e, n/k): y_n, t_n, h_n and the first-stage rate
+// A_1, which is the FSAL value the forward pass used there unless the previous step ended a control interval) and every step
+// keeps its signed step size in the schedule sched[first + n] (8 bytes); the reverse sweep re-runs a segment forward from
+// its checkpoint into a per-group buffer of k full records and then sweeps it.  Checkpoint records of environment e start
+// at record floor(first / k) + e, which leaves every environment ceil(cap / k) records.
 enum { TAPE_MAGIC = 0x646d7832, TAPE_META_INTS = 64 };
 template <class R> struct TapeView {
   int rec, o_th, o_A;          // reals per record; offsets of (t, h) and of the stage rates (o_A < 0: not taped)
   int uniform_cap;             // records per environment without a plan
-  long long capacity;          // records the buffer holds
-  int* meta;                   // [TAPE_META_INTS]: magic, nenv, rec, o_A, planned
+  int stride;                  // 1: a record per accepted step; k > 1: a checkpoint every k steps + the schedule
+  int seg_rec, seg_oA;         // stride > 1: geometry of the records (with stage rates) of the sweep's segment buffer
+  double* sched;               // stride > 1: [capacity] signed step sizes
+  long long capacity;          // accepted steps the buffer holds
+  int* meta;                   // [TAPE_META_INTS]: magic, nenv, rec, o_A, planned, stride
   int* hdr;                    // [nenv*2]: accepted steps on tape, final knot (-1-knot: failed)
   R* data;
 };
@@ -368,6 +377,7 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
   const int nknot = has_ctrl ? a.nknot : 0;
   if (a.want_tape && blockIdx.x == 0 && threadIdx.x == 0) {   // what this tape holds; checked by the reverse sweep
     a.tp.meta[0] = TAPE_MAGIC; a.tp.meta[1] = a.nenv; a.tp.meta[2] = rec; a.tp.meta[3] = a.tp.o_A; a.tp.meta[4] = a.pl.offset ? 1 : 0;
+    a.tp.meta[5] = a.tp.stride;
   }
 #pragma unroll 1
   for (;;) {
@@ -387,8 +397,12 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
     unsigned long long work[3] = {0, 0, 0};
     bool have_k1 = false, last_nonfinite = false;
     const double* hr = a.h_replay ? a.h_replay + (size_t)e * a.n_replay : nullptr;
-    R* tape = nullptr; int tape_cap = 0;
-    if (a.want_tape) { long long first; tape_slot(a.tp, a.pl, e, first, tape_cap); tape = a.tp.data + (size_t)first * rec; }
+    R* tape = nullptr; int tape_cap = 0; double* sched = nullptr;
+    if (a.want_tape) {
+      long long first; tape_slot(a.tp, a.pl, e, first, tape_cap);
+      if (a.tp.stride > 1) { tape = a.tp.data + (size_t)(first / a.tp.stride + e) * rec; sched = a.tp.sched + first; }
+      else tape = a.tp.data + (size_t)first * rec;
+    }
     while (t < a.horizon) {
       double tb = has_ctrl ? fmin((knot + 1) * a.knot_dt, a.horizon) : a.horizon;
       if (knot + 1 >= nknot) tb = a.horizon;
@@ -422,12 +436,13 @@ __global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ Mo
       } else if (!finite) { status = 3; break; }
       if (!accept) { n_rej++; continue; }
       bool knot_up = hits && tb < a.horizon;
-      if (tape) {   // S9: checkpoint record (y_n, t_n, +-h_n); a negative h marks a step that ends a control interval
-        R* r = tape + (size_t)n_acc * rec;
+      if (tape && (!sched || n_acc % a.tp.stride == 0)) {   // S9: checkpoint record (y_n, t_n, +-h_n); a negative h marks a step that ends a control interval
+        R* r = tape + (size_t)(sched ? n_acc / a.tp.stride : n_acc) * rec;
         const int nchunk = rec * (int)sizeof(R) / 16;
 #pragma unroll 1
-        for (int c = gr.lane; c < nchunk; c += G) tape_store_chunk(r, c, rk, nq, nx, a.tp.o_th, a.tp.o_A, 6 * nv, t, knot_up ? -h : h);
+        for (int c = gr.lane; c < nchunk; c += G) tape_store_chunk(r, c, rk, nq, nx, a.tp.o_th, a.tp.o_A, sched ? nv : 6 * nv, t, knot_up ? -h : h);
       }
+      if (sched && gr.lane == 0) sched[n_acc] = knot_up ? -h : h;
       gr.sync();
 #pragma unroll 1
       for (int j = gr.lane; j < nq; j += G) rk.q()[j] = rk.Yq()[j];

@@ -636,6 +636,62 @@ def test_gpu_chart_rate_keeps_order_five_on_a_tumbling_body(B, which):
     assert np.all(slopes > 4.7) and np.all(slopes < 5.6), (errs, slopes)
 
 
+# ---- checkpoint count knob ---------------------------------------------------------
+@pytest.mark.parametrize("cfg,cfd", [("C1", False), ("C2", True), ("C3", False), ("C5", False)])
+def test_checkpoint_stride_gives_the_gradients_of_the_full_tape(B, cfg, cfd):
+    """dmx_model_set_checkpoint_stride(k): the tape keeps every k-th accepted step + the 8-byte step schedule and the reverse
+    sweep re-runs each segment forward.  The re-run takes the same stages, FSAL rule and step sizes, so xT, stats and all
+    gradients must equal those of the full tape (k = 1) - asserted at 1e-12 relative, bitwise equality reported - for
+    strides that divide the step counts, do not, and exceed them; free-running and with a launch plan; tape bytes shrink."""
+    import torch
+    w = W.make(cfg, **SMALL[cfg])
+    nenv = w["nenv"]
+    m = B.Model(w["model"])
+    x0, ctrl = m.dev(w["x0"]), m.dev(w["ctrl"])
+    g = m.dev(np.random.default_rng(2).normal(size=w["x0"].shape))
+    st = m.alloc_stats(nenv)
+    m.rollout(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], stats=st)
+    na = st["n_accept"].clone(); nmax = int(na.max().item())
+    ref = m.rollout_grad(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], g, cfd, m.alloc_tape(nenv, nmax + 1), stats=st)
+    full_bytes = m.tape_bytes(nenv, nmax + 1)
+    assert (st["status"] == 0).all()
+    keys = [k for k in ("xT", "dLdx0", "dLdctrl", "dLdparams") if ref[k] is not None]
+    for k_stride, planned in ((4, False), (7, True), (16, False), (100000 // 2, False)):
+        m.set_checkpoint_stride(k_stride)
+        if planned:
+            plan, tape = m.plan(na, margin_pct=0, pad=1)
+        else:
+            plan, tape = None, m.alloc_tape(nenv, nmax + 1)
+        tape.fill_(0xAB)                                            # stale bytes must not matter
+        st2 = m.alloc_stats(nenv)
+        out = m.rollout_grad(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], g, cfd, tape, stats=st2, plan=plan)
+        assert (st2["status"] == 0).all() and torch.equal(st2["n_accept"], na)
+        bitwise = all(torch.equal(out[k], ref[k]) for k in keys)
+        worst = 0.0
+        for k in keys:
+            a, b = out[k].cpu().numpy().reshape(nenv, -1), ref[k].cpu().numpy().reshape(nenv, -1)
+            worst = max(worst, (np.abs(a - b).max(axis=1) / np.maximum(np.abs(b).max(axis=1), 1e-300)).max())
+        print("%s stride %d%s: tape %.3f MB (full %.3f MB), worst rel diff vs full tape %.1e, bitwise %s"
+              % (cfg, k_stride, " planned" if planned else "", tape.numel() / 1e6, full_bytes / 1e6, worst, bitwise))
+        assert torch.equal(out["xT"], ref["xT"]) and worst <= 1e-12
+        if k_stride <= 16 and not planned:
+            assert tape.numel() < full_bytes / min(k_stride, 3)
+    # a strided tape read with another stride (or by the k = 1 sweep) is rejected on the device: zero gradients
+    m.set_checkpoint_stride(4)
+    tape = m.alloc_tape(nenv, nmax + 1)
+    xT = m.rollout(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], tape=tape)
+    m.set_checkpoint_stride(1)
+    bad = m.rollout_backward(ctrl, w["nknot"], None, w["opts"], xT, g, cfd, tape)
+    assert (bad["dLdx0"] == 0).all()
+    # tape full is still reported per environment
+    m.set_checkpoint_stride(4)
+    st3 = m.alloc_stats(nenv)
+    m.rollout_grad(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], g, cfd, m.alloc_tape(nenv, max(nmax // 2, 1)), stats=st3)
+    s3 = st3["status"].cpu().numpy(); n3 = na.cpu().numpy()
+    assert ((s3 == 4) == (n3 > max(nmax // 2, 1))).all()
+    m.set_checkpoint_stride(1)
+
+
 # ---- optimize-then-discretize: the continuous adjoint with its own steps (PAPER.md:435-448, 462-477) ---------------------
 def _adjoint_case(name):
     if name == "billiard":                              # reduced billiard of Fig. 19: misses, CFD on
