@@ -94,20 +94,31 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
   R* segbuf = nullptr;
   if (CKPT) segbuf = a.seg_scratch + ((size_t)blockIdx.x * (G == 1 ? blockDim.x : blockDim.x / G) + (G == 1 ? threadIdx.x : threadIdx.x / G)) * (size_t)stride * srec;
   const bool restore = CKPT || a.tape_stages != 0;
+  // One pass of the loop = one segment of one environment (the whole tape when !CKPT).  With CKPT and lockstep on, the
+  // CTA alternates between two modes, all groups re-running their next segment, then all groups sweeping it, separated
+  // by mode_sync: otherwise groups in the forward code and groups in the VJP code would meet at every phase barrier and
+  // each interval would last as long as the longest phase of either (measured 3-4.6x on the whole sweep).
+  int e = 0, N = 0, knot = 0, n = -1, n_unc = 0, tape_cap = 0;
+  long long first = 0;
+  bool good = false, active = false, fresh = false;
+  const R* p = nullptr;
+  unsigned long long work[3] = {0, 0, 0};
 #pragma unroll 1
   for (;;) {
-    int e = 0;
-    if (gr.lane == 0) { e = atomicAdd(a.queue, 1); if (e < a.nenv && a.pl.order) e = a.pl.order[e]; }
-    e = gr.bcast_int(e);
-    if (e >= a.nenv) break;
-    const R* p = a.params ? a.params + (size_t)e * np : m.p_default;
-    const int N = a.tp.hdr[2 * e];
-    int knot = a.tp.hdr[2 * e + 1], n_unc = 0;
-    unsigned long long work[3] = {0, 0, 0};
-    long long first; int tape_cap;
-    tape_slot(a.tp, a.pl, e, first, tape_cap);
-    bool good = tape_ok && knot >= 0 && N <= tape_cap && (!a.status || a.status[e] == 0);
-    if (good) {
+    if (!active) {
+      if (gr.lane == 0) { e = atomicAdd(a.queue, 1); if (e < a.nenv && a.pl.order) e = a.pl.order[e]; }
+      e = gr.bcast_int(e);
+      if (e >= a.nenv) break;
+      p = a.params ? a.params + (size_t)e * np : m.p_default;
+      N = a.tp.hdr[2 * e];
+      knot = a.tp.hdr[2 * e + 1]; n_unc = 0;
+      work[0] = work[1] = work[2] = 0;
+      tape_slot(a.tp, a.pl, e, first, tape_cap);
+      good = tape_ok && knot >= 0 && N <= tape_cap && (!a.status || a.status[e] == 0);
+      n = N - 1; active = true; fresh = true;
+    }
+    if (good && fresh) {
+      fresh = false;
       // ambient gradient at x_T -> tangent cotangent: lam = E(q_T)^T g
       const R* xT = a.xT + (size_t)e * nx; const R* gT = a.dLdxT + (size_t)e * nx;
 #pragma unroll 1
@@ -127,10 +138,9 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
       for (int i = gr.lane; i < np; i += G) rk.gp()[i] = 0.0;
       gr.sync();
     }
-#pragma unroll 1
-    for (int n = N - 1; n >= 0 && good; --n) {
-      if (CKPT && (n == N - 1 || (n + 1) % stride == 0)) {       // first visit of segment n / stride: re-run it forward
-        const int s0 = (n / stride) * stride;
+    const int s0 = (CKPT && n >= 0) ? (n / stride) * stride : 0;
+    if (CKPT) {
+      if (good && n >= 0) {                                       // re-run segment n / stride forward from its checkpoint
         const double* sch = a.tp.sched + first;
         int kj = knot;                                            // knot in effect after step n; minus the intervals ended inside
 #pragma unroll 1
@@ -151,7 +161,7 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
           const R* uj = has_ctrl ? a.ctrl + ((size_t)e * nknot + kj) * nu : a.zero_u;
           bool okf; int uncf;
           rk_attempt<R, G, SH, false>(m, tab, rk, Yqr, Vr, uj, p, fabs(hsj), have_k1, ws, okf, uncf, gr);
-          if (!okf) { good = false; break; }
+          if (!okf) { good = false; break; }                      // cannot happen on a tape this model wrote
           R* w = segbuf + (size_t)(j - s0) * srec;
           const int nchunk = srec * (int)sizeof(R) / 16;
 #pragma unroll 1
@@ -165,8 +175,11 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
           else { have_k1 = true; for (int i = gr.lane; i < nv; i += G) rk.A()[i] = rk.A()[6 * nv + i]; }
           gr.sync();
         }
-        if (!good) break;
       }
+      mode_sync(false);
+    }
+#pragma unroll 1
+    for (; n >= s0 && good; --n) {
       const R* r = CKPT ? segbuf + (size_t)(n % stride) * srec : a.tp.data + ((size_t)first + n) * rec;
 #pragma unroll 1
       for (int j = gr.lane; j < nq; j += G) rk.q()[j] = (double)r[j];
@@ -231,15 +244,20 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
       for (int j = gr.lane; j < nv; j += G) { rk.lam()[j] = rk.qb()[j]; rk.lam()[nv + j] = rk.vb()[j]; }
       gr.sync();
     }
-    R* g0 = a.dLdx0 + (size_t)e * 2 * nv;
+    if (n < 0 || !good) {                                         // the environment is finished
+      R* g0 = a.dLdx0 + (size_t)e * 2 * nv;
 #pragma unroll 1
-    for (int j = gr.lane; j < 2 * nv; j += G) g0[j] = good ? (R)rk.lam()[j] : R(0);
-    if (a.dLdparams) for (int c = gr.lane; c < np; c += G) a.dLdparams[(size_t)e * np + c] = good ? (R)rk.gp()[c] : R(0);
-    if (!good && a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nknot * nu; c += G) a.dLdctrl[(size_t)e * nknot * nu + c] = R(0);
-    if (a.n_unconv && gr.lane == 0) a.n_unconv[e] = n_unc;
-    if (a.work && gr.lane == 0) { a.work[6 * (size_t)e + 3] = work[0]; a.work[6 * (size_t)e + 4] = work[1]; a.work[6 * (size_t)e + 5] = work[2]; }
-    gr.sync();
+      for (int j = gr.lane; j < 2 * nv; j += G) g0[j] = good ? (R)rk.lam()[j] : R(0);
+      if (a.dLdparams) for (int c = gr.lane; c < np; c += G) a.dLdparams[(size_t)e * np + c] = good ? (R)rk.gp()[c] : R(0);
+      if (!good && a.dLdctrl && has_ctrl) for (int c = gr.lane; c < nknot * nu; c += G) a.dLdctrl[(size_t)e * nknot * nu + c] = R(0);
+      if (a.n_unconv && gr.lane == 0) a.n_unconv[e] = n_unc;
+      if (a.work && gr.lane == 0) { a.work[6 * (size_t)e + 3] = work[0]; a.work[6 * (size_t)e + 4] = work[1]; a.work[6 * (size_t)e + 5] = work[2]; }
+      gr.sync();
+      active = false;
+    }
+    if (CKPT) mode_sync(false);
   }
+  if (CKPT) { while (!mode_sync(true)) {} return; }
   phase_drain();
 }
 

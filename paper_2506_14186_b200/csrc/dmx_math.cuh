@@ -45,6 +45,14 @@ DMX_DI int cta_barrier_and(int p) {
 }
 DMX_DI void phase_sync(int id) { if (g_lockstep & (1 << id)) cta_barrier_and(0); }   // g_lockstep: mask of synchronised phases
 DMX_DI void phase_drain() { if (g_lockstep) while (!cta_barrier_and(1)) {} }
+// A barrier between two modes of a CTA whose groups reach it after different numbers of phases: round one ends when every
+// group is waiting here (or is finished), round two tells whether all of them are finished.  A finished group keeps
+// calling mode_sync(true) until it returns true.
+DMX_DI bool mode_sync(bool finished) {
+  if (!g_lockstep) return true;
+  while (!cta_barrier_and(1)) {}
+  return cta_barrier_and(finished ? 1 : 0) != 0;
+}
 
 // the CTA's dynamic shared memory: per-group workspaces (and, optionally, the constant arena at its end)
 extern __shared__ __align__(16) unsigned char dyn_smem[];
