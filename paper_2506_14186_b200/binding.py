@@ -156,7 +156,7 @@ class Model:
         self.lanes = L.dmx_model_lanes(h)
 
     def __del__(self):
-        if getattr(self, "h", None):
+        if getattr(self, "h", None) and load is not None:      # at interpreter exit the module globals may be gone already
             load().dmx_model_destroy(self.h)
             self.h = None
 
