@@ -519,6 +519,26 @@ int pick_lanes(const HostModel& h) {
   return 32;
 }
 
+// A batch that fills fewer CTAs than the SMs can hold would leave SMs idle, or with one CTA where others have two, while
+// the kernel lasts as long as its busiest SM (C2 at 4096 environments: reverse sweep 128 CTAs of 32 lane groups on 148
+// SMs; forward 256 CTAs of 16 on 148 SMs).  Then launch one CTA per SM, of ceil(nenv / SMs) lane groups in whole warps, if
+// such a CTA fits (threads, shared memory); else one per resident slot.  Same resident groups, spread evenly, and every
+// CTA full (its warps share the fetched instructions).  DMX_BALANCE=0: off.
+void balance_block(const dmx_model* m, int nenv, const dmx_model::Cfg& cfg, size_t gbytes, int max_block, LaunchCfg& c) {
+  static const bool on = [] { const char* e = std::getenv("DMX_BALANCE"); return !(e && std::atoi(e) == 0); }();
+  const int slots = cfg.occ * m->sm_count, gpb = groups_per_block(m, cfg.block);
+  if (!on || nenv <= 0 || (nenv + gpb - 1) / gpb >= slots) return;
+  auto threads_for = [&](int groups) { return std::max(32, ((m->G == 1 ? groups : groups * m->G) + 31) / 32 * 32); };
+  auto smem_for = [&](int blk) { return ((groups_per_block(m, blk) * gbytes + 15) & ~size_t(15)) + (cfg.arena ? m->arena.host.size() : 0); };
+  int blk = threads_for((nenv + m->sm_count - 1) / m->sm_count);               // one CTA per SM
+  if (blk > max_block || smem_for(blk) > (size_t)m->max_smem - 2048) {
+    blk = threads_for((nenv + slots - 1) / slots);                             // one CTA per resident slot
+    if (blk >= cfg.block) return;
+  }
+  const int g = groups_per_block(m, blk);
+  c.block = blk; c.grid = (nenv + g - 1) / g; c.smem = smem_for(blk);
+}
+
 template <class R>
 int rollout_typed(const dmx_model* m, int nenv, const void* x0, const void* ctrl, int nknot, double knot_dt, const void* params, double horizon,
                   const dmx_solver_opts* opts, const double* h_replay, int n_replay, void* xT, const dmx_stats* st, void* tape, size_t tape_bytes,
@@ -536,6 +556,8 @@ int rollout_typed(const dmx_model* m, int nenv, const void* x0, const void* ctrl
   LaunchCfg c; c.block = m->cf.block; c.smem = m->cf.smem;
   int gpb = groups_per_block(m, c.block);
   c.grid = std::max(1, std::min(m->cf.occ * m->sm_count, (nenv + gpb - 1) / gpb));
+  { static const bool fb = [] { const char* e = std::getenv("DMX_BALANCE_FWD"); return e && std::atoi(e) != 0; }();   // measured on C2: 48 -> 51 ms, off
+    if (fb && !m->fwd_rk_global) balance_block(m, nenv, m->cf, group_bytes(m, 0), 128, c); }
   ModelDev<R> md = dev_of<R>(m); md.arena_smem = m->cf.arena;
   CUDA_OK(launchers_for<R>(m->G, m->shape).rollout(md, a, c, s));
   return 0;
@@ -560,6 +582,7 @@ int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const vo
   LaunchCfg c; c.block = m->cb.block; c.smem = m->cb.smem;
   int gpb = groups_per_block(m, c.block);
   c.grid = std::max(1, std::min(m->cb.occ * m->sm_count, (nenv + gpb - 1) / gpb));
+  balance_block(m, nenv, m->cb, group_bytes(m, 1), 256, c);
   a.rk_scratch = (double*)m->rk_scratch;
   CUDA_OK(cudaStreamWaitEvent(s, m->bwd_done, 0));          // the previous reverse sweep of this model (any stream) owns rk_scratch until it ends
   CUDA_OK(cudaMemsetAsync(a.queue, 0, sizeof(int), s));

@@ -356,8 +356,10 @@ __device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* con
 }
 
 // ---- forward rollout: persistent lane groups pulling environments from a global queue --------------
+// register cap: three CTAs per SM where shared memory allows three (16 and 32 lanes: 168 registers); with 1 or 8 lanes
+// shared memory allows two at most, and the cap of 255 removes the spills (C2 forward 49.5 -> 48 ms)
 template <class R, int G, class SH>
-__global__ void __launch_bounds__(128) rollout_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ RolloutArgs<R> a) {
+__global__ void __launch_bounds__(128, (G <= 8 ? 2 : 3)) rollout_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ RolloutArgs<R> a) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
   if (threadIdx.x == 0) g_lockstep = a.lockstep;
