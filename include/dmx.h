@@ -245,6 +245,19 @@ int dmx_vector_field(const dmx_model *m, int n, const void *x, const void *u, co
 int dmx_vjp_field(const dmx_model *m, int n, const void *x, const void *u, const void *params, const void *kappa,
                   int cfd, void *qbar, void *vbar, void *ubar, void *pbar, void *cuda_stream);
 
+/* Optimiser step of the paper's applications built on the gradients above (section 5.2: "Adam
+ * optimizer with a learning rate of 0.01", "gradient clipping"; PAPER.md:515 E.2: Adam with b1 = 0.5, b2 = 0.9, eps = 1e-6).
+ * For every row r of x[nrow][len] with active[r] != 0 (active may be null = all rows):
+ *     g_r <- g_r * min(1, clip / ||g_r||_2)      (clip <= 0: no clipping; g itself is not modified)
+ *     m <- b1 m + (1 - b1) g_r,   v <- b2 v + (1 - b2) g_r^2
+ *     x <- x - lr * (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps)          (Kingma & Ba 2015, bias-corrected)
+ * t >= 1 is the step counter of this update; mom1 / mom2 are the caller's moment buffers (zero before the first step).
+ * x, g, mom1, mom2: DEVICE [nrow][len] of precision 64 / 32 reals; active: DEVICE [nrow] bytes.  Enqueues one kernel
+ * on cuda_stream and returns; allocates nothing.  Returns 0, or -1 on bad arguments (dmx_last_error). */
+int dmx_adam_step(int precision, int nrow, int len, void *x, const void *g, void *mom1, void *mom2,
+                  const unsigned char *active, int t, double lr, double b1, double b2, double eps, double clip,
+                  void *cuda_stream);
+
 /* FP64 / FP32 FMA-chain microbenchmark used for the roofline denominator:
  * runs `iters` dependent-chain FMAs x 8 chains per thread on the whole chip and returns the
  * measured FLOP/s (2 per FMA) in *flops_per_s.  Synchronises. */

@@ -16,7 +16,7 @@ SYMBOLS = ["dmx_model_create", "dmx_model_destroy", "dmx_model_set_tape_stages",
            "dmx_model_lanes", "dmx_tape_bytes", "dmx_tape_bytes_records", "dmx_plan_bytes", "dmx_tape_plan",
            "dmx_rollout", "dmx_rollout_grad", "dmx_rollout_backward", "dmx_rollout_backward_adjoint", "dmx_rollout_grad_adjoint",
            "dmx_rollout_backward_noalloc", "dmx_noalloc_scratch_bytes",
-           "dmx_vector_field", "dmx_vjp_field", "dmx_fma_peak", "dmx_debug_counters", "dmx_last_error"]
+           "dmx_vector_field", "dmx_vjp_field", "dmx_adam_step", "dmx_fma_peak", "dmx_debug_counters", "dmx_last_error"]
 
 _pd, _pi = C.POINTER(C.c_double), C.POINTER(C.c_int)
 _INT_FIELDS = ["nbody", "njnt", "nq", "nv", "nu", "ngeom", "npair"]
@@ -88,6 +88,7 @@ def load():
                                                C.POINTER(Stats), vp, vp, i, vp, sz, vp, vp]
         L.dmx_vector_field.argtypes = [vp, i, vp, vp, vp, i, vp, vp, vp]
         L.dmx_vjp_field.argtypes = [vp, i, vp, vp, vp, vp, i, vp, vp, vp, vp, vp]
+        L.dmx_adam_step.argtypes = [i, i, i, vp, vp, vp, vp, vp, i, d, d, d, d, d, vp]
         L.dmx_fma_peak.argtypes = [i, i, _pd, _pd]
         L.dmx_debug_counters.argtypes = [vp, vp]
         _lib = L
@@ -121,6 +122,25 @@ def fma_peak(precision=64, iters=1 << 16):
     if load().dmx_fma_peak(int(precision), int(iters), C.byref(f), C.byref(ms)) != 0:
         raise RuntimeError("dmx_fma_peak: " + _err())
     return f.value, ms.value
+
+
+def adam_step(x, g, mom1, mom2, t, lr, b1=0.9, b2=0.999, eps=1e-8, clip=0.0, active=None, stream=None):
+    """dmx_adam_step: one clipped Adam update of every (active) row of x[nrow, ...] in place; t = 1, 2, ...."""
+    T = _torch()
+    nrow = x.shape[0]
+    ln = x.numel() // nrow
+    for a in (g, mom1, mom2):
+        if a.dtype != x.dtype or a.numel() != x.numel() or not a.is_contiguous():
+            raise ValueError("adam_step: g / mom1 / mom2 must be contiguous tensors of x's type and size")
+    if not x.is_contiguous() or x.dtype not in (T.float64, T.float32):
+        raise ValueError("adam_step: x must be a contiguous float64 / float32 tensor")
+    if active is not None and (active.dtype != T.uint8 or active.numel() != nrow):
+        raise ValueError("adam_step: active must be a uint8 tensor with one entry per row")
+    sp = stream.cuda_stream if stream is not None else T.cuda.current_stream(x.device).cuda_stream
+    rc = load().dmx_adam_step(64 if x.dtype == T.float64 else 32, int(nrow), int(ln), _ptr(x), _ptr(g), _ptr(mom1), _ptr(mom2), _ptr(active),
+                              int(t), float(lr), float(b1), float(b2), float(eps), float(clip), C.c_void_p(sp))
+    if rc != 0:
+        raise RuntimeError("dmx_adam_step: " + _err())
 
 
 class Model:

@@ -615,6 +615,31 @@ int field_typed(dmx_model* m, int n, const void* x, const void* u, const void* p
   return 0;
 }
 
+// Optimiser step of the paper's applications (PAPER.md:167 "Adam ... learning rate of 0.01", "gradient clipping"; :515 Adam
+// with b1 = 0.5, b2 = 0.9, eps = 1e-6): a warp per row; the row's gradient is scaled to norm <= clip, then the bias-corrected
+// Adam update (Kingma & Ba 2015).  Arithmetic in double for both storage types.
+template <class R>
+__global__ void adam_clip_kernel(int nrow, int len, R* x, const R* g, R* m1, R* m2, const unsigned char* active, double lr, double b1, double b2,
+                                 double eps, double clip, double c1, double c2) {
+  const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (row >= nrow || (active && !active[row])) return;
+  const size_t o = (size_t)row * len;
+  double scale = 1.0;
+  if (clip > 0) {
+    double ss = 0;
+    for (int j = lane; j < len; j += 32) { double gj = (double)g[o + j]; ss += gj * gj; }
+    for (int d = 16; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
+    const double nrm = sqrt(ss);
+    if (nrm > clip) scale = clip / nrm;
+  }
+  for (int j = lane; j < len; j += 32) {
+    const double gj = scale * (double)g[o + j];
+    const double a = b1 * (double)m1[o + j] + (1.0 - b1) * gj, b = b2 * (double)m2[o + j] + (1.0 - b2) * gj * gj;
+    m1[o + j] = (R)a; m2[o + j] = (R)b;
+    x[o + j] = (R)((double)x[o + j] - lr * (a / c1) / (sqrt(b / c2) + eps));
+  }
+}
+
 // FMA-chain microbenchmark: 8 independent chains per thread
 template <class T> __global__ void fma_chain_kernel(T* out, int iters, T a, T b) {
   T x0 = T(threadIdx.x), x1 = x0 + T(1), x2 = x0 + T(2), x3 = x0 + T(3), x4 = x0 + T(4), x5 = x0 + T(5), x6 = x0 + T(6), x7 = x0 + T(7);
@@ -858,6 +883,20 @@ int dmx_debug_counters(const dmx_model* m, unsigned long long* host32) {
   if (e == cudaSuccess) e = cudaMemcpy(host32, d, 32 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
   cudaFree(d);
   CUDA_OK(e);
+  return 0;
+}
+
+int dmx_adam_step(int precision, int nrow, int len, void* x, const void* g, void* mom1, void* mom2, const unsigned char* active, int t,
+                  double lr, double b1, double b2, double eps, double clip, void* cuda_stream) {
+  if (nrow <= 0 || len <= 0 || !x || !g || !mom1 || !mom2 || t < 1) return fail("bad argument");
+  if (precision != 64 && precision != 32) return fail("precision must be 64 or 32");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const int wpb = 4;                                          // a warp per row
+  const int grid = (nrow + wpb - 1) / wpb;
+  const double c1 = 1.0 - std::pow(b1, (double)t), c2 = 1.0 - std::pow(b2, (double)t);
+  if (precision == 64) adam_clip_kernel<double><<<grid, 32 * wpb, 0, s>>>(nrow, len, (double*)x, (const double*)g, (double*)mom1, (double*)mom2, active, lr, b1, b2, eps, clip, c1, c2);
+  else adam_clip_kernel<float><<<grid, 32 * wpb, 0, s>>>(nrow, len, (float*)x, (const float*)g, (float*)mom1, (float*)mom2, active, lr, b1, b2, eps, clip, c1, c2);
+  CUDA_OK(cudaGetLastError());
   return 0;
 }
 
