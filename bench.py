@@ -304,6 +304,37 @@ class Runner:
         }
 
 
+def mpc_row(torch, B, dev):
+    """one plan step of the gradient-based MPC of PAPER.md:167 (32 Adam iterations with clipping and keep-best,
+    paper_2506_14186_b200/apps.py) on the C2 batch: wall time between two device synchronisations, after a warm-up plan step
+    of 2 iterations."""
+    try:
+        from paper_2506_14186_b200 import apps
+        w = make_workload("C2", 0, 0)
+        m = B.Model(w["model"], precision=64, device=dev)
+        goal = torch.tensor([0.6, 0.0], dtype=m.dtype, device=dev)
+
+        def cost(xT):
+            e = xT[:, 2:4] - goal
+            g = torch.zeros_like(xT); g[:, 2:4] = 2 * e
+            return (e * e).sum(1), g
+        nenv = w["nenv"]
+        mpc = apps.MPC(m, nenv, w["nknot"], w["knot_dt"], w["opts"], cost, cfd=True, iters=2, lr=0.01, clip=1.0, execute=16)
+        x0, u0 = m.dev(w["x0"]), m.dev(w["ctrl"])
+        mpc.plan_step(x0, u0)                                    # warm-up (sizes the tape)
+        mpc.iters = 32
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        _, best, hist = mpc.plan_step(x0, u0)
+        torch.cuda.synchronize(); dt = time.perf_counter() - t0
+        steps = int(mpc.roll.stats["n_accept"].sum().item())
+        return {"workload": w["name"], "nenv": nenv, "iterations": 32, "horizon_knots": w["nknot"], "s_per_plan_step": dt,
+                "gradient_env_steps_per_s": 32 * steps / dt, "accepted_steps_last_rollout": steps,
+                "mean_cost_first_iterate": float(hist[0].mean().item()), "mean_cost_best_iterate": float(best.mean().item()),
+                "timing": "host wall clock around 32 x (dmx_rollout with tape, cost on the device, dmx_rollout_backward, dmx_adam_step), one status read-back per iteration"}
+    except Exception as ex:            # noqa: BLE001
+        return {"error": "%s: %s" % (type(ex).__name__, ex)}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -457,6 +488,8 @@ def main():
             except Exception as ex:            # noqa: BLE001 - a failing companion row must not lose the headline
                 per[key_] = {"error": "%s: %s" % (type(ex).__name__, ex)}
             torch.cuda.empty_cache()
+        if not want or "C2_mpc_plan_step" in want:
+            per["C2_mpc_plan_step"] = mpc_row(torch, B, dev)
         line["per_config"] = per
     print(json.dumps(line), flush=True)
     if world > 1: dist.destroy_process_group()
