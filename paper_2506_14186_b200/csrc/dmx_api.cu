@@ -577,7 +577,7 @@ int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const vo
   a.ctrl = (const R*)ctrl; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u; a.xT = (const R*)xT; a.dLdxT = (const R*)dLdxT;
   a.status = st ? st->status : nullptr; a.n_unconv = st ? st->n_newton_unconverged_bwd : nullptr; a.work = st ? st->work : nullptr;
   a.so = opts_of(opts); a.dLdx0 = (R*)dLdx0; a.dLdctrl = (R*)dLdctrl; a.dLdparams = (R*)dLdparams;
-  { const char* e = std::getenv("DMX_LOCKSTEP_BWD"); a.lockstep = e ? std::atoi(e) : 0x1ff; }          // backward: fetch-bound, phases in lockstep (measured 1.6-2.2x)
+  { const char* e = std::getenv("DMX_LOCKSTEP_BWD"); a.lockstep = e ? std::atoi(e) : 0x21; }   // backward: fetch-bound, CTA in lockstep (off: 3.4x slower on C2); a barrier before the F evaluation and one before the VJP phases of a stage do as well as one before each of the nine phases (-1..3 %)
   a.queue = next_queue(m); a.wl = m->wl; a.rl = m->rl;
   LaunchCfg c; c.block = m->cb.block; c.smem = m->cb.smem;
   int gpb = groups_per_block(m, c.block);
