@@ -637,16 +637,19 @@ def test_gpu_chart_rate_keeps_order_five_on_a_tumbling_body(B, which):
 
 
 # ---- checkpoint count knob ---------------------------------------------------------
-@pytest.mark.parametrize("cfg,cfd", [("C1", False), ("C2", True), ("C3", False), ("C5", False)])
-def test_checkpoint_stride_gives_the_gradients_of_the_full_tape(B, cfg, cfd):
+@pytest.mark.parametrize("cfg,cfd,precision", [("C1", False, 64), ("C2", True, 64), ("C3", False, 64), ("C3", False, 32), ("C4", True, 64), ("C5", False, 64)])
+def test_checkpoint_stride_gives_the_gradients_of_the_full_tape(B, cfg, cfd, precision):
     """dmx_model_set_checkpoint_stride(k): the tape keeps every k-th accepted step + the 8-byte step schedule and the reverse
     sweep re-runs each segment forward.  The re-run takes the same stages, FSAL rule and step sizes, so xT, stats and all
     gradients must equal those of the full tape (k = 1) - asserted at 1e-12 relative, bitwise equality reported - for
-    strides that divide the step counts, do not, and exceed them; free-running and with a launch plan; tape bytes shrink."""
+    strides that divide the step counts, do not, and exceed them; free-running and with a launch plan; tape bytes shrink.
+    With fp32 storage the forward outputs are still identical, the gradients agree as fp32 gradients do (see below)."""
     import torch
     w = W.make(cfg, **SMALL[cfg])
     nenv = w["nenv"]
-    m = B.Model(w["model"])
+    m = B.Model(w["model"], precision=precision)
+    if precision == 32:                       # free flight only (first touch-down of C3 is later than 0.1 s): fp32 gradients are well conditioned there
+        w["horizon"] = 0.1
     x0, ctrl = m.dev(w["x0"]), m.dev(w["ctrl"])
     g = m.dev(np.random.default_rng(2).normal(size=w["x0"].shape))
     st = m.alloc_stats(nenv)
@@ -667,13 +670,25 @@ def test_checkpoint_stride_gives_the_gradients_of_the_full_tape(B, cfg, cfd):
         out = m.rollout_grad(x0, ctrl, w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"], g, cfd, tape, stats=st2, plan=plan)
         assert (st2["status"] == 0).all() and torch.equal(st2["n_accept"], na)
         bitwise = all(torch.equal(out[k], ref[k]) for k in keys)
-        worst = 0.0
+        worst, per_env = 0.0, np.zeros(nenv)
         for k in keys:
             a, b = out[k].cpu().numpy().reshape(nenv, -1), ref[k].cpu().numpy().reshape(nenv, -1)
-            worst = max(worst, (np.abs(a - b).max(axis=1) / np.maximum(np.abs(b).max(axis=1), 1e-300)).max())
-        print("%s stride %d%s: tape %.3f MB (full %.3f MB), worst rel diff vs full tape %.1e, bitwise %s"
-              % (cfg, k_stride, " planned" if planned else "", tape.numel() / 1e6, full_bytes / 1e6, worst, bitwise))
-        assert torch.equal(out["xT"], ref["xT"]) and worst <= 1e-12
+            # fp32 in free flight: the parameter gradients are rounding noise around zero (1e-5), compare them absolutely
+            floor = 1e-300 if precision == 64 else (1.0 if k == "dLdparams" else 1e-3)
+            per_env = np.maximum(per_env, np.abs(a - b).max(axis=1) / np.maximum(np.abs(b).max(axis=1), floor))
+        worst = per_env.max()
+        print("%s fp%d stride %d%s: tape %.3f MB (full %.3f MB), worst rel diff vs full tape %.1e, bitwise %s"
+              % (cfg, precision, k_stride, " planned" if planned else "", tape.numel() / 1e6, full_bytes / 1e6, worst, bitwise))
+        assert torch.equal(out["xT"], ref["xT"])
+        if precision == 64:
+            assert worst <= 1e-12
+        else:
+            # fp32 storage: the full tape rounds every record to fp32 while the re-run carries the integrator's doubles on from
+            # the rounded checkpoint, so the two sweeps see states that differ by fp32 rounding: not bitwise.  Over the whole
+            # 0.6 s (impacts) the difference is that of fp32 gradients themselves (measured median 2e-3);
+            # here, in free flight, it stays at rounding level
+            print("   fp32: median per-environment difference %.1e, worst %.1e" % (np.median(per_env), worst))
+            assert worst < 1e-4
         if k_stride <= 16 and not planned:
             assert tape.numel() < full_bytes / min(k_stride, 3)
     # a strided tape read with another stride (or by the k = 1 sweep) is rejected on the device: zero gradients
