@@ -105,7 +105,7 @@ class Oracle:
         self.nc = L.orc_nc(self.h)
 
     def __del__(self):
-        if getattr(self, "h", None):
+        if getattr(self, "h", None) and lib is not None:        # module globals may be gone at interpreter exit
             lib().orc_model_destroy(self.h)
             self.h = None
 
