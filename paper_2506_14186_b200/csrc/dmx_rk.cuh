@@ -79,30 +79,41 @@ template <class R, class AD>
 DMX_DI void retract_pullback_joint(const ModelDev<R>& m, int jn, const AD& delta, const AD& Qbar, const AD& base, const AD& dbar) {
   int va = m.jnt_vadr[jn];
   if (m.jnt_type[jn] != JNT_FREE) { base[va] += Qbar[va]; dbar[va] += Qbar[va]; return; }
-  double d[3], qb[3];
-#pragma unroll 1
-  for (int c = 0; c < 3; ++c) { base[va + c] += Qbar[va + c]; dbar[va + c] += Qbar[va + c]; d[c] = delta[va + 3 + c]; qb[c] = Qbar[va + 3 + c]; }
+  // all operands are read before anything is written: in the reverse sweep they live in global memory, and loads issued
+  // back to back overlap their latencies (one round trip instead of one per component)
+  double d[3], qb[3], ql[3], bs[6], db[6];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { ql[c] = Qbar[va + c]; qb[c] = Qbar[va + 3 + c]; d[c] = delta[va + 3 + c]; }
+#pragma unroll
+  for (int c = 0; c < 6; ++c) { bs[c] = base[va + c]; db[c] = dbar[va + c]; }
   double A, B, C; rot_AB(d, A, B, C);
   // R qb = qb + A d x qb + B d x (d x qb);  Jr^T qb = qb + B d x qb + C d x (d x qb)   (K^T = -K)
   double k1[3], k2[3]; cross3(d, qb, k1); cross3(d, k1, k2);
-#pragma unroll 1
-  for (int c = 0; c < 3; ++c) { base[va + 3 + c] += qb[c] + A * k1[c] + B * k2[c]; dbar[va + 3 + c] += qb[c] + B * k1[c] + C * k2[c]; }
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    base[va + c] = bs[c] + ql[c]; dbar[va + c] = db[c] + ql[c];
+    base[va + 3 + c] = bs[3 + c] + (qb[c] + A * k1[c] + B * k2[c]); dbar[va + 3 + c] = db[3 + c] + (qb[c] + B * k1[c] + C * k2[c]);
+  }
 }
 // joint jn of: Vbar += (dK/dV)^T Kbar, dbar += (dK/dTheta)^T Kbar
 template <class R, class AD>
 DMX_DI void chart_pullback_joint(const ModelDev<R>& m, int jn, const AD& delta, const AD& V, const AD& Kbar, const AD& Vbar, const AD& dbar) {
   int va = m.jnt_vadr[jn];
   if (m.jnt_type[jn] != JNT_FREE) { Vbar[va] += Kbar[va]; return; }
-  double th[3], w[3], kb[3];
-#pragma unroll 1
-  for (int c = 0; c < 3; ++c) { Vbar[va + c] += Kbar[va + c]; th[c] = delta[va + 3 + c]; w[c] = V[va + 3 + c]; kb[c] = Kbar[va + 3 + c]; }
+  double th[3], w[3], kb[3], kl[3], vb[6], db[3];            // reads first, writes last (see retract_pullback_joint)
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { kl[c] = Kbar[va + c]; kb[c] = Kbar[va + 3 + c]; th[c] = delta[va + 3 + c]; w[c] = V[va + 3 + c]; db[c] = dbar[va + 3 + c]; }
+#pragma unroll
+  for (int c = 0; c < 6; ++c) vb[c] = Vbar[va + c];
   double t1[3], t2[3], tw[3], a[3], b[3], c3v[3];
   cross3(th, kb, t1); cross3(th, t1, t2);
-#pragma unroll 1
-  for (int c = 0; c < 3; ++c) Vbar[va + 3 + c] += kb[c] - 0.5 * t1[c] + t2[c] / 12.0;
   cross3(w, kb, a); cross3(th, w, tw); cross3(tw, kb, b); cross3(w, t1, c3v);
-#pragma unroll 1
-  for (int c = 0; c < 3; ++c) dbar[va + 3 + c] += 0.5 * a[c] + b[c] / 12.0 - c3v[c] / 12.0;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    Vbar[va + c] = vb[c] + kl[c];
+    Vbar[va + 3 + c] = vb[3 + c] + (kb[c] - 0.5 * t1[c] + t2[c] / 12.0);
+    dbar[va + 3 + c] = db[c] + (0.5 * a[c] + b[c] / 12.0 - c3v[c] / 12.0);
+  }
 }
 
 // ---- per-environment fp64 integrator state in the group's workspace ---------------------------------
