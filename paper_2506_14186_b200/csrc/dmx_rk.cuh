@@ -48,11 +48,13 @@ template <class R, class AD>
 DMX_DI void retract_joint(const ModelDev<R>& m, int jn, const AD& q, const AD& delta, const AD& V, const AD& qout, const AD& K) {
   int qa = m.jnt_qadr[jn], va = m.jnt_vadr[jn];
   if (m.jnt_type[jn] != JNT_FREE) { qout[qa] = q[qa] + delta[va]; K[va] = V[va]; return; }
-  double d[3], w[3], e[4], a[4], r[4];
-#pragma unroll 1
-  for (int c = 0; c < 3; ++c) { qout[qa + c] = q[qa + c] + delta[va + c]; K[va + c] = V[va + c]; d[c] = delta[va + 3 + c]; w[c] = V[va + 3 + c]; }
-#pragma unroll 1
+  double d[3], w[3], e[4], a[4], r[4], ql[3], dl[3], vl[3];     // reads first, writes last (see retract_pullback_joint)
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { ql[c] = q[qa + c]; dl[c] = delta[va + c]; vl[c] = V[va + c]; d[c] = delta[va + 3 + c]; w[c] = V[va + 3 + c]; }
+#pragma unroll
   for (int c = 0; c < 4; ++c) a[c] = q[qa + 3 + c];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { qout[qa + c] = ql[c] + dl[c]; K[va + c] = vl[c]; }
   rotvec_to_quat(d, e);
   r[0] = a[0] * e[0] - a[1] * e[1] - a[2] * e[2] - a[3] * e[3];
   r[1] = a[0] * e[1] + a[1] * e[0] + a[2] * e[3] - a[3] * e[2];
