@@ -23,13 +23,15 @@ class _TapedRollout:
         self.stats = model.alloc_stats(nenv)
 
     def forward(self, x, ctrl, nknot, knot_dt, params, horizon, opts):
-        while True:
+        for _ in range(8):                                    # at most 256x the initial tape
             xT = self.m.rollout(x, ctrl, nknot, knot_dt, params, horizon, opts, stats=self.stats, tape=self.tape)
             st = self.stats["status"]
             if not bool((st == TAPE_FULL).any().item()):
                 return xT, st
             self.tape_steps *= 2
+            self.tape = None                                  # release before the larger one is allocated
             self.tape = self.m.alloc_tape(self.nenv, self.tape_steps)
+        raise RuntimeError("tape of %d steps per environment still too small: set max_steps in the solver options" % self.tape_steps)
 
     def backward(self, ctrl, nknot, params, opts, xT, dLdxT, cfd, want_params):
         return self.m.rollout_backward(ctrl, nknot, params, opts, xT, dLdxT, cfd, self.tape, want_params=want_params,
