@@ -101,10 +101,11 @@ __global__ void __launch_bounds__(256) adjoint_kernel(const __grid_constant__ Mo
   const SolverOpts& sa = aa.sa;
   const bool tape_ok = a.tp.meta[0] == TAPE_MAGIC && a.tp.meta[1] == a.nenv && a.tp.meta[2] == rec && a.tp.meta[3] == a.tp.o_A &&
                        a.tp.meta[4] == (a.pl.offset ? 1 : 0) && a.tp.meta[5] == 1 && a.tp.stride == 1;
+  bool first_env = true;
 #pragma unroll 1
   for (;;) {
     int e = 0;
-    if (gr.lane == 0) { e = atomicAdd(a.queue, 1); if (e < a.nenv && a.pl.order) e = a.pl.order[e]; }
+    if (gr.lane == 0) e = next_env<G>(a.queue, a.pl.order, a.nenv, -1, first_env);
     e = gr.bcast_int(e);
     if (e >= a.nenv) break;
     const R* p = a.params ? a.params + (size_t)e * np : m.p_default;

@@ -539,6 +539,25 @@ void balance_block(const dmx_model* m, int nenv, const dmx_model::Cfg& cfg, size
   c.block = blk; c.grid = (nenv + g - 1) / g; c.smem = smem_for(blk);
 }
 
+// A batch between half of and all the lane groups one 256-thread CTA per SM can hold runs as a single wave without the
+// queue: k CTAs half filled with the head of the launch order, the others full (next_env in dmx_rk.cuh).  Returns k, or -1
+// when the launch keeps the queue (batch too small or too large, CTA does not fit, DMX_HETERO=0 / DMX_HETERO_FWD=0 /
+// DMX_HETERO_BWD=0).
+int single_wave(const dmx_model* m, int nenv, const dmx_model::Cfg& cfg, size_t gbytes, bool forward, LaunchCfg& c) {
+  static const int on = [] { const char* e = std::getenv("DMX_HETERO"); return e ? std::atoi(e) : 1; }();
+  static const int on_f = [] { const char* e = std::getenv("DMX_HETERO_FWD"); return e ? std::atoi(e) : 1; }();
+  static const int on_b = [] { const char* e = std::getenv("DMX_HETERO_BWD"); return e ? std::atoi(e) : 1; }();
+  if (!on || (forward ? !on_f : !on_b)) return -1;
+  if (forward && (m->G > 8 || m->fwd_rk_global)) return -1;          // the forward kernel admits 256 threads with 1 or 8 lanes only
+  const int blk = 256, g = groups_per_block(m, blk), half = g / 2, cap = m->sm_count * g;
+  if (half < 1 || nenv <= cap / 2 || nenv > cap) return -1;
+  const size_t smem = ((g * gbytes + 15) & ~size_t(15)) + (cfg.arena ? m->arena.host.size() : 0);
+  if (smem > (size_t)m->max_smem - 2048) return -1;
+  const int k = std::min(m->sm_count, (cap - nenv) / half);
+  c.block = blk; c.grid = m->sm_count; c.smem = smem;
+  return k;
+}
+
 template <class R>
 int rollout_typed(const dmx_model* m, int nenv, const void* x0, const void* ctrl, int nknot, double knot_dt, const void* params, double horizon,
                   const dmx_solver_opts* opts, const double* h_replay, int n_replay, void* xT, const dmx_stats* st, void* tape, size_t tape_bytes,
@@ -558,6 +577,7 @@ int rollout_typed(const dmx_model* m, int nenv, const void* x0, const void* ctrl
   c.grid = std::max(1, std::min(m->cf.occ * m->sm_count, (nenv + gpb - 1) / gpb));
   { static const bool fb = [] { const char* e = std::getenv("DMX_BALANCE_FWD"); return e && std::atoi(e) != 0; }();   // measured on C2: 48 -> 51 ms, off
     if (fb && !m->fwd_rk_global) balance_block(m, nenv, m->cf, group_bytes(m, 0), 128, c); }
+  a.n_light = single_wave(m, nenv, m->cf, group_bytes(m, 0), true, c);
   ModelDev<R> md = dev_of<R>(m); md.arena_smem = m->cf.arena;
   CUDA_OK(launchers_for<R>(m->G, m->shape).rollout(md, a, c, s));
   return 0;
@@ -583,6 +603,7 @@ int backward_typed(dmx_model* m, int nenv, const void* ctrl, int nknot, const vo
   int gpb = groups_per_block(m, c.block);
   c.grid = std::max(1, std::min(m->cb.occ * m->sm_count, (nenv + gpb - 1) / gpb));
   balance_block(m, nenv, m->cb, group_bytes(m, 1), 256, c);
+  a.n_light = adj ? -1 : single_wave(m, nenv, m->cb, group_bytes(m, 1), false, c);
   a.rk_scratch = (double*)m->rk_scratch;
   CUDA_OK(cudaStreamWaitEvent(s, m->bwd_done, 0));          // the previous reverse sweep of this model (any stream) owns rk_scratch until it ends
   CUDA_OK(cudaMemsetAsync(a.queue, 0, sizeof(int), s));
@@ -962,7 +983,7 @@ int backward_noalloc_typed(const dmx_model* m, int nenv, const void* ctrl, int n
   a.ctrl = (const R*)ctrl; a.params = (const R*)params; a.zero_u = (const R*)m->zero_u; a.xT = (const R*)xT; a.dLdxT = (const R*)dLdxT;
   a.status = st ? st->status : nullptr; a.n_unconv = st ? st->n_newton_unconverged_bwd : nullptr; a.work = st ? st->work : nullptr;
   a.so = opts_of(opts); a.dLdx0 = (R*)dLdx0; a.dLdctrl = (R*)dLdctrl; a.dLdparams = (R*)dLdparams;
-  a.lockstep = 0x1ff; a.wl = m->wl; a.rl = m->rl;
+  a.lockstep = 0x1ff; a.wl = m->wl; a.rl = m->rl; a.n_light = -1;      // the work queue, as before
   a.queue = (int*)base;                                   // what must start at zero: the work-queue counter
   a.rk_scratch = (double*)(base + 256);
   CUDA_OK(cudaMemsetAsync(base, 0, 256, s));

@@ -53,7 +53,7 @@ DMX_DN bool vjp_stage(const ModelDev<R>& m, const Arr<R, StrideOf<G>::value>& Yq
 }
 
 template <class R> struct BackwardArgs {
-  int nenv, nknot, want_p, cfd, dbg, lockstep, tape_stages;
+  int nenv, nknot, want_p, cfd, dbg, lockstep, tape_stages, n_light;   // n_light: see next_env (dmx_rk.cuh)
   const R *ctrl, *params, *zero_u, *xT, *dLdxT;
   const int* status;
   int* n_unconv;            // [nenv] or null: contact solves of the reverse sweep that did not converge
@@ -100,13 +100,13 @@ __global__ void __launch_bounds__(256) backward_kernel(const __grid_constant__ M
   // each interval would last as long as the longest phase of either (measured 3-4.6x on the whole sweep).
   int e = 0, N = 0, knot = 0, n = -1, n_unc = 0, tape_cap = 0;
   long long first = 0;
-  bool good = false, active = false, fresh = false;
+  bool good = false, active = false, fresh = false, first_env = true;
   const R* p = nullptr;
   unsigned long long work[3] = {0, 0, 0};
 #pragma unroll 1
   for (;;) {
     if (!active) {
-      if (gr.lane == 0) { e = atomicAdd(a.queue, 1); if (e < a.nenv && a.pl.order) e = a.pl.order[e]; }
+      if (gr.lane == 0) e = next_env<G>(a.queue, a.pl.order, a.nenv, a.n_light, first_env);
       e = gr.bcast_int(e);
       if (e >= a.nenv) break;
       p = a.params ? a.params + (size_t)e * np : m.p_default;

@@ -255,7 +255,7 @@ template <class R> struct TapeView {
 struct PlanView { const int* order; const int* cap; const long long* offset; };
 
 template <class R> struct RolloutArgs {
-  int nenv, nknot, n_replay, want_tape, lockstep;
+  int nenv, nknot, n_replay, want_tape, lockstep, n_light;   // n_light: see next_env
   const R *x0, *ctrl, *params, *zero_u;
   const double* h_replay;
   double knot_dt, horizon;
@@ -296,6 +296,24 @@ template <int ST> DMX_DI void tape_store_chunk(float* r, int c, const Rk<ST>& rk
   else { v.x = (float)tape_elem(rk, i, nq, nx, o_A, nA); v.y = (float)tape_elem(rk, i + 1, nq, nx, o_A, nA);
          v.z = (float)tape_elem(rk, i + 2, nq, nx, o_A, nA); v.w = (float)tape_elem(rk, i + 3, nq, nx, o_A, nA); }
   reinterpret_cast<float4*>(r)[c] = v;
+}
+// Next environment of a lane group (lane 0's value; the caller broadcasts it).  n_light < 0: the work queue, in launch
+// order.  n_light >= 0: a single wave with one CTA per SM and no queue - the first n_light CTAs are half filled with the head
+// of the launch order (the longest environments under a plan), the others are full: a launch lasts as long as its
+// slowest SM, an SM with half the groups steps its environments ~8-14 % faster, so the spare group slots of a batch that
+// does not fill the chip go next to the longest chains.  Which group runs an environment never
+// changes its result (batch independence is tested).
+template <int G> DMX_DI int next_env(int* queue, const int* order, int nenv, int n_light, bool& first) {
+  int e;
+  if (n_light < 0) e = atomicAdd(queue, 1);
+  else if (first) {
+    const int gpb = G == 1 ? blockDim.x : blockDim.x / G, gi = G == 1 ? threadIdx.x : threadIdx.x / G, half = gpb / 2, b = blockIdx.x;
+    if (b < n_light) e = gi < half ? b * half + gi : nenv;
+    else e = n_light * half + (b - n_light) * gpb + gi;
+  } else e = nenv;
+  first = false;
+  if (e < nenv && order) e = order[e];
+  return e;
 }
 template <class R> DMX_DI void tape_load_th(const R* r, int o_th, double& t, double& hs) {
   const double* d = reinterpret_cast<const double*>(r + o_th);
@@ -370,9 +388,10 @@ __device__ __noinline__ int field_eval(const R* u, const R* p, int cfd, int* con
 
 // ---- forward rollout: persistent lane groups pulling environments from a global queue --------------
 // register cap: three CTAs per SM where shared memory allows three (16 and 32 lanes: 168 registers); with 1 or 8 lanes
-// shared memory allows two at most, and the cap of 255 removes the spills (C2 forward 49.5 -> 48 ms)
+// shared memory allows two at most, and the cap of 255 removes the spills (C2 forward 49.5 -> 48 ms) and admits one CTA
+// of 256 threads per SM (the single-wave launch of next_env)
 template <class R, int G, class SH>
-__global__ void __launch_bounds__(128, (G <= 8 ? 2 : 3)) rollout_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ RolloutArgs<R> a) {
+__global__ void __launch_bounds__((G <= 8 ? 256 : 128), (G <= 8 ? 1 : 3)) rollout_kernel(const __grid_constant__ ModelDev<R> m_, const __grid_constant__ RolloutArgs<R> a) {
   unsigned char* smem = dyn_smem;
   CtaConst<R>& cc = cta_const<R>();
   if (threadIdx.x == 0) g_lockstep = a.lockstep;
@@ -394,10 +413,11 @@ __global__ void __launch_bounds__(128, (G <= 8 ? 2 : 3)) rollout_kernel(const __
     a.tp.meta[0] = TAPE_MAGIC; a.tp.meta[1] = a.nenv; a.tp.meta[2] = rec; a.tp.meta[3] = a.tp.o_A; a.tp.meta[4] = a.pl.offset ? 1 : 0;
     a.tp.meta[5] = a.tp.stride;
   }
+  bool first_env = true;
 #pragma unroll 1
   for (;;) {
     int e = 0;
-    if (gr.lane == 0) { e = atomicAdd(a.queue, 1); if (e < a.nenv && a.pl.order) e = a.pl.order[e]; }
+    if (gr.lane == 0) e = next_env<G>(a.queue, a.pl.order, a.nenv, a.n_light, first_env);
     e = gr.bcast_int(e);
     if (e >= a.nenv) break;
     const R* x0 = a.x0 + (size_t)e * nx;
