@@ -42,8 +42,8 @@ UNIT = "accepted env-steps/s (forward + reverse sweep)"
 # those captures, NOT measured in the run that prints them (a profiler cannot run inside a timed region); the JSON line
 # labels them as such, next to the live algorithmic fraction.  Key: config_dtype_nenv of the capture.
 NCU_EXECUTED = {
-    "C2_f64_4096": {"rollout_kernel_executed_frac": 0.0309, "backward_kernel_executed_frac": 0.0336,
-                    "rollout_kernel_dram_bytes": 5.665e+08, "backward_kernel_dram_bytes": 7.092e+08},
+    "C2_f64_4096": {"rollout_kernel_executed_frac": 0.0339, "backward_kernel_executed_frac": 0.0349,
+                    "rollout_kernel_dram_bytes": 5.701e+08, "backward_kernel_dram_bytes": 7.149e+08},
     "C3_f64_2048": {"rollout_kernel_executed_frac": 0.0108, "backward_kernel_executed_frac": 0.0097,
                     "rollout_kernel_dram_bytes": 3.224e+08, "backward_kernel_dram_bytes": 3.821e+08},
     "C5_f64_512": {"rollout_kernel_executed_frac": 0.0110, "backward_kernel_executed_frac": 0.0130,
