@@ -814,3 +814,34 @@ def test_rollout_and_noalloc_sweep_replay_from_a_cuda_graph(B):
         torch.cuda.synchronize()
         assert torch.equal(got["xT"], xT) and torch.equal(got["dLdx0"], out["dLdx0"]) and torch.equal(got["dLdctrl"], out["dLdctrl"])
         assert float(out["dLdctrl"].abs().max()) > 0
+
+
+# ---- single-wave launch (one 256-thread CTA per SM, the first CTAs half filled) ------------------------
+def test_single_wave_launch_gives_the_results_of_the_queue_launch(B):
+    """2500 C2 environments fall between half of and all the lane-group slots of the chip, so forward and reverse sweep take
+    the single-wave launch (no work queue); 45 environments take the queue.  Same inputs: the first 45 environments of the
+    large launch equal the small launch bit for bit, with a plan, without one, and with a checkpoint stride."""
+    import torch
+    n_big, n_small = 2500, 45
+    w = W.make("C2", nenv=n_big, horizon=0.06)
+    m = B.Model(w["model"])
+    x0, ctrl = m.dev(w["x0"]), m.dev(w["ctrl"])
+    g = m.dev(np.random.default_rng(6).normal(size=w["x0"].shape))
+    args = (w["nknot"], w["knot_dt"], None, w["horizon"], w["opts"])
+    st = m.alloc_stats(n_big)
+    m.rollout(x0, ctrl, *args, stats=st)
+    nmax = int(st["n_accept"].max().item())
+    small = m.rollout_grad(x0[:n_small].contiguous(), ctrl[:n_small].contiguous(), *args, g[:n_small].contiguous(), True, m.alloc_tape(n_small, nmax + 1))
+    for stride, planned in ((1, False), (1, True), (4, True)):
+        m.set_checkpoint_stride(stride)
+        if planned:
+            plan, tape = m.plan(st["n_accept"], margin_pct=0, pad=1)
+        else:
+            plan, tape = None, m.alloc_tape(n_big, nmax + 1)
+        st2 = m.alloc_stats(n_big)
+        big = m.rollout_grad(x0, ctrl, *args, g, True, tape, stats=st2, plan=plan)
+        assert (st2["status"] == 0).all() and torch.equal(st2["n_accept"], st["n_accept"])
+        for k in ("xT", "dLdx0", "dLdctrl"):
+            assert torch.equal(big[k][:n_small], small[k]), (stride, planned, k)
+        assert bool(torch.isfinite(big["dLdx0"]).all()) and float(big["dLdctrl"][-1].abs().max()) > 0      # the last environment was run too
+    m.set_checkpoint_stride(1)
